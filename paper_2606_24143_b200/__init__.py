@@ -1,0 +1,6 @@
+"""B200-native fused OPD loss (learner-side hot path of AsyncOPD, arxiv/paper_2606_24143).
+
+`paper_2606_24143_b200.opd`   — ctypes binding of the C-ABI library libopd.so (include/opd.h)
+`paper_2606_24143_b200.synth` — seeded synthetic workloads (no method arithmetic)
+`paper_2606_24143_b200.build` — nvcc build of csrc/ for sm_100a
+"""

@@ -1,0 +1,157 @@
+"""Seeded synthetic workloads for the fused OPD loss (shared by tests, bench.py and the oracle tests).
+
+This module only *generates inputs*: student hidden states and head, an independent teacher
+head, a stale ("old") student head, and the finite caches the learner receives
+(cached actions, teacher scores on them, rollout-time log-probs).  It holds
+none of the loss / estimator arithmetic and imports neither the CUDA binding nor the oracle.
+
+Recipe (shapes from BASELINE.json configs):
+  seeds          s(c, i) = 20260624 + 1000*c + i   for config c, stream i
+  hidden         ~ N(0,1)                          (i=0)
+  W32            ~ N(0,1/d), W = cast(W32)         (i=1)       logical [d,V], v contiguous
+  teacher W_T    ~ N(0,1/d) independent            (i=2)       log q = logsoftmax(hidden @ W_T), temperature 1
+  stale student  W_old = cast(W32 + sigma*E), E ~ N(0,1/d) (i=3); sigma=0 => W_old == W bit for bit
+  mask           (i=4)   'none' | 'random10' (exactly floor(0.1*T) masked) | 'varlen' (sequences padded
+                         to seq_len, lengths uniform in [min_len, seq_len], i=6)
+  MC draws       (i=5)   a_j ~ Categorical(p_old) iid WITH replacement, K per token
+  top-k cache    idx = TopK(log q, k) chosen by the teacher, lam = log q[idx]
+  MC cache       idx = a, lam = log q[a], old = log p_old[a]
+All cache values are fp32, indices int32.  Rollout settings follow PAPER.md:332 (temperature 1,
+no truncation).  These are stand-ins for the paper's Qwen3 workloads: V=151936 and
+d in {2048,2560,4096} are the 1.7B/4B/8B-class student heads.
+"""
+from __future__ import annotations
+
+import torch
+
+SEED0 = 20260624
+
+# BASELINE.json configs (index = position in BASELINE.json "configs", 1-based to match DESIGN.md C1..C5)
+CONFIGS = {
+    1: dict(name="C1", dtype="fp32", T=256, d=256, V=4096, k=8, K=4, sigma=0.05, mask="random10"),
+    2: dict(name="C2", dtype="bf16", T=4096, d=1024, V=32768, k=16, K=4, sigma=0.02, mask="none"),
+    3: dict(name="C3", dtype="bf16", T=16384, d=2048, V=151936, k=32, K=8, sigma=0.02, mask="varlen",
+            seq_len=4096, min_len=512),
+    4: dict(name="C4", dtype="bf16", T=32768, d=4096, V=151936, k=16, K=16, sigma=0.02, mask="none"),
+    5: dict(name="C5", dtype="bf16", T=65536, d=2560, V=151936, k=64, K=8, sigma=0.02, mask="mixed_seq",
+            seq_len=8192),
+}
+
+
+def _gen(seed: int, device) -> torch.Generator:
+    g = torch.Generator(device=device)
+    g.manual_seed(seed)
+    return g
+
+
+def _tdtype(name: str):
+    return torch.bfloat16 if name == "bf16" else torch.float32
+
+
+def make_mask(cfg: dict, c: int, device="cpu") -> torch.Tensor:
+    """uint8 [T]; 0 = masked, 1 = live (in 'mixed_seq': 1 = FKL_TOPK row, 2 = RKL_MC row)."""
+    T = cfg["T"]
+    kind = cfg.get("mask", "none")
+    if kind == "none":
+        return torch.ones(T, dtype=torch.uint8, device=device)
+    if kind == "random10":
+        g = _gen(SEED0 + 1000 * c + 4, "cpu")
+        perm = torch.randperm(T, generator=g)
+        m = torch.ones(T, dtype=torch.uint8)
+        m[perm[: T // 10]] = 0
+        return m.to(device)
+    if kind == "varlen":
+        L = cfg["seq_len"]
+        nseq = T // L
+        g = _gen(SEED0 + 1000 * c + 6, "cpu")
+        lens = torch.randint(cfg["min_len"], L + 1, (nseq,), generator=g)
+        pos = torch.arange(L).unsqueeze(0).expand(nseq, L)
+        return (pos < lens.unsqueeze(1)).to(torch.uint8).reshape(T).to(device)
+    if kind == "mixed_seq":
+        L = cfg["seq_len"]
+        nseq = T // L
+        code = torch.ones(nseq, dtype=torch.uint8)
+        code[nseq // 2:] = 2          # first half of the sequences FKL_TOPK, second half RKL_MC
+        return code.repeat_interleave(L).to(device)
+    raise ValueError(kind)
+
+
+def make_inputs(cfg: dict, c: int = 0, device="cpu", keep_teacher_rows: bool = False,
+                chunk: int = 2048, sigma=None) -> dict:
+    """Generate one workload.  Returns tensors on ``device``:
+
+    hidden [T,d], W [d,V] (cfg dtype); mask [T] u8;
+    topk_idx [T,k] i32, topk_logq [T,k] f32            (teacher-selected support + its log-probs)
+    mc_idx [T,K] i32, mc_logq [T,K] f32, mc_logp_old [T,K] f32
+    and, if keep_teacher_rows, logq [T,V] / logp_old [T,V] f32 (small configs, for oracle pins).
+    """
+    T, d, V, k, K = cfg["T"], cfg["d"], cfg["V"], cfg["k"], cfg["K"]
+    sig = cfg["sigma"] if sigma is None else sigma
+    dt = _tdtype(cfg["dtype"])
+    dev = torch.device(device)
+    s = SEED0 + 1000 * c
+    hidden = torch.randn(T, d, generator=_gen(s + 0, dev), device=dev, dtype=torch.float32).to(dt)
+    W32 = torch.randn(d, V, generator=_gen(s + 1, dev), device=dev, dtype=torch.float32) * (d ** -0.5)
+    W = W32.to(dt)
+    WT = (torch.randn(d, V, generator=_gen(s + 2, dev), device=dev, dtype=torch.float32) * (d ** -0.5)).to(dt)
+    if sig == 0:
+        Wold = W
+    else:
+        E = torch.randn(d, V, generator=_gen(s + 3, dev), device=dev, dtype=torch.float32) * (d ** -0.5)
+        Wold = (W32 + sig * E).to(dt)
+        del E
+    del W32
+    g5 = _gen(s + 5, dev)
+
+    topk_idx = torch.empty(T, k, dtype=torch.int32, device=dev)
+    topk_logq = torch.empty(T, k, dtype=torch.float32, device=dev)
+    mc_idx = torch.empty(T, K, dtype=torch.int32, device=dev)
+    mc_logq = torch.empty(T, K, dtype=torch.float32, device=dev)
+    mc_old = torch.empty(T, K, dtype=torch.float32, device=dev)
+    logq_all = torch.empty(T, V, dtype=torch.float32, device=dev) if keep_teacher_rows else None
+    logpold_all = torch.empty(T, V, dtype=torch.float32, device=dev) if keep_teacher_rows else None
+    WTf, Woldf = WT.float(), Wold.float()
+    for r0 in range(0, T, chunk):
+        r1 = min(T, r0 + chunk)
+        h = hidden[r0:r1].float()
+        logq = torch.log_softmax(h @ WTf, dim=-1)
+        logpo = torch.log_softmax(h @ Woldf, dim=-1)
+        tv, ti = torch.topk(logq, k, dim=-1)               # descending
+        topk_idx[r0:r1] = ti.to(torch.int32)
+        topk_logq[r0:r1] = tv
+        a = torch.multinomial(torch.exp(logpo), K, replacement=True, generator=g5)
+        mc_idx[r0:r1] = a.to(torch.int32)
+        mc_logq[r0:r1] = torch.gather(logq, 1, a)
+        mc_old[r0:r1] = torch.gather(logpo, 1, a)
+        if keep_teacher_rows:
+            logq_all[r0:r1] = logq
+            logpold_all[r0:r1] = logpo
+    out = dict(hidden=hidden, W=W, mask=make_mask(cfg, c, dev), topk_idx=topk_idx, topk_logq=topk_logq,
+               mc_idx=mc_idx, mc_logq=mc_logq, mc_logp_old=mc_old, cfg=dict(cfg), sigma=sig)
+    if keep_teacher_rows:
+        out["logq"] = logq_all
+        out["logp_old"] = logpold_all
+        out["W_old"] = Wold
+        out["W_T"] = WT
+    return out
+
+
+def mixed_cache(inp: dict):
+    """One [T,C] cache for OPD_MIXED, C = max(k,K): FKL rows (mask==1) hold the top-k cache in their
+    first k slots, MC rows (mask==2) the MC cache in their first K slots; unused slots are zero."""
+    k = inp["topk_idx"].shape[1]
+    K = inp["mc_idx"].shape[1]
+    C = max(k, K)
+    T = inp["mask"].shape[0]
+    dev = inp["mask"].device
+    idx = torch.zeros(T, C, dtype=torch.int32, device=dev)
+    lam = torch.zeros(T, C, dtype=torch.float32, device=dev)
+    old = torch.zeros(T, C, dtype=torch.float32, device=dev)
+    f = inp["mask"] == 1
+    m = inp["mask"] == 2
+    idx[f, :k] = inp["topk_idx"][f]
+    lam[f, :k] = inp["topk_logq"][f]
+    idx[m, :K] = inp["mc_idx"][m]
+    lam[m, :K] = inp["mc_logq"][m]
+    old[m, :K] = inp["mc_logp_old"][m]
+    return idx, lam, old, k | (K << 16)

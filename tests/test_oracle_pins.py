@@ -1,0 +1,348 @@
+"""Pins for the fp64 oracle (oracle/opd_oracle.py): what the paper and the mathematics fix.
+
+Each pin names the part of the oracle it fixes (P-numbers as in DESIGN.md "Oracle pins").
+None of these tests touches the CUDA path.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import opd_oracle as O
+from paper_2606_24143_b200 import synth
+
+
+def tiny(seed, T=4, d=6, V=12, C=3, dup=False, mask=None):
+    rng = np.random.default_rng(seed)
+    X = rng.normal(size=(T, d))
+    W = rng.normal(size=(d, V)) / math.sqrt(d)
+    WT = rng.normal(size=(d, V)) / math.sqrt(d)
+    Wold = W + 0.3 * rng.normal(size=(d, V)) / math.sqrt(d)
+    logq, _ = O.log_softmax_rows(X @ WT)
+    logpo, _ = O.log_softmax_rows(X @ Wold)
+    idx = np.stack([rng.choice(V, size=C, replace=dup) for _ in range(T)])
+    if dup:
+        idx[:, -1] = idx[:, 0]           # force a duplicate in every row
+    lam = np.take_along_axis(logq, idx, 1)
+    old = np.take_along_axis(logpo, idx, 1)
+    m = np.ones(T, dtype=np.uint8) if mask is None else np.asarray(mask, dtype=np.uint8)
+    return dict(X=X, W=W, WT=WT, Wold=Wold, logq=logq, logpo=logpo, idx=idx, lam=lam, old=old, mask=m)
+
+
+def c1_inputs():
+    cfg = dict(synth.CONFIGS[1])
+    inp = synth.make_inputs(cfg, c=1, device="cpu", keep_teacher_rows=True)
+    f = lambda t: t.to(torch.float64).numpy() if t.is_floating_point() else t.numpy()
+    return {k: (f(v) if isinstance(v, torch.Tensor) else v) for k, v in inp.items()}
+
+
+# ---------------------------------------------------------------- P1
+@pytest.mark.parametrize("flags", [0, O.F_NO_RENORM_TEACHER, O.F_RENORM_STUDENT,
+                                   O.F_NO_RENORM_TEACHER | O.F_RENORM_STUDENT])
+def test_P1_topk_with_k_equal_V_is_dense_forward_kl(flags):
+    """PAPER.md:57 Eq.(1): the sparse top-k forward KL with S = V is the dense D_F (north_star)."""
+    t = tiny(1, T=5, d=7, V=16)
+    V = 16
+    idx = np.tile(np.arange(V), (5, 1))
+    r = O.opd_oracle(t["X"], t["W"], idx, t["logq"], None, t["mask"], O.FKL_TOPK, V, flags=flags)
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    DF = O.dense_forward_kl(t["logq"], logp)
+    np.testing.assert_allclose(r["per_token_kl"], DF, rtol=0, atol=1e-12)
+    assert abs(r["loss"] - DF.mean()) < 1e-12
+
+
+def test_P1_on_C1_permuted_support():
+    c = c1_inputs()
+    T, V = 16, c["W"].shape[1]
+    rng = np.random.default_rng(0)
+    idx = np.stack([rng.permutation(V) for _ in range(T)])
+    c["logq"] = O.log_softmax_rows(c["logq"])[0]        # the generator's fp32 rows, renormalised exactly in fp64
+    lam = np.take_along_axis(c["logq"][:T], idx, 1)
+    r = O.opd_oracle(c["hidden"][:T], c["W"], idx, lam, None, np.ones(T), O.FKL_TOPK, V, want_grads=False)
+    logp, _ = O.log_softmax_rows(c["hidden"][:T] @ c["W"])
+    np.testing.assert_allclose(r["per_token_kl"], O.dense_forward_kl(c["logq"][:T], logp), atol=1e-11)
+
+
+# ---------------------------------------------------------------- P2
+def test_P2_k1_is_library_cross_entropy_with_softmax_minus_onehot_gradient():
+    """k=1 with teacher renorm: L = -log p(a).  Checked end to end against torch's fp64 cross_entropy + autograd."""
+    t = tiny(2, T=6, d=5, V=11, C=1)
+    r = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], None, t["mask"], O.FKL_TOPK, 1)
+    X = torch.tensor(t["X"], requires_grad=True)
+    W = torch.tensor(t["W"], requires_grad=True)
+    loss = torch.nn.functional.cross_entropy(X @ W, torch.tensor(t["idx"][:, 0]), reduction="mean")
+    loss.backward()
+    assert abs(r["loss"] - loss.item()) < 1e-12
+    np.testing.assert_allclose(r["grad_hidden"], X.grad.numpy(), atol=1e-13)
+    np.testing.assert_allclose(r["grad_W"], W.grad.numpy(), atol=1e-13)
+
+
+# ---------------------------------------------------------------- P3
+def test_P3_mc_with_uniform_proposal_over_all_V_is_dense_reverse_kl():
+    """Eq.(2),(3),(5) PAPER.md:63-68,128: K=V, a = 0..V-1, o = -log V  =>  L = D_R and the surrogate
+    gradient (A frozen) equals the finite-difference gradient of the dense D_R."""
+    t = tiny(3, T=3, d=5, V=9)
+    V = 9
+    idx = np.tile(np.arange(V), (3, 1))
+    old = np.full((3, V), -math.log(V))
+    r = O.opd_oracle(t["X"], t["W"], idx, t["logq"], old, t["mask"], O.RKL_MC, V)
+    def DR(X, W):
+        logp, _ = O.log_softmax_rows(X @ W)
+        return O.dense_reverse_kl(t["logq"], logp)
+    np.testing.assert_allclose(r["per_token_kl"], DR(t["X"], t["W"]), atol=1e-12)
+    h = 1e-6
+    for (ti, ki) in [(0, 0), (1, 3), (2, 4)]:
+        Xp, Xm = t["X"].copy(), t["X"].copy()
+        Xp[ti, ki] += h; Xm[ti, ki] -= h
+        fd = (DR(Xp, t["W"]).mean() - DR(Xm, t["W"]).mean()) / (2 * h)
+        assert abs(fd - r["grad_hidden"][ti, ki]) < 1e-8
+    for (ki, vi) in [(0, 0), (2, 5), (4, 8)]:
+        Wp, Wm = t["W"].copy(), t["W"].copy()
+        Wp[ki, vi] += h; Wm[ki, vi] -= h
+        fd = (DR(t["X"], Wp).mean() - DR(t["X"], Wm).mean()) / (2 * h)
+        assert abs(fd - r["grad_W"][ki, vi]) < 1e-8
+
+
+# ---------------------------------------------------------------- P4
+def test_P4_importance_sampling_identity_by_enumeration():
+    """Eq.(5): sum_a p_old(a) rho(a) A(a) = -D_R for any full-support p_old."""
+    t = tiny(4, T=4, d=6, V=10)
+    V = 10
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    for ti in range(4):
+        tot = 0.0
+        for a in range(V):
+            L, _, _ = O.token_terms(O.RKL_MC, [t["logq"][ti, a]], [t["logpo"][ti, a]], [logp[ti, a]], 0)
+            tot += math.exp(t["logpo"][ti, a]) * L         # L = -rho A for K=1
+        DR = O.dense_reverse_kl(t["logq"][ti], logp[ti])
+        assert abs(tot - DR) < 1e-12
+
+
+# ---------------------------------------------------------------- P5 / P12
+def test_P5_P12_on_policy_unbiasedness_and_one_over_m_variance():
+    """PAPER.md:161, Eq.(11)-(13) PAPER.md:309-317: with p_old = p_theta the estimator's mean converges to D_R;
+    PAPER.md:191 + Table 6: Var[L_m] = Var[L_1]/m for iid samples (paper measured
+    0.255 / 0.0588 / 0.0149 at m = 4, 16, 64)."""
+    t = tiny(5, T=3, d=6, V=14)
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    rng = np.random.default_rng(123)
+    R = 40000
+    for ti in range(3):
+        p = np.exp(logp[ti])
+        DR = O.dense_reverse_kl(t["logq"][ti], logp[ti])
+        var = {}
+        for m in (1, 4, 16):
+            a = rng.choice(14, size=(R, m), p=p)
+            est = np.array([O.token_terms(O.RKL_MC, t["logq"][ti, a[r]], logp[ti, a[r]], logp[ti, a[r]], 0)[0]
+                            for r in range(0, R, 8 if m > 1 else 1)])
+            se = est.std() / math.sqrt(est.size)
+            assert abs(est.mean() - DR) < 5 * se + 1e-12, (m, est.mean(), DR, se)
+            var[m] = est.var()
+        assert abs(var[4] / var[1] - 0.25) < 0.03
+        assert abs(var[16] / var[1] - 1 / 16) < 0.012
+
+
+def test_P5_stale_proposal_is_still_unbiased_with_IS():
+    """Eq.(5): sampling from the generator's stale p_old and weighting by rho is unbiased for D_R."""
+    t = tiny(6, T=2, d=6, V=12)
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    rng = np.random.default_rng(7)
+    for ti in range(2):
+        po = np.exp(t["logpo"][ti])
+        a = rng.choice(12, size=(30000, 4), p=po / po.sum())
+        est = np.array([O.token_terms(O.RKL_MC, t["logq"][ti, r], t["logpo"][ti, r], logp[ti, r], 0)[0] for r in a])
+        DR = O.dense_reverse_kl(t["logq"][ti], logp[ti])
+        assert abs(est.mean() - DR) < 5 * est.std() / math.sqrt(est.size)
+
+
+# ---------------------------------------------------------------- P6 / P7
+def test_P6_P7_renorm_variants_and_nonnegativity():
+    """KL(q~||p) - KL(q~||p~^S) = -log Z_p^S = lse_full - lse_S >= 0; both KLs >= 0 (Gibbs)."""
+    c = c1_inputs()
+    T = 64
+    args = (c["hidden"][:T], c["W"], c["topk_idx"][:T], c["topk_logq"][:T], None, np.ones(T), O.FKL_TOPK, 8)
+    a = O.opd_oracle(*args, flags=0, want_grads=False)
+    b = O.opd_oracle(*args, flags=O.F_RENORM_STUDENT, want_grads=False)
+    lseS = np.array([O.logsumexp(a["student_logp"][t]) for t in range(T)])      # log Z_p^S
+    np.testing.assert_allclose(a["per_token_kl"] - b["per_token_kl"], -lseS, atol=1e-12)
+    assert (-lseS >= 0).all()
+    assert (a["per_token_kl"] >= -1e-15).all() and (b["per_token_kl"] >= -1e-15).all()
+    logp, _ = O.log_softmax_rows(c["hidden"][:T] @ c["W"])
+    assert (O.dense_forward_kl(c["logq"][:T], logp) >= 0).all()
+    assert (O.dense_reverse_kl(c["logq"][:T], logp) >= 0).all()
+
+
+# ---------------------------------------------------------------- P8
+def test_P8_zero_cases_teacher_equals_student():
+    t = tiny(8, T=4, d=6, V=12, C=4)
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    lam = np.take_along_axis(logp, t["idx"], 1)
+    r = O.opd_oracle(t["X"], t["W"], t["idx"], lam, t["old"], t["mask"], O.RKL_MC, 4)
+    assert np.all(r["per_token_kl"] == 0) and np.all(r["grad_hidden"] == 0) and np.all(r["grad_W"] == 0)
+    f = O.opd_oracle(t["X"], t["W"], t["idx"], lam, None, t["mask"], O.FKL_TOPK, 4)
+    lseS = np.array([O.logsumexp(lam[i]) for i in range(4)])
+    np.testing.assert_allclose(f["per_token_kl"], -lseS, atol=1e-13)
+    full = np.tile(np.arange(12), (4, 1))
+    z = O.opd_oracle(t["X"], t["W"], full, logp, None, t["mask"], O.FKL_TOPK, 12)
+    assert np.abs(z["per_token_kl"]).max() < 1e-14 and np.abs(z["grad_W"]).max() < 1e-15
+
+
+# ---------------------------------------------------------------- P9
+def _surrogate_loss(t, X, W, mode, C, flags, A_frozen, mask, k_or_K):
+    """Loss value recomputed from scratch (independent of token_terms) with MC advantages frozen."""
+    logp, _ = O.log_softmax_rows(X @ W)
+    N = np.count_nonzero(mask)
+    tot = 0.0
+    for ti in range(X.shape[0]):
+        if mask[ti] == 0:
+            continue
+        tm = mode if mode != O.MIXED else (O.FKL_TOPK if mask[ti] == 1 else O.RKL_MC)
+        Ct = C if mode != O.MIXED else ((k_or_K & 0xFFFF) if tm == O.FKL_TOPK else (k_or_K >> 16))
+        a = t["idx"][ti, :Ct]
+        ell = logp[ti, a]
+        lam = t["lam"][ti, :Ct]
+        if tm == O.FKL_TOPK:
+            lq = lam if flags & O.F_NO_RENORM_TEACHER else lam - np.log(np.exp(lam).sum())
+            lp = ell - np.log(np.exp(ell).sum()) if flags & O.F_RENORM_STUDENT else ell
+            tot += float((np.exp(lq) * (lq - lp)).sum())
+        else:
+            tot += -float((np.exp(ell - t["old"][ti, :Ct]) * A_frozen[ti, :Ct]).mean())
+    return tot / N
+
+
+@pytest.mark.parametrize("mode,flags,dup", [
+    (O.FKL_TOPK, 0, False), (O.FKL_TOPK, O.F_NO_RENORM_TEACHER, False), (O.FKL_TOPK, O.F_RENORM_STUDENT, False),
+    (O.FKL_TOPK, O.F_RENORM_STUDENT | O.F_NO_RENORM_TEACHER, False),
+    (O.RKL_MC, 0, False), (O.RKL_MC, 0, True), (O.MIXED, 0, True)])
+def test_P9_central_finite_differences(mode, flags, dup):
+    """grad_hidden / grad_W against central differences of an independently written loss; MC uses the
+    frozen-A surrogate (stop-gradient)."""
+    mask = [1, 0, 2, 1] if mode == O.MIXED else [1, 0, 1, 1]
+    t = tiny(9, T=4, d=6, V=12, C=3, dup=dup and mode != O.FKL_TOPK, mask=mask)
+    kk = (2 | (3 << 16)) if mode == O.MIXED else 3
+    r = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], mode, kk, flags=flags)
+    A0 = t["lam"] - np.nan_to_num(r["student_logp"])
+    f = lambda X, W: _surrogate_loss(t, X, W, mode, 3, flags, A0, t["mask"], kk)
+    h = 1e-6
+    rng = np.random.default_rng(0)
+    for _ in range(12):
+        ti, ki, vi = rng.integers(4), rng.integers(6), rng.integers(12)
+        Xp, Xm = t["X"].copy(), t["X"].copy(); Xp[ti, ki] += h; Xm[ti, ki] -= h
+        assert abs((f(Xp, t["W"]) - f(Xm, t["W"])) / (2 * h) - r["grad_hidden"][ti, ki]) < 2e-8
+        Wp, Wm = t["W"].copy(), t["W"].copy(); Wp[ki, vi] += h; Wm[ki, vi] -= h
+        assert abs((f(t["X"], Wp) - f(t["X"], Wm)) / (2 * h) - r["grad_W"][ki, vi]) < 2e-8
+    # every cached column is probed too
+    for ti in (0, 2, 3):
+        vi = int(t["idx"][ti, 0])
+        Wp, Wm = t["W"].copy(), t["W"].copy(); Wp[1, vi] += h; Wm[1, vi] -= h
+        assert abs((f(t["X"], Wp) - f(t["X"], Wm)) / (2 * h) - r["grad_W"][1, vi]) < 2e-8
+    assert np.all(r["grad_hidden"][1] == 0)
+
+
+# ---------------------------------------------------------------- P10
+@pytest.mark.parametrize("mode", [O.FKL_TOPK, O.RKL_MC])
+def test_P10_shift_invariance(mode):
+    """alpha + sum_j beta_j = 0  =>  every row of g sums to 0  =>  sum_v grad_W[k,v] = 0; adding a constant to a
+    row of logits (a ones feature times a constant row of W) leaves the loss unchanged."""
+    t = tiny(10, T=5, d=6, V=13, C=4, dup=(mode == O.RKL_MC))
+    r = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], mode, 4)
+    assert np.abs(r["grad_W"].sum(axis=1)).max() < 1e-14
+    X2 = np.concatenate([t["X"], np.ones((5, 1))], axis=1)
+    W2 = np.concatenate([t["W"], np.full((1, 13), 3.7)], axis=0)
+    r2 = O.opd_oracle(X2, W2, t["idx"], t["lam"], t["old"], t["mask"], mode, 4)
+    assert abs(r2["loss"] - r["loss"]) < 1e-12
+    np.testing.assert_allclose(r2["grad_W"][:-1], r["grad_W"], atol=1e-13)
+
+
+# ---------------------------------------------------------------- P11
+def test_P11_mask_and_permutations():
+    t = tiny(11, T=6, d=5, V=10, C=3, mask=[1, 0, 1, 1, 0, 1])
+    base = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], O.RKL_MC, 3)
+    X2, lam2, idx2 = t["X"].copy(), t["lam"].copy(), t["idx"].copy()
+    X2[[1, 4]] = 1e3; lam2[[1, 4]] = -77.0; idx2[[1, 4]] = 0
+    g = O.opd_oracle(X2, t["W"], idx2, lam2, t["old"], t["mask"], O.RKL_MC, 3)
+    assert g["loss"] == base["loss"] and np.array_equal(g["grad_W"], base["grad_W"])
+    assert np.all(base["grad_hidden"][[1, 4]] == 0) and np.all(base["per_token_kl"][[1, 4]] == 0)
+    perm = np.array([3, 0, 5, 1, 2, 4])
+    p = O.opd_oracle(t["X"][perm], t["W"], t["idx"][perm], t["lam"][perm], t["old"][perm], t["mask"][perm], O.RKL_MC, 3)
+    np.testing.assert_allclose(p["per_token_kl"], base["per_token_kl"][perm], atol=1e-15)
+    np.testing.assert_allclose(p["grad_hidden"], base["grad_hidden"][perm], atol=1e-15)
+    np.testing.assert_allclose(p["grad_W"], base["grad_W"], atol=1e-14)
+    sp = np.array([2, 0, 1])
+    s = O.opd_oracle(t["X"], t["W"], t["idx"][:, sp], t["lam"][:, sp], t["old"][:, sp], t["mask"], O.RKL_MC, 3)
+    np.testing.assert_allclose(s["per_token_kl"], base["per_token_kl"], atol=1e-15)
+    # N = number of live tokens; norm_override rescales
+    o = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], O.RKL_MC, 3, norm_override=8.0)
+    assert abs(o["loss"] - base["loss"] * 4 / 8) < 1e-15
+    z = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], t["old"], np.zeros(6), O.RKL_MC, 3)
+    assert z["loss"] == 0 and np.all(z["grad_W"] == 0)
+
+
+# ---------------------------------------------------------------- P13
+def test_P13_duplicates_and_teacher_constant():
+    t = tiny(13, T=4, d=6, V=12, C=1)
+    one = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], O.RKL_MC, 1)
+    rep = lambda a: np.repeat(a, 5, axis=1)
+    five = O.opd_oracle(t["X"], t["W"], rep(t["idx"]), rep(t["lam"]), rep(t["old"]), t["mask"], O.RKL_MC, 5)
+    np.testing.assert_allclose(five["per_token_kl"], one["per_token_kl"], atol=1e-14)
+    np.testing.assert_allclose(five["grad_W"], one["grad_W"], atol=1e-14)
+    u = tiny(14, T=4, d=6, V=12, C=4)
+    a = O.opd_oracle(u["X"], u["W"], u["idx"], u["lam"], None, u["mask"], O.FKL_TOPK, 4)
+    b = O.opd_oracle(u["X"], u["W"], u["idx"], u["lam"] + np.array([[1.5], [-2.0], [0.3], [9.0]]), None,
+                     u["mask"], O.FKL_TOPK, 4)
+    np.testing.assert_allclose(a["per_token_kl"], b["per_token_kl"], atol=1e-13)
+    np.testing.assert_allclose(a["grad_hidden"], b["grad_hidden"], atol=1e-14)
+
+
+# ---------------------------------------------------------------- P14
+@pytest.mark.parametrize("mode,flags", [(O.FKL_TOPK, 0), (O.FKL_TOPK, O.F_RENORM_STUDENT), (O.RKL_MC, 0), (O.MIXED, 0)])
+def test_P14_loops_agree_with_vectorised(mode, flags):
+    mask = [2, 1, 0, 1, 2] if mode == O.MIXED else [1, 1, 0, 1, 1]
+    t = tiny(15, T=5, d=4, V=9, C=3, dup=(mode != O.FKL_TOPK), mask=mask)
+    kk = (3 | (2 << 16)) if mode == O.MIXED else 3
+    a = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], mode, kk, flags=flags, chunk=2)
+    b = O.opd_oracle_loops(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], mode, kk, flags=flags)
+    assert abs(a["loss"] - b["loss"]) < 1e-13
+    np.testing.assert_allclose(a["grad_hidden"], b["grad_hidden"], atol=1e-13)
+    np.testing.assert_allclose(a["grad_W"], b["grad_W"], atol=1e-13)
+    cols = [0, 4, int(t["idx"][0, 0]), 8]
+    gc = O.grad_W_columns(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], mode, kk, cols, flags=flags)
+    np.testing.assert_allclose(gc, b["grad_W"][:, cols], atol=1e-13)
+    sub = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], mode, kk, flags=flags, rows=[0, 3])
+    np.testing.assert_allclose(sub["grad_hidden"][[0, 3]], b["grad_hidden"][[0, 3]], atol=1e-13)
+
+
+# ---------------------------------------------------------------- NEXT-1 / NEXT-2 pins
+def test_surrogate_variants_reduce_to_reference():
+    """Eq.(6),(7) PAPER.md:132-141: with eps -> inf the clipped forms equal the unclipped ones; with W_old = W
+    (rho = 1, A_old = A_theta) all four coincide."""
+    t = tiny(16, T=3, d=5, V=10, C=4)
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    for ti in range(3):
+        ell = logp[ti, t["idx"][ti]]
+        ref = O.token_terms(O.RKL_MC, t["lam"][ti], t["old"][ti], ell, 0, O.SUR_THETA_NOCLIP)
+        big = O.token_terms(O.RKL_MC, t["lam"][ti], t["old"][ti], ell, 0, O.SUR_THETA_CLIP, clip_eps=1e9)
+        assert abs(ref[0] - big[0]) < 1e-15 and np.allclose(ref[2], big[2], atol=1e-15)
+        same = [O.token_terms(O.RKL_MC, t["lam"][ti], ell, ell, 0, s) for s in range(4)]
+        for s in same[1:]:
+            assert abs(s[0] - same[0][0]) < 1e-15 and np.allclose(s[2], same[0][2], atol=1e-15)
+        # clipped objective never exceeds... min(.,.) <= unclipped term, so L_clip >= L_noclip
+        cl = O.token_terms(O.RKL_MC, t["lam"][ti], t["old"][ti], ell, 0, O.SUR_OLD_CLIP, clip_eps=0.2)
+        nc = O.token_terms(O.RKL_MC, t["lam"][ti], t["old"][ti], ell, 0, O.SUR_OLD_NOCLIP)
+        assert cl[0] >= nc[0] - 1e-15
+
+
+def test_sparse_reverse_kl_definition_and_gradient():
+    """Eq.(9),(10) PAPER.md:293-301: S = V gives dense D_R; gradient by finite differences; D >= 0."""
+    t = tiny(17, T=2, d=5, V=8)
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    D, g = O.sparse_reverse_kl(t["logq"][0], logp[0])
+    assert abs(D - O.dense_reverse_kl(t["logq"][0], logp[0])) < 1e-13
+    lam, ell = t["logq"][1, :5] + 0.4, logp[1, :5]
+    D, g = O.sparse_reverse_kl(lam, ell)
+    assert D >= 0
+    for j in range(5):
+        e = np.zeros(5); e[j] = 1e-6
+        fd = (O.sparse_reverse_kl(lam, ell + e)[0] - O.sparse_reverse_kl(lam, ell - e)[0]) / 2e-6
+        assert abs(fd - g[j]) < 1e-9
