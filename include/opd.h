@@ -1,0 +1,149 @@
+/* opd.h — C ABI of libopd: the fused on-policy-distillation (OPD) loss on one B200 (sm_100a).
+ *
+ * Learner-side hot path of AsyncOPD (arxiv/paper_2606_24143; citations are PAPER.md lines):
+ *   student logits z = hidden . W over the whole vocabulary, streamed tile by tile through
+ *   tcgen05/TMEM and never stored (p_theta(.|s) is a policy over V);
+ *   lse_t = log sum_v exp z_tv; l_tj = z_t[a_tj] - lse_t at the cached actions ("recompute
+ *   log p_theta(a|s) for a in C_score(s)"); the estimators
+ *     OPD_FKL_TOPK  sparse top-k teacher-weighted forward KL on the cached support
+ *                   (Eq.(1) PAPER.md:57 restricted to S; renormalisers Eq.(9))
+ *     OPD_RKL_MC    multi-sample Monte-Carlo reverse KL  L = -(1/m) sum_i rho_i sg(A_theta,i)
+ *                   (Eq.(15)) with the advantage recomputed at learner
+ *                   time A = log q - log p_theta and the unclipped ratio rho = p_theta / p_old
+ *                   (Finding 2 PAPER.md:153)
+ *   loss = (1/N) sum over live tokens; and the backward into grad_hidden and grad_W, for which the
+ *   softmax tiles are re-formed (never read back from memory).
+ *
+ * Conventions
+ *   - Pointers are DEVICE pointers unless the name says host. The caller owns every buffer; inputs are
+ *     never modified. All work is enqueued on `cuda_stream` (a cudaStream_t) and the call returns
+ *     without synchronising (exception: OPD_F_VALIDATE_IDX, and the *_host entry point).
+ *   - Errors are status codes; argument errors are detected on the host before any launch.
+ *     opd_last_error() returns a host string describing the last failure on the handle.
+ *   - No CPU fallback: on a device that is not compute capability 10.x every compute entry point
+ *     returns OPD_ERR_ARCH.
+ *   - One handle per host thread / stream. The handle owns its workspace unless opd_set_workspace
+ *     was called.
+ */
+#ifndef OPD_H_
+#define OPD_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct opd_handle_s* opd_handle_t;
+
+typedef enum {
+    OPD_OK = 0,
+    OPD_ERR_BAD_ARG = -1,    /* null pointer, unknown mode/dtype/flag, misaligned pointer or stride */
+    OPD_ERR_BAD_SHAPE = -2,  /* T,d,V,C out of the supported range (see opd_loss_fwd_bwd) */
+    OPD_ERR_BAD_INDEX = -3,  /* OPD_F_VALIDATE_IDX found a cache index outside [0,V) on a live row */
+    OPD_ERR_WORKSPACE = -4,  /* caller-provided workspace too small / allocation failed */
+    OPD_ERR_ARCH = -5,       /* device is not sm_100 class */
+    OPD_ERR_CUDA = -6        /* a CUDA runtime/driver call failed; see opd_last_error */
+} opd_status_t;
+
+typedef enum { OPD_FKL_TOPK = 0, OPD_RKL_MC = 1, OPD_MIXED = 2 } opd_mode_t;
+typedef enum { OPD_BF16 = 0, OPD_FP32 = 1 } opd_dtype_t;
+
+enum {
+    OPD_F_NO_RENORM_TEACHER = 1, /* FKL: do not renormalise the cached teacher scores on S (truncated sum)      */
+    OPD_F_RENORM_STUDENT = 2,    /* FKL: renormalise the student on S too (paper-literal Eq.(9); sparse backward) */
+    OPD_F_GRADW_ACCUM = 4,       /* grad_W += ... instead of overwrite (micro-batches)                           */
+    OPD_F_VALIDATE_IDX = 16,     /* check cache indices of live rows; makes the call synchronous                 */
+    OPD_F_FWD_ONLY = 32,         /* loss / per-token outputs only; grad pointers may be NULL                     */
+    /* reverse-KL surrogate of the 2x2 ablation, Eq.(6),(7) PAPER.md:132-141 (default: A_theta, no clip = Eq.(15)) */
+    OPD_F_SUR_CLIP = 64,         /* PPO clip of rho to [1-eps, 1+eps], eps = 0.2                  */
+    OPD_F_SUR_A_OLD = 128        /* frozen rollout-time advantage A_old = log q - log p_old instead of A_theta   */
+};
+
+/* lifetime ------------------------------------------------------------------------------------- */
+opd_status_t opd_create(opd_handle_t* out, int device);
+opd_status_t opd_destroy(opd_handle_t h);
+const char* opd_last_error(opd_handle_t h); /* host string, valid until the next call on h */
+const char* opd_version(void);
+
+/* workspace ------------------------------------------------------------------------------------
+ * Bytes of device scratch one opd_loss_fwd_bwd call with these arguments needs. No buffer of size
+ * O(T*V) exists: the largest items are the compacted copy of hidden (T*d), the per-tile (max,sumexp)
+ * partials (T*ceil(V/256)*8 B) and a bounded super-tile of re-formed softmax gradients G
+ * (<= 32 MiB per operand plane) that lives in L2 between the three backward contractions. */
+size_t opd_workspace_bytes(int T, int d, int V, int C, opd_dtype_t dtype, opd_mode_t mode, unsigned flags);
+/* Optional: use caller memory (256-byte aligned) instead of the handle's own allocation. */
+opd_status_t opd_set_workspace(opd_handle_t h, void* ws, size_t bytes);
+
+/* the hot path --------------------------------------------------------------------------------
+ * hidden   [T,d], row stride ld_hidden elements, dtype bf16 or fp32.
+ * W        logical W(k,v), k in [0,d), v in [0,V): element (k,v) at W[k*ldw_k + v*ldw_v]; exactly one of
+ *          the strides is 1 ([d,V] row-major: ldw_v = 1;  [V,d] row-major lm_head.weight: ldw_k = 1).
+ * cache_idx [T,C] int32 in [0,V) (row stride ld_cache, also used for the two float caches);
+ * cache_teacher_logp [T,C] log q(a|s); cache_old_logp [T,C] log p_old(a|s) (may be NULL for OPD_FKL_TOPK).
+ * mask     [T] bytes: 0 = masked (row contributes nothing, its cache row is never read).
+ *          OPD_MIXED: 1 = FKL_TOPK row, 2 = RKL_MC row; one token-mean over all live rows.
+ * k_or_K   cache width C (1..64). OPD_MIXED: k | (K << 16); FKL rows use the first k slots, MC rows the
+ *          first K; C = max(k,K).
+ * norm_override  > 0: divide by it instead of N = number of live tokens (N = 0 -> loss 0, grads 0).
+ * loss [1], per_token_kl [T] (0 on masked rows); optional lse_out [T], student_logp_out [T,C] (row stride
+ *          ld_cache; log p_theta(a_tj|s_t), written on live rows' used slots only).
+ * grad_hidden [T,d] dtype of hidden, row stride ld_gh, masked rows exactly 0.
+ * grad_W   fp32, same logical layout as W: element (k,v) at grad_W[k*ldgw_k + v*ldgw_v], the unit stride
+ *          must be the same one as W's.
+ * Supported shapes: 1 <= T < 2^24, d % 64 == 0, 64 <= d <= 16384, V % 8 == 0, 256 <= V < 2^24, 1 <= C <= 64;
+ *          hidden / W / grad bases 16-byte aligned; non-unit strides multiples of 8 (bf16) / 4 (fp32) elements.
+ * Precision: bf16 inputs are used as they are, accumulation is fp32; fp32 inputs are split into three
+ *          bf16 terms each (error ~2^-23 per product), so fp32 results are fp32-accurate. */
+opd_status_t opd_loss_fwd_bwd(opd_handle_t h, void* cuda_stream,
+    int T, int d, int V, opd_dtype_t dtype,
+    const void* hidden, long ld_hidden,
+    const void* W, long ldw_k, long ldw_v,
+    const int* cache_idx, long ld_cache,
+    const float* cache_teacher_logp,
+    const float* cache_old_logp,
+    const unsigned char* mask,
+    opd_mode_t mode, int k_or_K,
+    unsigned flags, float norm_override,
+    float* loss,
+    float* per_token_kl,
+    float* lse_out, float* student_logp_out,
+    void* grad_hidden, long ld_gh,
+    void* grad_W, long ldgw_k, long ldgw_v);
+
+/* Same computation with HOST buffers (pinned or pageable): copies the inputs to handle-owned device
+ * buffers, runs opd_loss_fwd_bwd, copies loss / per_token_kl / grad_hidden / grad_W back and
+ * synchronises. All arrays are dense (ld = inner extent); W is [d,V] row-major. Pointers that are NULL
+ * among the outputs are skipped. *h2d_bytes / *d2h_bytes (may be NULL) receive the bytes copied. */
+opd_status_t opd_loss_fwd_bwd_host(opd_handle_t h,
+    int T, int d, int V, opd_dtype_t dtype,
+    const void* hidden_host, const void* W_host,
+    const int* cache_idx_host, const float* cache_teacher_logp_host, const float* cache_old_logp_host,
+    const unsigned char* mask_host,
+    opd_mode_t mode, int k_or_K, unsigned flags, float norm_override,
+    float* loss_host, float* per_token_kl_host, void* grad_hidden_host, void* grad_W_host,
+    size_t* h2d_bytes, size_t* d2h_bytes);
+
+/* debugging / verification aids ----------------------------------------------------------------
+ * opd_debug_logits: runs the forward contraction kernel only and dumps the fp32 logit tiles it held in
+ * TMEM to logits_out [T,V] (row stride V) and the values its epilogue gathered to gathered_out [T,C]
+ * (row stride C, caller slot order). Small shapes only (it writes T*V floats). All rows are treated as live. */
+opd_status_t opd_debug_logits(opd_handle_t h, void* cuda_stream, int T, int d, int V, opd_dtype_t dtype,
+    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v,
+    const int* cache_idx, long ld_cache, int C, float* logits_out, float* gathered_out);
+/* opd_debug_gemm: D[M,N] (fp32, row stride N) = A . B^T through the library's tcgen05 GEMM core.
+ * A is [M,K] (a_mn_major = 0) or stored as [K,M] (a_mn_major = 1); B is [N,K] or stored as [K,N]. bf16. */
+opd_status_t opd_debug_gemm(opd_handle_t h, void* cuda_stream, int M, int N, int K,
+    const void* A, int a_mn_major, const void* B, int b_mn_major, float* D);
+/* Launch statistics of the last opd_loss_fwd_bwd on this handle: kernels launched, GEMM-kernel launches,
+ * super-tile rows/cols used by the backward. Any pointer may be NULL. */
+opd_status_t opd_last_launch_stats(opd_handle_t h, int* n_kernels, int* n_gemm_kernels, int* super_rows, int* super_cols);
+/* Timing hooks: if `events` (array of 2*OPD_N_PHASES cudaEvent_t, created by the caller) is set, the next
+ * calls record start/stop events around each phase on the call's stream. Pass NULL to disable. */
+enum { OPD_PHASE_PREP = 0, OPD_PHASE_FWD = 1, OPD_PHASE_EST = 2, OPD_PHASE_BWD = 3, OPD_N_PHASES = 4 };
+opd_status_t opd_set_phase_events(opd_handle_t h, void** events);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OPD_H_ */

@@ -1,0 +1,197 @@
+// Backward epilogues (S6-S8), see opd_epilogues.cuh for the conventions.
+#pragma once
+#include "opd_epilogues.cuh"
+
+namespace opd {
+
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+    __nv_bfloat162 t = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&t);
+}
+
+// ------------------------------------------------------------------------------------------ GEpi
+// S6: re-form G[t,v] = coef_t * exp(z[t,v] - lse_t) + sum_j beta_tj [a_tj == v]  with coef = alpha/N,
+// beta pre-scaled by 1/N (derivation: DESIGN.md "Backward"), round to bf16 and store it into the
+// super-tile Gs[Tb][ldg] (row-major, v contiguous) that the dX and dW contractions read back from L2.
+// Rows past the live count and columns past V are written as zeros: both contractions rely on it.
+struct GEpi {
+    struct Params {
+        __nv_bfloat16* gs;       // [planes][Tb_pad][ldg]
+        long ldg;
+        long plane_stride;       // elements
+        int planes;              // 1 (bf16 path) or 3 (fp32 path: three-term bf16 split of G)
+        const float* lse2;       // [T] lse * log2(e), compact row order
+        const float* coef;       // [T] alpha_t / N
+        const int* sorted_idx;   // [T][C]
+        const float* beta;       // [T][C] beta_tj / N in sorted-slot order
+        int C;
+        int V;
+    };
+    struct State { int cursor; int next_col; float lse2; float coef; };
+    static __device__ __forceinline__ State prepare(const Params& p, const GemmParams& gp, int m_blk, int n_blk,
+                                                    int row_in_tile, int M_eff) {
+        State st{p.C, IDX_SENTINEL, 0.f, 0.f};
+        const int lrow = m_blk * BM + row_in_tile;
+        if (lrow < M_eff) {
+            const int row = gp.tok_off + lrow;
+            const int* idx = p.sorted_idx + static_cast<size_t>(row) * p.C;
+            st.cursor = lower_bound_slot(idx, p.C, gp.b_off + n_blk * BN);
+            st.next_col = st.cursor < p.C ? __ldg(idx + st.cursor) : IDX_SENTINEL;
+            st.lse2 = p.lse2[row];
+            st.coef = p.coef[row];
+        }
+        return st;
+    }
+    static __device__ __forceinline__ void run(const Params& p, const GemmParams& gp, State st, uint32_t taddr,
+                                               int m_blk, int n_blk, int row_in_tile, int M_eff, uint8_t*, int) {
+        const int lrow = m_blk * BM + row_in_tile;
+        const bool live = lrow < M_eff;
+        const int row = gp.tok_off + lrow;
+        const int* idx = p.sorted_idx + static_cast<size_t>(row) * p.C;
+        const float* beta = p.beta + static_cast<size_t>(row) * p.C;
+        __nv_bfloat16* out = p.gs + static_cast<size_t>(lrow) * p.ldg + n_blk * BN;
+#pragma unroll 1
+        for (int c = 0; c < BN / 32; ++c) {
+            float v[32];
+            tmem_ld32(taddr + c * 32, v);
+            tmem_ld_wait();
+            const int col0 = gp.b_off + n_blk * BN + c * 32;          // vocabulary column of v[0]
+            if (live) {
+#pragma unroll
+                for (int i = 0; i < 32; ++i) v[i] = st.coef * exp2f(fmaf(v[i], LOG2E, -st.lse2));
+            } else {
+#pragma unroll
+                for (int i = 0; i < 32; ++i) v[i] = 0.f;
+            }
+            if (__any_sync(0xffffffffu, st.next_col < col0 + 32)) {
+                while (st.next_col < col0 + 32) {                    // duplicates add up
+                    add_at32(v, st.next_col - col0, __ldg(beta + st.cursor));
+                    ++st.cursor;
+                    st.next_col = st.cursor < p.C ? __ldg(idx + st.cursor) : IDX_SENTINEL;
+                }
+            }
+            if (col0 + 32 > p.V) {
+#pragma unroll
+                for (int i = 0; i < 32; ++i)
+                    if (col0 + i >= p.V) v[i] = 0.f;
+            }
+            for (int pl = 0; pl < p.planes; ++pl) {
+                uint32_t w[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    w[i] = pack_bf16x2(v[2 * i], v[2 * i + 1]);
+                    if (pl + 1 < p.planes) {                          // residual for the next split term
+                        __nv_bfloat162 t = *reinterpret_cast<__nv_bfloat162*>(&w[i]);
+                        v[2 * i] -= __low2float(t);
+                        v[2 * i + 1] -= __high2float(t);
+                    }
+                }
+                uint4* dst = reinterpret_cast<uint4*>(out + pl * p.plane_stride + c * 32);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) dst[q] = make_uint4(w[4 * q], w[4 * q + 1], w[4 * q + 2], w[4 * q + 3]);
+            }
+        }
+    }
+};
+
+// ------------------------------------------------------------------------------------------ DxEpi
+// S7: grad_hidden super-tile [Tb][d] = sum over vocabulary super-tiles of  G . W^T.  Partial sums live in an
+// fp32 workspace between super-tiles; the last one emits rows into grad_hidden (dtype of hidden) at the
+// token positions of the compacted rows.
+struct DxEpi {
+    struct Params {
+        float* acc;              // [Tb_pad][ld_acc] fp32
+        long ld_acc;
+        void* out;               // grad_hidden
+        long ld_out;
+        int out_fp32;
+        const int* live_rows;    // compact row -> token index
+        int first, last;         // first / last vocabulary super-tile of this token super-tile
+    };
+    struct State { int tok; };
+    static __device__ __forceinline__ State prepare(const Params& p, const GemmParams& gp, int m_blk, int,
+                                                    int row_in_tile, int M_eff) {
+        State st{-1};
+        const int lrow = m_blk * BM + row_in_tile;
+        if (p.last && lrow < M_eff) st.tok = p.live_rows[gp.tok_off + lrow];
+        return st;
+    }
+    static __device__ __forceinline__ void run(const Params& p, const GemmParams& gp, State st, uint32_t taddr,
+                                               int m_blk, int n_blk, int row_in_tile, int M_eff, uint8_t*, int) {
+        const int lrow = m_blk * BM + row_in_tile;
+        const bool live = lrow < M_eff;
+        float* acc = p.acc + static_cast<size_t>(lrow) * p.ld_acc + n_blk * BN;
+#pragma unroll 1
+        for (int c = 0; c < BN / 32; ++c) {
+            float v[32];
+            tmem_ld32(taddr + c * 32, v);
+            tmem_ld_wait();
+            const int col0 = n_blk * BN + c * 32;
+            if (live && col0 < gp.N) {                                // d % 64 == 0: chunks are all-in or all-out
+            float4* a4 = reinterpret_cast<float4*>(acc + c * 32);
+            if (!p.first) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const float4 o = a4[q];
+                    v[4 * q] += o.x; v[4 * q + 1] += o.y; v[4 * q + 2] += o.z; v[4 * q + 3] += o.w;
+                }
+            }
+            if (!p.last) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q) a4[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+            } else if (p.out_fp32) {
+                float4* o4 = reinterpret_cast<float4*>(static_cast<float*>(p.out) + static_cast<size_t>(st.tok) * p.ld_out + col0);
+#pragma unroll
+                for (int q = 0; q < 8; ++q) o4[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+            } else {
+                uint4* o4 = reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(p.out) + static_cast<size_t>(st.tok) * p.ld_out + col0);
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    o4[q] = make_uint4(pack_bf16x2(v[8 * q], v[8 * q + 1]), pack_bf16x2(v[8 * q + 2], v[8 * q + 3]),
+                                       pack_bf16x2(v[8 * q + 4], v[8 * q + 5]), pack_bf16x2(v[8 * q + 6], v[8 * q + 7]));
+            }
+            }
+        }
+    }
+};
+
+// ------------------------------------------------------------------------------------------ DwEpi
+// S8: grad_W tile += accumulator.  Output element (row, col) of this GEMM lives at gw[row*ld + col] with
+// row = row_off + tile row, col = col_off + tile col (the host maps (d,V) or (V,d) onto rows/cols).
+struct DwEpi {
+    struct Params {
+        float* gw;
+        long ld;
+        int row_off, col_off;
+        int rows_total, cols_total;
+    };
+    using State = NoState;
+    static __device__ __forceinline__ State prepare(const Params&, const GemmParams&, int, int, int, int) { return {}; }
+    static __device__ __forceinline__ void run(const Params& p, const GemmParams& gp, const State&, uint32_t taddr,
+                                               int m_blk, int n_blk, int row_in_tile, int M_eff, uint8_t*, int) {
+        const int row = p.row_off + m_blk * BM + row_in_tile;
+        const bool ok = (m_blk * BM + row_in_tile) < M_eff && row < p.rows_total;
+        float* g = p.gw + static_cast<size_t>(row) * p.ld + p.col_off + n_blk * BN;
+#pragma unroll 1
+        for (int c = 0; c < BN / 32; ++c) {
+            float v[32];
+            tmem_ld32(taddr + c * 32, v);
+            tmem_ld_wait();
+            const int lc0 = n_blk * BN + c * 32;
+            const int col0 = p.col_off + lc0;
+            if (ok && lc0 < gp.N) {
+            float4* g4 = reinterpret_cast<float4*>(g + c * 32);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                if (col0 + 4 * q < p.cols_total && lc0 + 4 * q < gp.N) {          // extents are multiples of 4
+                    float4 o = g4[q];
+                    o.x += v[4 * q]; o.y += v[4 * q + 1]; o.z += v[4 * q + 2]; o.w += v[4 * q + 3];
+                    g4[q] = o;
+                }
+            }
+            }
+        }
+    }
+};
+
+}  // namespace opd

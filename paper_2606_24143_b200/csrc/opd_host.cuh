@@ -1,0 +1,145 @@
+// Host-side plumbing of libopd: handle, workspace planner, TMA descriptor encoding, GEMM launcher.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+
+#include "../../include/opd.h"
+#include "opd_epilogues_bwd.cuh"
+#include "opd_estimators.cuh"
+
+struct opd_handle_s {
+    int device = 0;
+    int num_sms = 0;
+    bool arch_ok = false;
+    void* ws = nullptr;            // workspace in use
+    size_t ws_bytes = 0;
+    bool ws_owned = false;
+    std::string err;
+    // host-entry staging buffers (opd_loss_fwd_bwd_host)
+    void* stage = nullptr;
+    size_t stage_bytes = 0;
+    cudaStream_t host_stream = nullptr;
+    // stats of the last call
+    int n_kernels = 0, n_gemm = 0, super_rows = 0, super_cols = 0;
+    cudaEvent_t* phase_events = nullptr;
+};
+
+namespace opd {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+inline EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+// bf16 tensor [planes][rows][inner] (inner contiguous), 128-byte swizzled boxes of 64 x box_rows x 1
+inline bool make_map(CUtensorMap* m, const void* base, uint64_t inner, uint64_t rows, uint64_t planes,
+                     uint64_t row_stride_bytes, uint64_t plane_stride_bytes, uint32_t box_rows) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return false;
+    cuuint64_t dims[3] = {inner, rows, planes};
+    cuuint64_t strides[2] = {row_stride_bytes, plane_stride_bytes};
+    cuuint32_t box[3] = {64, box_rows, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+// ---------------------------------------------------------------- workspace plan
+struct Plan {
+    int T, d, V, C, planes;
+    int t_pad;            // T rounded up to 128
+    int num_n;            // vocabulary tiles of 256
+    int Tb, Vb;           // backward super-tile (rows of tokens x vocabulary columns), multiples of 128 / 256
+    int est_blocks;
+    size_t off_nlive, off_badidx, off_live_rows, off_xc, off_wsplit, off_sorted, off_perm, off_zc, off_beta,
+           off_partials, off_lse2, off_coef, off_gs, off_dxacc, off_block_sums, total;
+    size_t xc_plane, w_plane, gs_plane;   // elements per plane
+};
+
+inline int env_int(const char* name, int dflt) {
+    const char* s = std::getenv(name);
+    return (s && *s) ? std::atoi(s) : dflt;
+}
+
+inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags) {
+    Plan p{};
+    p.T = T; p.d = d; p.V = V; p.C = C; p.planes = fp32 ? 3 : 1;
+    p.t_pad = ceil_div(T, BM) * BM;
+    p.num_n = ceil_div(V, BN);
+    const int tb = env_int("OPD_TB", 4096), vb = env_int("OPD_VB", 4096);
+    p.Tb = std::min(p.t_pad, std::max(BM, tb / BM * BM));
+    p.Vb = std::min(p.num_n * BN, std::max(BN, vb / BN * BN));
+    p.est_blocks = ceil_div(T, 128);
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 1024); return r; };
+    p.off_nlive = take(4);
+    p.off_badidx = take(4);
+    p.off_live_rows = take(sizeof(int) * (size_t)p.t_pad);
+    p.xc_plane = (size_t)p.t_pad * d;
+    p.off_xc = take(2 * p.xc_plane * p.planes);
+    p.w_plane = (size_t)d * V;
+    p.off_wsplit = take(fp32 ? 2 * p.w_plane * 3 : 0);
+    p.off_sorted = take(sizeof(int) * (size_t)p.t_pad * C);
+    p.off_perm = take((size_t)p.t_pad * C);
+    p.off_zc = take(sizeof(float) * (size_t)p.t_pad * C);
+    p.off_beta = take(sizeof(float) * (size_t)p.t_pad * C);
+    p.off_partials = take(sizeof(float2) * (size_t)p.num_n * p.t_pad);
+    p.off_lse2 = take(sizeof(float) * (size_t)p.t_pad);
+    p.off_coef = take(sizeof(float) * (size_t)p.t_pad);
+    const bool bwd = !(flags & OPD_F_FWD_ONLY);
+    p.gs_plane = (size_t)p.Tb * p.Vb;
+    p.off_gs = take(bwd ? 2 * p.gs_plane * p.planes : 0);
+    p.off_dxacc = take(bwd ? sizeof(float) * (size_t)p.Tb * d : 0);
+    p.off_block_sums = take(sizeof(double) * (size_t)p.est_blocks);
+    p.total = o;
+    return p;
+}
+
+// ---------------------------------------------------------------- GEMM launcher
+template <class Epi>
+inline cudaError_t launch_gemm(opd_handle_s* h, cudaStream_t st, const CUtensorMap& tA, const CUtensorMap& tB,
+                               const GemmParams& gp, const typename Epi::Params& ep) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(gemm_kernel<Epi>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const long tiles = (long)ceil_div(gp.M, BM) * gp.num_n;
+    const int grid = (int)std::min<long>(tiles, h->num_sms);
+    if (grid <= 0) return cudaSuccess;
+    gemm_kernel<Epi><<<grid, GEMM_THREADS, GEMM_SMEM_BYTES, st>>>(tA, tB, gp, ep);
+    h->n_kernels++;
+    h->n_gemm++;
+    return cudaGetLastError();
+}
+
+inline void set_segments(GemmParams& gp, int planes) {
+    if (planes == 1) { gp.nseg = 1; gp.sa[0] = 0; gp.sb[0] = 0; return; }
+    // x = x0+x1+x2, w = w0+w1+w2 (bf16 terms): keep all products down to 2^-16 relative
+    static const unsigned char pa[6] = {0, 0, 1, 0, 2, 1}, pb[6] = {0, 1, 0, 2, 0, 1};
+    gp.nseg = 6;
+    for (int i = 0; i < 6; ++i) { gp.sa[i] = pa[i]; gp.sb[i] = pb[i]; }
+}
+
+}  // namespace opd

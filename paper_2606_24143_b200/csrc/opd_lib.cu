@@ -1,0 +1,104 @@
+// libopd — C ABI (include/opd.h) of the fused OPD loss for sm_100a.  Single translation unit:
+//   nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -shared -Xcompiler -fPIC opd_lib.cu -o libopd.so
+#include "opd_host.cuh"
+
+using namespace opd;
+
+#define OPD_FAIL(h, code, ...)                                   \
+    do {                                                         \
+        char _b[512];                                            \
+        std::snprintf(_b, sizeof _b, __VA_ARGS__);               \
+        if (h) (h)->err = _b;                                    \
+        return (code);                                           \
+    } while (0)
+
+#define OPD_CUDA(h, expr)                                                                              \
+    do {                                                                                               \
+        cudaError_t _e = (expr);                                                                       \
+        if (_e != cudaSuccess) OPD_FAIL(h, OPD_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(_e)); \
+    } while (0)
+
+extern "C" const char* opd_version(void) { return "opd-b200 0.1 (sm_100a, tcgen05/TMEM/TMA)"; }
+
+extern "C" opd_status_t opd_create(opd_handle_t* out, int device) {
+    if (!out) return OPD_ERR_BAD_ARG;
+    *out = nullptr;
+    opd_handle_s* h = new opd_handle_s();
+    h->device = device;
+    cudaDeviceProp prop;
+    cudaError_t e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) { delete h; return OPD_ERR_CUDA; }
+    h->num_sms = prop.multiProcessorCount;
+    h->arch_ok = (prop.major == 10);
+    *out = h;
+    return OPD_OK;
+}
+
+extern "C" opd_status_t opd_destroy(opd_handle_t h) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    if (h->ws_owned && h->ws) cudaFree(h->ws);
+    if (h->stage) cudaFree(h->stage);
+    if (h->host_stream) cudaStreamDestroy(h->host_stream);
+    delete h;
+    return OPD_OK;
+}
+
+extern "C" const char* opd_last_error(opd_handle_t h) { return h ? h->err.c_str() : "null handle"; }
+
+static opd_status_t check_shape(opd_handle_s* h, int T, int d, int V, int C) {
+    if (T < 1 || T >= (1 << 24)) OPD_FAIL(h, OPD_ERR_BAD_SHAPE, "T=%d out of range [1, 2^24)", T);
+    if (d < 64 || d > 16384 || d % 64) OPD_FAIL(h, OPD_ERR_BAD_SHAPE, "d=%d must be a multiple of 64 in [64,16384]", d);
+    if (V < 256 || V >= (1 << 24) || V % 8) OPD_FAIL(h, OPD_ERR_BAD_SHAPE, "V=%d must be a multiple of 8 in [256, 2^24)", V);
+    if (C < 1 || C > 64) OPD_FAIL(h, OPD_ERR_BAD_SHAPE, "cache width C=%d must be in [1,64]", C);
+    return OPD_OK;
+}
+
+static int cache_width(opd_mode_t mode, int k_or_K, int* k, int* K) {
+    if (mode == OPD_MIXED) {
+        *k = k_or_K & 0xFFFF; *K = (k_or_K >> 16) & 0xFFFF;
+        return *k > *K ? *k : *K;
+    }
+    *k = *K = k_or_K;
+    return k_or_K;
+}
+
+extern "C" size_t opd_workspace_bytes(int T, int d, int V, int C, opd_dtype_t dtype, opd_mode_t, unsigned flags) {
+    if (T < 1 || d < 64 || V < 256 || C < 1 || C > 64) return 0;
+    return make_plan(T, d, V, C, dtype == OPD_FP32, flags).total;
+}
+
+extern "C" opd_status_t opd_set_workspace(opd_handle_t h, void* ws, size_t bytes) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    if (ws && (reinterpret_cast<uintptr_t>(ws) & 255)) OPD_FAIL(h, OPD_ERR_BAD_ARG, "workspace must be 256-byte aligned");
+    if (h->ws_owned && h->ws) cudaFree(h->ws);
+    h->ws = ws; h->ws_bytes = ws ? bytes : 0; h->ws_owned = false;
+    return OPD_OK;
+}
+
+static opd_status_t ensure_workspace(opd_handle_s* h, size_t need) {
+    if (h->ws && h->ws_bytes >= need) return OPD_OK;
+    if (h->ws && !h->ws_owned) OPD_FAIL(h, OPD_ERR_WORKSPACE, "caller workspace has %zu bytes, %zu needed", h->ws_bytes, need);
+    if (h->ws) { cudaFree(h->ws); h->ws = nullptr; h->ws_bytes = 0; }
+    cudaError_t e = cudaMalloc(&h->ws, need);
+    if (e != cudaSuccess) { h->ws = nullptr; OPD_FAIL(h, OPD_ERR_WORKSPACE, "cudaMalloc(%zu) failed: %s", need, cudaGetErrorString(e)); }
+    h->ws_bytes = need; h->ws_owned = true;
+    return OPD_OK;
+}
+
+extern "C" opd_status_t opd_last_launch_stats(opd_handle_t h, int* nk, int* ng, int* sr, int* sc) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    if (nk) *nk = h->n_kernels;
+    if (ng) *ng = h->n_gemm;
+    if (sr) *sr = h->super_rows;
+    if (sc) *sc = h->super_cols;
+    return OPD_OK;
+}
+
+extern "C" opd_status_t opd_set_phase_events(opd_handle_t h, void** events) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    h->phase_events = reinterpret_cast<cudaEvent_t*>(events);
+    return OPD_OK;
+}
+
+#include "opd_lib_path.inl"
+#include "opd_lib_extra.inl"

@@ -1,0 +1,93 @@
+// Debug / verification entry points and the host-buffer entry point.  Included by opd_lib.cu.
+
+extern "C" opd_status_t opd_debug_logits(opd_handle_t h, void* cuda_stream, int T, int d, int V, opd_dtype_t dtype,
+    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, const int* cache_idx, long ld_cache, int C,
+    float* logits_out, float* gathered_out) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    if (!logits_out) OPD_FAIL(h, OPD_ERR_BAD_ARG, "logits_out is null");
+    PathIO a{};
+    a.T = T; a.d = d; a.V = V; a.dtype = dtype; a.hidden = hidden; a.ld_hidden = ld_hidden; a.W = W; a.ldw_k = ldw_k; a.ldw_v = ldw_v;
+    a.cache_idx = cache_idx; a.ld_cache = ld_cache; a.mode = OPD_FKL_TOPK; a.k_or_K = C;
+    a.dbg_logits = logits_out; a.dbg_gathered = gathered_out; a.stop_after_fwd = true; a.all_live = true;
+    return run_path(h, static_cast<cudaStream_t>(cuda_stream), a);
+}
+
+extern "C" opd_status_t opd_debug_gemm(opd_handle_t h, void* cuda_stream, int M, int N, int K, const void* A, int a_mn,
+                                       const void* B, int b_mn, float* D) {
+    if (!h || !A || !B || !D) return OPD_ERR_BAD_ARG;
+    if (!h->arch_ok) OPD_FAIL(h, OPD_ERR_ARCH, "device %d is not compute capability 10.x", h->device);
+    if (M < 1 || N < 1 || K < 1 || M % 8 || N % 8 || K % 8) OPD_FAIL(h, OPD_ERR_BAD_SHAPE, "M, N, K must be positive multiples of 8");
+    if (!get_encode_fn()) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled not available");
+    OPD_CUDA(h, cudaSetDevice(h->device));
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    CUtensorMap tA, tB;
+    bool ok = true;
+    if (a_mn) ok &= make_map(&tA, A, M, K, 1, (uint64_t)M * 2, (uint64_t)M * K * 2, MN_BOX);
+    else      ok &= make_map(&tA, A, K, M, 1, (uint64_t)K * 2, (uint64_t)M * K * 2, BM);
+    if (b_mn) ok &= make_map(&tB, B, N, K, 1, (uint64_t)N * 2, (uint64_t)N * K * 2, MN_BOX);
+    else      ok &= make_map(&tB, B, K, N, 1, (uint64_t)K * 2, (uint64_t)N * K * 2, BN);
+    if (!ok) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled failed");
+    GemmParams gp{};
+    gp.M = M; gp.N = N; gp.K = K; gp.num_n = ceil_div(N, BN); gp.group_m = 8;
+    gp.a_mn = a_mn ? 1 : 0; gp.b_mn = b_mn ? 1 : 0;
+    set_segments(gp, 1);
+    gp.tok_dim = TOK_NONE; gp.n_live = nullptr;
+    StoreEpi::Params ep{D, (long)N};
+    h->n_kernels = h->n_gemm = 0;
+    OPD_CUDA(h, launch_gemm<StoreEpi>(h, st, tA, tB, gp, ep));
+    return OPD_OK;
+}
+
+// ---------------------------------------------------------------- host-buffer entry point
+extern "C" opd_status_t opd_loss_fwd_bwd_host(opd_handle_t h, int T, int d, int V, opd_dtype_t dtype,
+    const void* hidden_h, const void* W_h, const int* idx_h, const float* lam_h, const float* old_h, const unsigned char* mask_h,
+    opd_mode_t mode, int k_or_K, unsigned flags, float norm_override,
+    float* loss_h, float* ptk_h, void* gh_h, void* gw_h, size_t* h2d_bytes, size_t* d2h_bytes) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    if (!hidden_h || !W_h || !idx_h || !lam_h || !mask_h) OPD_FAIL(h, OPD_ERR_BAD_ARG, "null host input");
+    int kf, Km;
+    const int C = cache_width(mode, k_or_K, &kf, &Km);
+    opd_status_t s = check_shape(h, T, d, V, C);
+    if (s != OPD_OK) return s;
+    OPD_CUDA(h, cudaSetDevice(h->device));
+    if (!h->host_stream) OPD_CUDA(h, cudaStreamCreateWithFlags(&h->host_stream, cudaStreamNonBlocking));
+    cudaStream_t st = h->host_stream;
+    const size_t esz = dtype == OPD_FP32 ? 4 : 2;
+    const bool bwd = !(flags & OPD_F_FWD_ONLY);
+    size_t o = 0;
+    auto take = [&](size_t b) { size_t r = o; o = align_up(o + b, 256); return r; };
+    const size_t o_hid = take((size_t)T * d * esz), o_w = take((size_t)d * V * esz), o_idx = take((size_t)T * C * 4),
+                 o_lam = take((size_t)T * C * 4), o_old = take((size_t)T * C * 4), o_mask = take(T), o_loss = take(4),
+                 o_ptk = take((size_t)T * 4), o_gh = take(bwd ? (size_t)T * d * esz : 0), o_gw = take(bwd ? (size_t)d * V * 4 : 0);
+    if (h->stage_bytes < o) {
+        if (h->stage) cudaFree(h->stage);
+        h->stage = nullptr; h->stage_bytes = 0;
+        cudaError_t e = cudaMalloc(&h->stage, o);
+        if (e != cudaSuccess) OPD_FAIL(h, OPD_ERR_WORKSPACE, "cudaMalloc(%zu) for host staging failed: %s", o, cudaGetErrorString(e));
+        h->stage_bytes = o;
+    }
+    uint8_t* sb = static_cast<uint8_t*>(h->stage);
+    size_t up = 0, down = 0;
+    auto h2d = [&](size_t off, const void* src, size_t b) { up += b; return cudaMemcpyAsync(sb + off, src, b, cudaMemcpyHostToDevice, st); };
+    OPD_CUDA(h, h2d(o_hid, hidden_h, (size_t)T * d * esz));
+    OPD_CUDA(h, h2d(o_w, W_h, (size_t)d * V * esz));
+    OPD_CUDA(h, h2d(o_idx, idx_h, (size_t)T * C * 4));
+    OPD_CUDA(h, h2d(o_lam, lam_h, (size_t)T * C * 4));
+    if (old_h) OPD_CUDA(h, h2d(o_old, old_h, (size_t)T * C * 4));
+    OPD_CUDA(h, h2d(o_mask, mask_h, T));
+    s = opd_loss_fwd_bwd(h, st, T, d, V, dtype, sb + o_hid, d, sb + o_w, V, 1, reinterpret_cast<int*>(sb + o_idx), C,
+                         reinterpret_cast<float*>(sb + o_lam), old_h ? reinterpret_cast<float*>(sb + o_old) : nullptr, sb + o_mask,
+                         mode, k_or_K, flags & ~OPD_F_GRADW_ACCUM, norm_override, reinterpret_cast<float*>(sb + o_loss),
+                         reinterpret_cast<float*>(sb + o_ptk), nullptr, nullptr, bwd ? sb + o_gh : nullptr, d,
+                         bwd ? sb + o_gw : nullptr, V, 1);
+    if (s != OPD_OK) return s;
+    auto d2h = [&](void* dst, size_t off, size_t b) { down += b; return cudaMemcpyAsync(dst, sb + off, b, cudaMemcpyDeviceToHost, st); };
+    if (loss_h) OPD_CUDA(h, d2h(loss_h, o_loss, 4));
+    if (ptk_h) OPD_CUDA(h, d2h(ptk_h, o_ptk, (size_t)T * 4));
+    if (bwd && gh_h) OPD_CUDA(h, d2h(gh_h, o_gh, (size_t)T * d * esz));
+    if (bwd && gw_h) OPD_CUDA(h, d2h(gw_h, o_gw, (size_t)d * V * 4));
+    OPD_CUDA(h, cudaStreamSynchronize(st));
+    if (h2d_bytes) *h2d_bytes = up;
+    if (d2h_bytes) *d2h_bytes = down;
+    return OPD_OK;
+}

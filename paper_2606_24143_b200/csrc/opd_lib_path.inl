@@ -1,0 +1,244 @@
+// The hot path: S0 pre-pass -> S1-S3 forward GEMM -> S4-S5 estimators -> S6-S8 backward super-tiles.
+// Included by opd_lib.cu.
+
+struct PathIO {
+    int T, d, V; opd_dtype_t dtype;
+    const void* hidden; long ld_hidden;
+    const void* W; long ldw_k, ldw_v;
+    const int* cache_idx; long ld_cache;
+    const float* lam; const float* old;
+    const unsigned char* mask;
+    opd_mode_t mode; int k_or_K; unsigned flags; float norm_override;
+    float* loss; float* per_token_kl; float* lse_out; float* slp_out;
+    void* grad_hidden; long ld_gh;
+    void* grad_W; long ldgw_k, ldgw_v;
+    // debug
+    float* dbg_logits; float* dbg_gathered; bool stop_after_fwd; bool all_live;
+};
+
+static void phase_mark(opd_handle_s* h, cudaStream_t st, int phase, int end) {
+    if (h->phase_events) cudaEventRecord(h->phase_events[2 * phase + end], st);
+}
+
+static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) {
+    if (!h->arch_ok) OPD_FAIL(h, OPD_ERR_ARCH, "device %d is not compute capability 10.x (sm_100a required, no fallback)", h->device);
+    const int T = a.T, d = a.d, V = a.V;
+    int kf, Km;
+    const int C = cache_width(a.mode, a.k_or_K, &kf, &Km);
+    if (a.mode != OPD_FKL_TOPK && a.mode != OPD_RKL_MC && a.mode != OPD_MIXED) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unknown mode %d", (int)a.mode);
+    if (a.dtype != OPD_BF16 && a.dtype != OPD_FP32) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unknown dtype %d", (int)a.dtype);
+    opd_status_t s = check_shape(h, T, d, V, C);
+    if (s != OPD_OK) return s;
+    if (a.mode == OPD_MIXED && (kf < 1 || Km < 1)) OPD_FAIL(h, OPD_ERR_BAD_SHAPE, "OPD_MIXED needs k>=1 and K>=1 (k_or_K = k | K<<16)");
+    const unsigned known = OPD_F_NO_RENORM_TEACHER | OPD_F_RENORM_STUDENT | OPD_F_GRADW_ACCUM | OPD_F_VALIDATE_IDX |
+                           OPD_F_FWD_ONLY | OPD_F_SUR_CLIP | OPD_F_SUR_A_OLD;
+    if (a.flags & ~known) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unknown flag bits 0x%x", a.flags & ~known);
+    const bool fwd_only = (a.flags & OPD_F_FWD_ONLY) || a.stop_after_fwd;
+    const bool fp32 = a.dtype == OPD_FP32;
+    const int esz = fp32 ? 4 : 2;
+    if (!a.hidden || !a.W || !a.cache_idx || (!a.stop_after_fwd && (!a.lam || !a.loss || !a.per_token_kl)))
+        OPD_FAIL(h, OPD_ERR_BAD_ARG, "null input/output pointer");
+    if (!a.all_live && !a.mask) OPD_FAIL(h, OPD_ERR_BAD_ARG, "mask is null");
+    if (a.mode != OPD_FKL_TOPK && !a.old && !a.stop_after_fwd) OPD_FAIL(h, OPD_ERR_BAD_ARG, "cache_old_logp is required for RKL_MC / MIXED");
+    if (!fwd_only && (!a.grad_hidden || !a.grad_W)) OPD_FAIL(h, OPD_ERR_BAD_ARG, "grad pointers are null (use OPD_F_FWD_ONLY)");
+    const int wl = (a.ldw_v == 1) ? 0 : ((a.ldw_k == 1) ? 1 : -1);       // 0: [d,V] row-major, 1: [V,d] row-major
+    if (wl < 0) OPD_FAIL(h, OPD_ERR_BAD_ARG, "one of ldw_k / ldw_v must be 1");
+    const long ldw = wl == 0 ? a.ldw_k : a.ldw_v;
+    if (ldw < (wl == 0 ? V : d)) OPD_FAIL(h, OPD_ERR_BAD_ARG, "W row stride %ld too small", ldw);
+    const int al = 16 / esz;
+    if ((reinterpret_cast<uintptr_t>(a.hidden) & 15) || (reinterpret_cast<uintptr_t>(a.W) & 15) || a.ld_hidden % al || ldw % al ||
+        a.ld_hidden < d)
+        OPD_FAIL(h, OPD_ERR_BAD_ARG, "hidden / W must be 16-byte aligned with row strides that are multiples of %d elements", al);
+    if (a.ld_cache < C) OPD_FAIL(h, OPD_ERR_BAD_ARG, "ld_cache %ld < C %d", a.ld_cache, C);
+    long ldgw = 0;
+    if (!fwd_only) {
+        const int gwl = (a.ldgw_v == 1) ? 0 : ((a.ldgw_k == 1) ? 1 : -1);
+        if (gwl != wl && !(wl == 0 && a.ldgw_v == 1) ) OPD_FAIL(h, OPD_ERR_BAD_ARG, "grad_W must use the same unit stride as W");
+        ldgw = wl == 0 ? a.ldgw_k : a.ldgw_v;
+        if (ldgw < (wl == 0 ? V : d) || ldgw % 4 || (reinterpret_cast<uintptr_t>(a.grad_W) & 15))
+            OPD_FAIL(h, OPD_ERR_BAD_ARG, "grad_W must be 16-byte aligned, row stride a multiple of 4 and >= the inner extent");
+        if (a.ld_gh < d || a.ld_gh % al || (reinterpret_cast<uintptr_t>(a.grad_hidden) & 15))
+            OPD_FAIL(h, OPD_ERR_BAD_ARG, "grad_hidden must be 16-byte aligned with a row stride that is a multiple of %d", al);
+    }
+    if (!get_encode_fn()) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
+
+    OPD_CUDA(h, cudaSetDevice(h->device));
+    const Plan p = make_plan(T, d, V, C, fp32, a.flags | (a.stop_after_fwd ? OPD_F_FWD_ONLY : 0));
+    s = ensure_workspace(h, p.total);
+    if (s != OPD_OK) return s;
+    h->n_kernels = h->n_gemm = 0;
+    h->super_rows = p.Tb; h->super_cols = p.Vb;
+    uint8_t* ws = static_cast<uint8_t*>(h->ws);
+    int* n_live = reinterpret_cast<int*>(ws + p.off_nlive);
+    int* bad_idx = reinterpret_cast<int*>(ws + p.off_badidx);
+    int* live_rows = reinterpret_cast<int*>(ws + p.off_live_rows);
+    __nv_bfloat16* xc = reinterpret_cast<__nv_bfloat16*>(ws + p.off_xc);
+    __nv_bfloat16* wsplit = reinterpret_cast<__nv_bfloat16*>(ws + p.off_wsplit);
+    int* sorted_idx = reinterpret_cast<int*>(ws + p.off_sorted);
+    unsigned char* perm = ws + p.off_perm;
+    float* zc = reinterpret_cast<float*>(ws + p.off_zc);
+    float* beta = reinterpret_cast<float*>(ws + p.off_beta);
+    float2* partials = reinterpret_cast<float2*>(ws + p.off_partials);
+    float* lse2 = reinterpret_cast<float*>(ws + p.off_lse2);
+    float* coef = reinterpret_cast<float*>(ws + p.off_coef);
+    __nv_bfloat16* gs = reinterpret_cast<__nv_bfloat16*>(ws + p.off_gs);
+    float* dxacc = reinterpret_cast<float*>(ws + p.off_dxacc);
+    double* block_sums = reinterpret_cast<double*>(ws + p.off_block_sums);
+
+    // ------------------------------------------------------------------ S0 pre-pass
+    phase_mark(h, st, OPD_PHASE_PREP, 0);
+    OPD_CUDA(h, cudaMemsetAsync(bad_idx, 0, 4, st));
+    OPD_CUDA(h, cudaMemsetAsync(zc, 0, sizeof(float) * (size_t)p.t_pad * C, st));
+    if (a.per_token_kl) OPD_CUDA(h, cudaMemsetAsync(a.per_token_kl, 0, sizeof(float) * T, st));
+    if (!fwd_only) {
+        OPD_CUDA(h, cudaMemset2DAsync(a.grad_hidden, (size_t)a.ld_gh * esz, 0, (size_t)d * esz, T, st));
+        if (!(a.flags & OPD_F_GRADW_ACCUM))
+            OPD_CUDA(h, cudaMemset2DAsync(a.grad_W, (size_t)ldgw * 4, 0, (size_t)(wl == 0 ? V : d) * 4, wl == 0 ? d : V, st));
+    }
+    k_compact<<<1, 1024, 0, st>>>(a.mask, T, a.all_live ? 1 : 0, live_rows, n_live);
+    k_gather_rows<<<p.t_pad, 256, 0, st>>>(a.hidden, a.ld_hidden, fp32 ? 1 : 0, d, p.t_pad, live_rows, n_live, xc, (long)p.xc_plane);
+    k_sort_cache<<<ceil_div(T, 8), 256, 0, st>>>(a.cache_idx, a.ld_cache, a.mask, (int)a.mode, kf, Km, C, V, live_rows, n_live,
+                                                 sorted_idx, perm, bad_idx);
+    h->n_kernels += 3;
+    const __nv_bfloat16* wq = static_cast<const __nv_bfloat16*>(a.W);   // bf16 operand planes of W
+    long ldwq = ldw;
+    size_t wq_plane = 0;
+    if (fp32) {
+        const int rows = wl == 0 ? d : V, cols = wl == 0 ? V : d;
+        k_split_matrix<<<h->num_sms * 8, 256, 0, st>>>(static_cast<const float*>(a.W), ldw, rows, cols, wsplit, (long)p.w_plane);
+        h->n_kernels++;
+        wq = wsplit; ldwq = cols; wq_plane = p.w_plane;
+    }
+    OPD_CUDA(h, cudaGetLastError());
+    phase_mark(h, st, OPD_PHASE_PREP, 1);
+
+    // ------------------------------------------------------------------ tensor maps
+    const uint64_t np = p.planes;
+    CUtensorMap m_xc_k, m_xc_mn, m_w_fwd, m_w_dx, m_gs_k, m_gs_mn;
+    bool ok = true;
+    // Xc [t_pad][d]: K-major A of the logits GEMMs (box 64 x 128); MN-major operand of the grad_W GEMM (box 64 x 64)
+    ok &= make_map(&m_xc_k, xc, d, p.t_pad, np, (uint64_t)d * 2, p.xc_plane * 2, BM);
+    ok &= make_map(&m_xc_mn, xc, d, p.t_pad, np, (uint64_t)d * 2, p.xc_plane * 2, MN_BOX);
+    const uint64_t wplane_b = fp32 ? wq_plane * 2 : (uint64_t)ldwq * 2 * (wl == 0 ? d : V);
+    if (wl == 0) {   // W [d][V]: logits B is MN-major (n = v contiguous); dX B is K-major (k = v contiguous)
+        ok &= make_map(&m_w_fwd, wq, V, d, np, (uint64_t)ldwq * 2, wplane_b, MN_BOX);
+        ok &= make_map(&m_w_dx, wq, V, d, np, (uint64_t)ldwq * 2, wplane_b, BN);
+    } else {         // W [V][d]: logits B is K-major; dX B is MN-major (n = d contiguous, k = v rows)
+        ok &= make_map(&m_w_fwd, wq, d, V, np, (uint64_t)ldwq * 2, wplane_b, BN);
+        ok &= make_map(&m_w_dx, wq, d, V, np, (uint64_t)ldwq * 2, wplane_b, MN_BOX);
+    }
+    if (!fwd_only) {
+        ok &= make_map(&m_gs_k, gs, p.Vb, p.Tb, np, (uint64_t)p.Vb * 2, p.gs_plane * 2, BM);
+        ok &= make_map(&m_gs_mn, gs, p.Vb, p.Tb, np, (uint64_t)p.Vb * 2, p.gs_plane * 2, MN_BOX);
+    }
+    if (!ok) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled failed");
+
+    // ------------------------------------------------------------------ S1-S3 forward
+    phase_mark(h, st, OPD_PHASE_FWD, 0);
+    {
+        GemmParams gp{};
+        gp.M = T; gp.N = V; gp.K = d; gp.num_n = p.num_n;
+        gp.group_m = std::max(1, env_int("OPD_GROUP_M", 16));
+        gp.a_mn = 0; gp.b_mn = (wl == 0); gp.a_off = 0; gp.b_off = 0; gp.ka_off = 0; gp.kb_off = 0;
+        set_segments(gp, p.planes);
+        gp.tok_dim = TOK_M; gp.tok_off = 0; gp.n_live = n_live;
+        FwdEpi::Params ep{partials, p.t_pad, sorted_idx, zc, C, V, a.dbg_logits};
+        OPD_CUDA(h, launch_gemm<FwdEpi>(h, st, m_xc_k, m_w_fwd, gp, ep));
+    }
+    phase_mark(h, st, OPD_PHASE_FWD, 1);
+    if (a.stop_after_fwd) {
+        if (a.dbg_gathered) {
+            k_unsort_gather<<<ceil_div(T * C, 256), 256, 0, st>>>(zc, perm, T, C, a.dbg_gathered);
+            h->n_kernels++;
+        }
+        OPD_CUDA(h, cudaGetLastError());
+        return OPD_OK;
+    }
+
+    // ------------------------------------------------------------------ S4-S5 estimators, loss
+    phase_mark(h, st, OPD_PHASE_EST, 0);
+    {
+        EstParams e{};
+        e.partials = partials; e.num_n = p.num_n; e.t_pad = p.t_pad; e.zc = zc; e.perm = perm;
+        e.lam = a.lam; e.old = a.old; e.ld_cache = a.ld_cache; e.mask = a.mask; e.live_rows = live_rows; e.n_live = n_live;
+        e.mode = (int)a.mode; e.k_fkl = kf; e.K_mc = Km; e.C = C; e.flags = a.flags; e.norm_override = a.norm_override;
+        e.lse2 = lse2; e.coef = coef; e.beta = beta; e.per_token_kl = a.per_token_kl; e.lse_out = a.lse_out; e.slp_out = a.slp_out;
+        e.block_sums = block_sums;
+        k_estimator<<<p.est_blocks, 128, 0, st>>>(e);
+        k_loss_final<<<1, 256, 0, st>>>(block_sums, p.est_blocks, n_live, a.norm_override, a.loss);
+        h->n_kernels += 2;
+        OPD_CUDA(h, cudaGetLastError());
+    }
+    phase_mark(h, st, OPD_PHASE_EST, 1);
+
+    // ------------------------------------------------------------------ S6-S8 backward, super-tile by super-tile
+    phase_mark(h, st, OPD_PHASE_BWD, 0);
+    if (!fwd_only) {
+        const int nvb = ceil_div(V, p.Vb);
+        for (int tb0 = 0; tb0 < T; tb0 += p.Tb) {
+            const int Tb = std::min(p.Tb, p.t_pad - tb0);
+            for (int vi = 0; vi < nvb; ++vi) {
+                const int vb0 = vi * p.Vb;
+                const int Vb = std::min(p.Vb, V - vb0);
+                {   // S6: G super-tile = softmax-gradient of the recomputed logits (never leaves L2)
+                    GemmParams gp{};
+                    gp.M = Tb; gp.N = Vb; gp.K = d; gp.num_n = ceil_div(Vb, BN); gp.group_m = 1 << 20;
+                    gp.a_mn = 0; gp.b_mn = (wl == 0); gp.a_off = tb0; gp.b_off = vb0; gp.ka_off = 0; gp.kb_off = 0;
+                    set_segments(gp, p.planes);
+                    gp.tok_dim = TOK_M; gp.tok_off = tb0; gp.n_live = n_live;
+                    GEpi::Params ep{gs, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V};
+                    OPD_CUDA(h, launch_gemm<GEpi>(h, st, m_xc_k, m_w_fwd, gp, ep));
+                }
+                {   // S7: grad_hidden[tb] += G . W[:, vb]^T
+                    GemmParams gp{};
+                    gp.M = Tb; gp.N = d; gp.K = Vb; gp.num_n = ceil_div(d, BN); gp.group_m = 1 << 20;
+                    gp.a_mn = 0; gp.b_mn = (wl == 1); gp.a_off = 0; gp.b_off = 0; gp.ka_off = 0; gp.kb_off = vb0;
+                    set_segments(gp, p.planes);
+                    gp.tok_dim = TOK_M; gp.tok_off = tb0; gp.n_live = n_live;
+                    DxEpi::Params ep{dxacc, (long)d, a.grad_hidden, a.ld_gh, fp32 ? 1 : 0, live_rows, vi == 0, vi == nvb - 1};
+                    OPD_CUDA(h, launch_gemm<DxEpi>(h, st, m_gs_k, m_w_dx, gp, ep));
+                }
+                {   // S8: grad_W[:, vb] += hidden[tb]^T . G
+                    GemmParams gp{};
+                    gp.group_m = 1 << 20; gp.tok_dim = TOK_K; gp.tok_off = tb0; gp.n_live = n_live; gp.K = Tb;
+                    gp.a_mn = 1; gp.b_mn = 1;
+                    set_segments(gp, p.planes);
+                    DwEpi::Params ep{};
+                    ep.gw = static_cast<float*>(a.grad_W); ep.ld = ldgw;
+                    if (wl == 0) {   // rows = d (A = Xc^T), cols = v (B = G)
+                        gp.M = d; gp.N = Vb; gp.num_n = ceil_div(Vb, BN);
+                        gp.a_off = 0; gp.ka_off = tb0; gp.b_off = 0; gp.kb_off = 0;
+                        ep.row_off = 0; ep.col_off = vb0; ep.rows_total = d; ep.cols_total = V;
+                        OPD_CUDA(h, launch_gemm<DwEpi>(h, st, m_xc_mn, m_gs_mn, gp, ep));
+                    } else {         // rows = v (A = G^T), cols = d (B = Xc)
+                        gp.M = Vb; gp.N = d; gp.num_n = ceil_div(d, BN);
+                        gp.a_off = 0; gp.ka_off = 0; gp.b_off = 0; gp.kb_off = tb0;
+                        ep.row_off = vb0; ep.col_off = 0; ep.rows_total = V; ep.cols_total = d;
+                        OPD_CUDA(h, launch_gemm<DwEpi>(h, st, m_gs_mn, m_xc_mn, gp, ep));
+                    }
+                }
+            }
+        }
+    }
+    phase_mark(h, st, OPD_PHASE_BWD, 1);
+
+    if (a.flags & OPD_F_VALIDATE_IDX) {
+        int bad = 0;
+        OPD_CUDA(h, cudaMemcpyAsync(&bad, bad_idx, 4, cudaMemcpyDeviceToHost, st));
+        OPD_CUDA(h, cudaStreamSynchronize(st));
+        if (bad) OPD_FAIL(h, OPD_ERR_BAD_INDEX, "a cache index of a live row is outside [0, %d)", V);
+    }
+    return OPD_OK;
+}
+
+extern "C" opd_status_t opd_loss_fwd_bwd(opd_handle_t h, void* cuda_stream, int T, int d, int V, opd_dtype_t dtype,
+    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, const int* cache_idx, long ld_cache,
+    const float* cache_teacher_logp, const float* cache_old_logp, const unsigned char* mask, opd_mode_t mode, int k_or_K,
+    unsigned flags, float norm_override, float* loss, float* per_token_kl, float* lse_out, float* student_logp_out,
+    void* grad_hidden, long ld_gh, void* grad_W, long ldgw_k, long ldgw_v) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    PathIO a{T, d, V, dtype, hidden, ld_hidden, W, ldw_k, ldw_v, cache_idx, ld_cache, cache_teacher_logp, cache_old_logp, mask,
+             mode, k_or_K, flags, norm_override, loss, per_token_kl, lse_out, student_logp_out, grad_hidden, ld_gh,
+             grad_W, ldgw_k, ldgw_v, nullptr, nullptr, false, false};
+    return run_path(h, static_cast<cudaStream_t>(cuda_stream), a);
+}

@@ -1,0 +1,249 @@
+"""ctypes binding of libopd.so (include/opd.h).  Argument marshalling only: every step of the path
+runs in the library's CUDA kernels.  torch is used for device memory and streams.
+
+There is no CPU fallback: if the shared library is missing, or the device is not sm_100, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, c_char_p, c_float, c_int, c_long, c_size_t, c_ubyte, c_uint, c_void_p
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libopd.so")
+
+OPD_OK = 0
+ERR_BAD_ARG, ERR_BAD_SHAPE, ERR_BAD_INDEX, ERR_WORKSPACE, ERR_ARCH, ERR_CUDA = -1, -2, -3, -4, -5, -6
+FKL_TOPK, RKL_MC, MIXED = 0, 1, 2
+BF16, FP32 = 0, 1
+F_NO_RENORM_TEACHER, F_RENORM_STUDENT, F_GRADW_ACCUM, F_VALIDATE_IDX, F_FWD_ONLY = 1, 2, 4, 16, 32
+F_SUR_CLIP, F_SUR_A_OLD = 64, 128
+N_PHASES = 4
+PHASE_NAMES = ("prep", "fwd", "est", "bwd")
+
+EXPORTS = ("opd_create", "opd_destroy", "opd_last_error", "opd_version", "opd_workspace_bytes", "opd_set_workspace",
+           "opd_loss_fwd_bwd", "opd_loss_fwd_bwd_host", "opd_debug_logits", "opd_debug_gemm", "opd_last_launch_stats",
+           "opd_set_phase_events")
+
+_lib = None
+
+
+class OpdError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"libopd status {status}: {msg}")
+        self.status = status
+
+
+def load_library():
+    """Load libopd.so (built in-tree by paper_2606_24143_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise OpdError(ERR_CUDA, f"{LIB_PATH} not built: run `python -m paper_2606_24143_b200.build` (no CPU fallback exists)")
+    lib = ctypes.CDLL(LIB_PATH)
+    lib.opd_create.argtypes = [POINTER(c_void_p), c_int]
+    lib.opd_create.restype = c_int
+    lib.opd_destroy.argtypes = [c_void_p]
+    lib.opd_destroy.restype = c_int
+    lib.opd_last_error.argtypes = [c_void_p]
+    lib.opd_last_error.restype = c_char_p
+    lib.opd_version.restype = c_char_p
+    lib.opd_workspace_bytes.argtypes = [c_int, c_int, c_int, c_int, c_int, c_int, c_uint]
+    lib.opd_workspace_bytes.restype = c_size_t
+    lib.opd_set_workspace.argtypes = [c_void_p, c_void_p, c_size_t]
+    lib.opd_set_workspace.restype = c_int
+    lib.opd_loss_fwd_bwd.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int,
+                                     c_void_p, c_long, c_void_p, c_long, c_long, c_void_p, c_long, c_void_p, c_void_p, c_void_p,
+                                     c_int, c_int, c_uint, c_float, c_void_p, c_void_p, c_void_p, c_void_p,
+                                     c_void_p, c_long, c_void_p, c_long, c_long]
+    lib.opd_loss_fwd_bwd.restype = c_int
+    lib.opd_loss_fwd_bwd_host.argtypes = [c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
+                                          c_void_p, c_int, c_int, c_uint, c_float, c_void_p, c_void_p, c_void_p, c_void_p,
+                                          POINTER(c_size_t), POINTER(c_size_t)]
+    lib.opd_loss_fwd_bwd_host.restype = c_int
+    lib.opd_debug_logits.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_long, c_void_p, c_long, c_long,
+                                     c_void_p, c_long, c_int, c_void_p, c_void_p]
+    lib.opd_debug_logits.restype = c_int
+    lib.opd_debug_gemm.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_void_p, c_int, c_void_p, c_int, c_void_p]
+    lib.opd_debug_gemm.restype = c_int
+    lib.opd_last_launch_stats.argtypes = [c_void_p, POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(c_int)]
+    lib.opd_last_launch_stats.restype = c_int
+    lib.opd_set_phase_events.argtypes = [c_void_p, c_void_p]
+    lib.opd_set_phase_events.restype = c_int
+    _lib = lib
+    return lib
+
+
+def _ptr(t):
+    return None if t is None else c_void_p(t.data_ptr())
+
+
+def _dtype_code(t: torch.Tensor) -> int:
+    if t.dtype == torch.bfloat16:
+        return BF16
+    if t.dtype == torch.float32:
+        return FP32
+    raise OpdError(ERR_BAD_ARG, f"unsupported dtype {t.dtype}")
+
+
+def _w_strides(W: torch.Tensor, d: int):
+    """W is either [d,V] (v contiguous) or a [V,d] weight passed as W.t() view / with layout='vd'."""
+    if W.shape[0] != d:
+        raise OpdError(ERR_BAD_SHAPE, f"W must be logical [d,V]; got {tuple(W.shape)} with d={d} (pass weight.t() for a [V,d] weight)")
+    return W.stride(0), W.stride(1)
+
+
+class Handle:
+    """One libopd handle (owns its device workspace).  One per thread / stream."""
+
+    def __init__(self, device: int | None = None):
+        self.lib = load_library()
+        if device is None:
+            device = torch.cuda.current_device()
+        self.device = device
+        self._h = c_void_p()
+        st = self.lib.opd_create(ctypes.byref(self._h), device)
+        if st != OPD_OK:
+            raise OpdError(st, "opd_create failed")
+        self._events = None
+
+    def close(self):
+        if self._h:
+            self.lib.opd_destroy(self._h)
+            self._h = c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st: int):
+        if st != OPD_OK:
+            raise OpdError(st, self.lib.opd_last_error(self._h).decode())
+
+    def workspace_bytes(self, T, d, V, C, dtype=BF16, mode=RKL_MC, flags=0) -> int:
+        return int(self.lib.opd_workspace_bytes(T, d, V, C, dtype, mode, flags))
+
+    def launch_stats(self) -> dict:
+        a, b, c, e = c_int(), c_int(), c_int(), c_int()
+        self.lib.opd_last_launch_stats(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c), ctypes.byref(e))
+        return dict(kernels=a.value, gemm_kernels=b.value, super_rows=c.value, super_cols=e.value)
+
+    # ------------------------------------------------------------------ phase timing
+    def enable_phase_timing(self, on: bool = True):
+        if on:
+            self._events = [torch.cuda.Event(enable_timing=True) for _ in range(2 * N_PHASES)]
+            for e in self._events:           # force creation of the underlying cudaEvent_t
+                e.record()
+            arr = (c_void_p * (2 * N_PHASES))(*[c_void_p(e.cuda_event) for e in self._events])
+            self._event_arr = arr
+            self.lib.opd_set_phase_events(self._h, ctypes.cast(arr, c_void_p))
+        else:
+            self._events = None
+            self.lib.opd_set_phase_events(self._h, None)
+
+    def phase_times_ms(self) -> dict:
+        torch.cuda.synchronize()
+        return {PHASE_NAMES[i]: self._events[2 * i].elapsed_time(self._events[2 * i + 1]) for i in range(N_PHASES)}
+
+    # ------------------------------------------------------------------ the hot path
+    def loss_fwd_bwd(self, hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K, flags=0,
+                     norm_override=0.0, grad_hidden=None, grad_W=None, want_lse=False, want_student_logp=False, stream=None):
+        """opd_loss_fwd_bwd(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K)
+        -> dict(loss, per_token_kl, grad_hidden, grad_W[, lse, student_logp]).  All tensors live on the GPU.
+        W is the logical [d,V] matrix (any of the two layouts through its strides)."""
+        T, d = hidden.shape
+        V = W.shape[1]
+        dt = _dtype_code(hidden)
+        if W.dtype != hidden.dtype:
+            raise OpdError(ERR_BAD_ARG, "hidden and W must have the same dtype")
+        ldk, ldv = _w_strides(W, d)
+        dev = hidden.device
+        fwd_only = bool(flags & F_FWD_ONLY)
+        loss = torch.empty(1, dtype=torch.float32, device=dev)
+        ptk = torch.empty(T, dtype=torch.float32, device=dev)
+        lse = torch.empty(T, dtype=torch.float32, device=dev) if want_lse else None
+        slp = torch.full(tuple(cache_idx.shape), float("nan"), dtype=torch.float32, device=dev) if want_student_logp else None
+        if not fwd_only:
+            if grad_hidden is None:
+                grad_hidden = torch.empty_like(hidden)
+            if grad_W is None:
+                grad_W = torch.empty_strided(tuple(W.shape), (ldk, ldv), dtype=torch.float32, device=dev)
+        s = torch.cuda.current_stream(dev).cuda_stream if stream is None else stream
+        gk, gv = (grad_W.stride(0), grad_W.stride(1)) if grad_W is not None else (0, 0)
+        st = self.lib.opd_loss_fwd_bwd(
+            self._h, c_void_p(s), T, d, V, dt, _ptr(hidden), hidden.stride(0), _ptr(W), ldk, ldv,
+            _ptr(cache_idx), cache_idx.stride(0), _ptr(cache_teacher_logp), _ptr(cache_old_logp), _ptr(mask),
+            mode, k_or_K, flags, float(norm_override), _ptr(loss), _ptr(ptk), _ptr(lse), _ptr(slp),
+            _ptr(grad_hidden), grad_hidden.stride(0) if grad_hidden is not None else 0, _ptr(grad_W), gk, gv)
+        self._check(st)
+        return dict(loss=loss, per_token_kl=ptk, grad_hidden=grad_hidden, grad_W=grad_W, lse=lse, student_logp=slp)
+
+    def loss_fwd_bwd_host(self, hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K, flags=0,
+                          norm_override=0.0, out=None):
+        """Same call with HOST tensors (pinned or pageable, dense); copies in, runs, copies out, synchronises.
+        `out`: optional dict of preallocated host tensors (loss, per_token_kl, grad_hidden, grad_W)."""
+        T, d = hidden.shape
+        V = W.shape[1]
+        dt = _dtype_code(hidden)
+        fwd_only = bool(flags & F_FWD_ONLY)
+        if out is None:
+            out = dict(loss=torch.empty(1, dtype=torch.float32), per_token_kl=torch.empty(T, dtype=torch.float32),
+                       grad_hidden=None if fwd_only else torch.empty_like(hidden),
+                       grad_W=None if fwd_only else torch.empty(d, V, dtype=torch.float32))
+        up, down = c_size_t(), c_size_t()
+        st = self.lib.opd_loss_fwd_bwd_host(
+            self._h, T, d, V, dt, _ptr(hidden), _ptr(W), _ptr(cache_idx), _ptr(cache_teacher_logp), _ptr(cache_old_logp),
+            _ptr(mask), mode, k_or_K, flags, float(norm_override), _ptr(out["loss"]), _ptr(out["per_token_kl"]),
+            _ptr(out.get("grad_hidden")), _ptr(out.get("grad_W")), ctypes.byref(up), ctypes.byref(down))
+        self._check(st)
+        out["h2d_bytes"], out["d2h_bytes"] = up.value, down.value
+        return out
+
+    # ------------------------------------------------------------------ debug entries
+    def debug_logits(self, hidden, W, cache_idx):
+        T, d = hidden.shape
+        V = W.shape[1]
+        ldk, ldv = _w_strides(W, d)
+        C = cache_idx.shape[1]
+        logits = torch.empty(T, V, dtype=torch.float32, device=hidden.device)
+        gathered = torch.empty(T, C, dtype=torch.float32, device=hidden.device)
+        s = torch.cuda.current_stream(hidden.device).cuda_stream
+        st = self.lib.opd_debug_logits(self._h, c_void_p(s), T, d, V, _dtype_code(hidden), _ptr(hidden), hidden.stride(0), _ptr(W),
+                                       ldk, ldv, _ptr(cache_idx), cache_idx.stride(0), C, _ptr(logits), _ptr(gathered))
+        self._check(st)
+        return logits, gathered
+
+    def debug_gemm(self, A, B, a_mn_major=False, b_mn_major=False):
+        """D = A_logical[M,K] @ B_logical[N,K]^T (fp32).  A is stored [M,K] (or [K,M] if a_mn_major), same for B."""
+        if a_mn_major:
+            K, M = A.shape
+        else:
+            M, K = A.shape
+        N = B.shape[1] if b_mn_major else B.shape[0]
+        D = torch.empty(M, N, dtype=torch.float32, device=A.device)
+        s = torch.cuda.current_stream(A.device).cuda_stream
+        st = self.lib.opd_debug_gemm(self._h, c_void_p(s), M, N, K, _ptr(A), int(a_mn_major), _ptr(B), int(b_mn_major), _ptr(D))
+        self._check(st)
+        return D
+
+
+_default = {}
+
+
+def default_handle(device: int | None = None) -> Handle:
+    if device is None:
+        device = torch.cuda.current_device()
+    if device not in _default:
+        _default[device] = Handle(device)
+    return _default[device]
+
+
+def opd_loss_fwd_bwd(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K, **kw):
+    """Module-level convenience: the north-star signature on the default handle of the current device."""
+    return default_handle(hidden.device.index).loss_fwd_bwd(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp,
+                                                            mask, mode, k_or_K, **kw)
