@@ -1,0 +1,312 @@
+#!/usr/bin/env python
+"""bench.py — fused OPD loss forward+backward throughput on B200 (metric of BASELINE.json).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (pre-pass, forward contraction + LSE + gather, estimators,
+backward super-tiles) over one batch of seeded synthetic input.  Prints ONE JSON line (rank 0).
+Under torchrun (N>1) every rank runs its own token shard (replicas of W, no data-path collective:
+DESIGN.md "Multi-GPU"), timing = max over ranks, value = tokens of all ranks / that time ("weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "OPD loss fwd+bwd tokens/s on 1 B200; % of dense BF16 tensor peak"
+UNIT = "live tokens/s"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        j = json.load(open(p))
+        return dict(burst=float(j["bf16_tflops"]), sustained=float(j.get("bf16_tflops_sustained", j["bf16_tflops"])),
+                    hbm=float(j["hbm_gbs"]), src="measured")
+    return dict(burst=1590.0, sustained=1400.0, hbm=6650.0, src="fallback")
+
+
+def workload(cfg_id: int, args):
+    from paper_2606_24143_b200 import synth
+    cfg = dict(synth.CONFIGS[cfg_id])
+    if args.tokens:
+        cfg["T"] = args.tokens
+    return cfg
+
+
+def pick_cache(inp, cfg, mode_name):
+    from paper_2606_24143_b200 import opd, synth
+    if mode_name == "fkl":
+        return opd.FKL_TOPK, inp["topk_idx"], inp["topk_logq"], None, cfg["k"]
+    if mode_name == "mixed":
+        idx, lam, old, kk = synth.mixed_cache(inp)
+        return opd.MIXED, idx, lam, old, kk
+    return opd.RKL_MC, inp["mc_idx"], inp["mc_logq"], inp["mc_logp_old"], cfg["K"]
+
+
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, gpu: int):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            out = self.p.communicate(timeout=5)[0]
+        except Exception:
+            out = ""
+        sm, mx, pw, reasons = [], [], [], set()
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
+        return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w=float(np.median(pw)), samples=len(sm),
+                    reasons=sorted(reasons))
+
+
+def to_np(t):
+    if t is None:
+        return None
+    t = t.detach().cpu()
+    return t.double().numpy() if t.is_floating_point() else t.numpy()
+
+
+def oracle_sample(inp, mode, idx, lam, old, kk, n_rows: int):
+    """The fp64 oracle as it stands on the first n_rows live tokens of the workload (full d and V), forward+backward."""
+    from oracle import opd_oracle as O
+    mask = to_np(inp["mask"])
+    rows = np.flatnonzero(mask)[:n_rows]
+    X, W = to_np(inp["hidden"][: int(rows.max()) + 1]), to_np(inp["W"])
+    t0 = time.perf_counter()
+    O.opd_oracle(X, W, to_np(idx[: X.shape[0]]), to_np(lam[: X.shape[0]]), None if old is None else to_np(old[: X.shape[0]]),
+                 mask[: X.shape[0]], mode, kk, rows=list(rows))
+    return len(rows), time.perf_counter() - t0
+
+
+def cpu_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p["num_threads"] for p in threadpool_info() if p.get("user_api") == "blas"]
+        return int(max(n)) if n else os.cpu_count()
+    except Exception:
+        return os.cpu_count()
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    cfg = workload(args.config, args)
+    gen = dict(cfg)
+    gen["T"] = min(cfg["T"], 2048)                 # the oracle only sees a bounded sample of the workload's rows
+    from paper_2606_24143_b200 import synth
+    inp = synth.make_inputs(gen, c=args.config, device=dev)
+    mode, idx, lam, old, kk = pick_cache(inp, gen, args.mode)
+    inp = {k: (v.cpu() if isinstance(v, torch.Tensor) else v) for k, v in inp.items()}
+    idx, lam, old = idx.cpu(), lam.cpu(), (None if old is None else old.cpu())
+    n, dt = oracle_sample(inp, mode, idx, lam, old, kk, 2)       # calibration
+    rows = int(max(2, min(256, args.ref_seconds / max(dt / n, 1e-6))))
+    for _ in range(args.warmup if args.warmup < 2 else 1):
+        oracle_sample(inp, mode, idx, lam, old, kk, rows)
+    tot_t, tot_n = 0.0, 0
+    for _ in range(args.steps):
+        n, dt = oracle_sample(inp, mode, idx, lam, old, kk, rows)
+        tot_t += dt; tot_n += n
+    v = tot_n / tot_t
+    sample = f"{rows} live tokens of {cfg['name']} per step (full d={cfg['d']}, V={cfg['V']}), forward+backward incl. grad_W, numpy fp64"
+    line = dict(impl="reference", metric=METRIC, value=v, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=1e3 * tot_t / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                data="synthetic", config=dict(workload=f"{cfg['name']} {args.mode}", T=cfg["T"], d=cfg["d"], V=cfg["V"]),
+                cpu_baseline=dict(value=v, unit=UNIT, cores=cpu_threads(), kind="oracle", sample=sample),
+                e2e=dict(value=v, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1..5); 4 = the config the metric is quoted on")
+    ap.add_argument("--mode", default=None, choices=["fkl", "mc", "mixed"])
+    ap.add_argument("--tokens", type=int, default=0, help="override T (debugging)")
+    ap.add_argument("--sigma", type=float, default=None)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--ref-seconds", type=float, default=12.0)
+    ap.add_argument("--traffic-json", default=os.path.join(ROOT, "profiles", "traffic.json"))
+    args = ap.parse_args()
+    if args.mode is None:
+        args.mode = "mixed" if args.config == 5 else "mc"
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the OPD path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2606_24143_b200 import opd, synth
+    cfg = workload(args.config, args)
+    inp = synth.make_inputs(cfg, c=args.config + 10 * rank, device=dev, sigma=args.sigma)
+    mode, idx, lam, old, kk = pick_cache(inp, cfg, args.mode)
+    T, d, V = cfg["T"], cfg["d"], cfg["V"]
+    n_live = int((inp["mask"] != 0).sum().item())
+    h = opd.Handle(local)
+    gh = torch.empty_like(inp["hidden"])
+    gw = torch.empty(d, V, dtype=torch.float32, device=dev)
+
+    def step():
+        return h.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, grad_hidden=gh, grad_W=gw)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        r = step()
+    barrier()
+    stats = h.launch_stats()
+    h.enable_phase_timing(True)
+    phase_ms = {k: 0.0 for k in opd.PHASE_NAMES}
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    ev[0].record()
+    for i in range(args.steps):
+        r = step()
+        ev[i + 1].record()
+        if i == args.steps - 1:
+            pass
+    barrier()
+    total_ms = ev[0].elapsed_time(ev[-1])
+    pm = h.phase_times_ms()                      # phases of the last timed step
+    h.enable_phase_timing(False)
+    clocks = sampler.stop() if sampler else None
+    loss_val = float(r["loss"].item())
+    if dist is not None:
+        t = torch.tensor([total_ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        nl = torch.tensor([n_live], device=dev, dtype=torch.int64)
+        dist.all_reduce(nl)
+        n_live_all = int(nl.item())
+    else:
+        n_live_all = n_live
+    ms_per_step = total_ms / args.steps
+    value = n_live_all / (ms_per_step * 1e-3)
+
+    # ---- e2e: same call through the C ABI with HOST buffers (H2D + D2H inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        hh = {k: inp[k].cpu().pin_memory() for k in ("hidden", "W", "mask")}
+        hidx, hlam = idx.cpu().pin_memory(), lam.cpu().pin_memory()
+        hold = None if old is None else old.cpu().pin_memory()
+        out = dict(loss=torch.empty(1).pin_memory(), per_token_kl=torch.empty(T).pin_memory(),
+                   grad_hidden=torch.empty(T, d, dtype=inp["hidden"].dtype).pin_memory(),
+                   grad_W=torch.empty(d, V, dtype=torch.float32).pin_memory())
+        del gw, gh
+        torch.cuda.empty_cache()
+        n_e2e = max(1, min(args.steps, 3))
+        h.loss_fwd_bwd_host(hh["hidden"], hh["W"], hidx, hlam, hold, hh["mask"], mode, kk, out=out)   # warm-up (allocates staging)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            o = h.loss_fwd_bwd_host(hh["hidden"], hh["W"], hidx, hlam, hold, hh["mask"], mode, kk, out=out)
+        barrier()
+        dt = (time.perf_counter() - t0) / n_e2e
+        if dist is not None:
+            t = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = dict(value=n_live_all / dt, unit=UNIT, h2d_bytes_per_step=int(o["h2d_bytes"]), d2h_bytes_per_step=int(o["d2h_bytes"]),
+                   steps=n_e2e, ms_per_step=dt * 1e3, loss=float(out["loss"].item()))
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    pk = peaks()
+    gemm_ms = pm["fwd"] + pm["bwd"]
+    flops_exec = 8.0 * d * V * n_live            # logits + recomputed logits + dX + dW  (2 d V each)
+    ach = flops_exec / (gemm_ms * 1e-3) / 1e12
+    traffic = None
+    if os.path.exists(args.traffic_json):
+        try:
+            tj = json.load(open(args.traffic_json))
+            traffic = tj.get(f"C{args.config}", {}).get("dram_bytes_per_launch")
+        except Exception:
+            traffic = None
+    roofline = dict(bound="tensor", achieved=ach, peak=pk["sustained"], unit="TFLOP/s", frac=ach / pk["sustained"], traffic=traffic,
+                    kernel="opd::gemm_kernel<*> (logits, G re-formation, grad_hidden, grad_W: one tcgen05 core, four epilogues)",
+                    flops_per_step=flops_exec, gemm_launches_per_step=stats["gemm_kernels"], gemm_ms_per_step=gemm_ms,
+                    peak_kind=f"bf16_tflops_sustained of {pk['src']} (kernel timed inside a long step); burst peak {pk['burst']}",
+                    frac_of_burst=ach / pk["burst"])
+    whole = flops_exec / (ms_per_step * 1e-3) / 1e12
+    cpu = None
+    if not args.no_cpu:
+        cinp = {k: (v.cpu() if isinstance(v, torch.Tensor) else v) for k, v in inp.items() if k in ("hidden", "W", "mask")}
+        cidx, clam, cold = idx[:4096].cpu(), lam[:4096].cpu(), (None if old is None else old[:4096].cpu())
+        cinp["hidden"] = cinp["hidden"][:4096]; cinp["mask"] = cinp["mask"][:4096]
+        n, dt = oracle_sample(cinp, mode, cidx, clam, cold, kk, 2)
+        rows = int(max(2, min(256, args.ref_seconds / max(dt / n, 1e-6))))
+        n, dt = oracle_sample(cinp, mode, cidx, clam, cold, kk, rows)
+        cpu = dict(value=n / dt, unit=UNIT, cores=cpu_threads(), kind="oracle",
+                   sample=f"{n} live tokens of this workload (full d, V), forward+backward incl. grad_W, numpy fp64, {dt:.1f} s")
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="bf16" if cfg["dtype"] == "bf16" else "f32(3xbf16)", data="synthetic",
+                config=dict(workload=f"{cfg['name']} {args.mode} C={idx.shape[1]} sigma={inp['sigma']}", T=T, d=d, V=V,
+                            live_tokens_per_gpu=n_live, l2_policy="inputs larger than L2 (W alone is %.0f MB)" % (d * V * 2 / 1e6),
+                            super_tile=[stats["super_rows"], stats["super_cols"]]),
+                pct_of_bf16_peak=dict(executed_8dV_vs_burst=100 * whole / pk["burst"], executed_8dV_vs_sustained=100 * whole / pk["sustained"],
+                                      model_6dV_vs_burst=100 * whole * 0.75 / pk["burst"], tflops_executed=whole, peaks=pk),
+                phase_ms=pm, loss=loss_val, clocks=clocks, e2e=e2e, gpu_launches=stats["kernels"] * args.steps,
+                roofline=roofline, cpu_baseline=cpu)
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -167,7 +167,9 @@ class Handle:
         loss = torch.empty(1, dtype=torch.float32, device=dev)
         ptk = torch.empty(T, dtype=torch.float32, device=dev)
         lse = torch.empty(T, dtype=torch.float32, device=dev) if want_lse else None
-        slp = torch.full(tuple(cache_idx.shape), float("nan"), dtype=torch.float32, device=dev) if want_student_logp else None
+        slp = None
+        if want_student_logp:       # student_logp_out shares the caches' row stride (include/opd.h)
+            slp = torch.full((T, cache_idx.stride(0)), float("nan"), dtype=torch.float32, device=dev)
         if not fwd_only:
             if grad_hidden is None:
                 grad_hidden = torch.empty_like(hidden)
@@ -181,6 +183,8 @@ class Handle:
             mode, k_or_K, flags, float(norm_override), _ptr(loss), _ptr(ptk), _ptr(lse), _ptr(slp),
             _ptr(grad_hidden), grad_hidden.stride(0) if grad_hidden is not None else 0, _ptr(grad_W), gk, gv)
         self._check(st)
+        if slp is not None:
+            slp = slp[:, :cache_idx.shape[1]]
         return dict(loss=loss, per_token_kl=ptk, grad_hidden=grad_hidden, grad_W=grad_W, lse=lse, student_logp=slp)
 
     def loss_fwd_bwd_host(self, hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K, flags=0,

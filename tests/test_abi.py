@@ -1,0 +1,77 @@
+"""CPU-side checks of the boundary: the C-ABI library builds, loads and exports every symbol that
+include/opd.h declares; host-side planning works without a GPU; compute entry points fail loudly
+(no CPU fallback)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_24143_b200 import build, opd
+    build.build()
+    return opd.load_library()
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "opd.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(opd_[a-z_]+)\s*\(", src)))
+
+
+def test_header_symbols_are_exported(lib):
+    from paper_2606_24143_b200 import opd
+    syms = declared_symbols()
+    assert "opd_loss_fwd_bwd" in syms and len(syms) >= 10
+    for s in syms:
+        assert hasattr(lib, s), f"{s} declared in include/opd.h but not exported by libopd.so"
+    assert sorted(opd.EXPORTS) == syms
+
+
+def test_enum_values_match_header():
+    from paper_2606_24143_b200 import opd
+    src = open(os.path.join(ROOT, "include", "opd.h")).read()
+    for name, val in [("OPD_FKL_TOPK", opd.FKL_TOPK), ("OPD_RKL_MC", opd.RKL_MC), ("OPD_MIXED", opd.MIXED), ("OPD_BF16", opd.BF16),
+                      ("OPD_FP32", opd.FP32), ("OPD_F_NO_RENORM_TEACHER", opd.F_NO_RENORM_TEACHER),
+                      ("OPD_F_RENORM_STUDENT", opd.F_RENORM_STUDENT), ("OPD_F_GRADW_ACCUM", opd.F_GRADW_ACCUM),
+                      ("OPD_F_VALIDATE_IDX", opd.F_VALIDATE_IDX), ("OPD_F_FWD_ONLY", opd.F_FWD_ONLY),
+                      ("OPD_F_SUR_CLIP", opd.F_SUR_CLIP), ("OPD_F_SUR_A_OLD", opd.F_SUR_A_OLD),
+                      ("OPD_ERR_BAD_INDEX", opd.ERR_BAD_INDEX), ("OPD_ERR_ARCH", opd.ERR_ARCH)]:
+        m = re.search(rf"\b{name}\s*=\s*(-?\d+)", src)
+        assert m and int(m.group(1)) == val, name
+
+
+def test_workspace_plan_has_no_logits_sized_buffer(lib):
+    """Host-only: opd_workspace_bytes at the BASELINE.json shapes stays far below T*V*2 bytes."""
+    from paper_2606_24143_b200 import synth
+    assert b"sm_100a" in lib.opd_version()
+    for c in (2, 3, 4, 5):
+        cfg = synth.CONFIGS[c]
+        ws = lib.opd_workspace_bytes(cfg["T"], cfg["d"], cfg["V"], max(cfg["k"], cfg["K"]), 0, 1, 0)
+        # the G super-tile is bounded (<= 32 MiB per plane), so the ratio shrinks with the problem; C2 is small
+        assert 0 < ws < (0.30 if c == 2 else 0.06) * cfg["T"] * cfg["V"] * 2
+        fwd = lib.opd_workspace_bytes(cfg["T"], cfg["d"], cfg["V"], max(cfg["k"], cfg["K"]), 0, 1, 32)
+        assert fwd < ws
+    assert lib.opd_workspace_bytes(0, 256, 4096, 4, 0, 0, 0) == 0
+
+
+def test_no_cpu_fallback():
+    """Without a GPU the product path raises; it never routes anywhere else."""
+    import torch
+    from paper_2606_24143_b200 import opd
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(Exception):
+        opd.Handle(0)
+    src = open(os.path.join(ROOT, "paper_2606_24143_b200", "opd.py")).read()
+    assert "oracle" not in src.replace("no CPU fallback", "")
+
+
+def test_null_handle_is_an_error(lib):
+    assert lib.opd_destroy(None) == -1
+    assert lib.opd_set_workspace(None, None, 0) == -1
+    assert lib.opd_last_error(None) == b"null handle"

@@ -1,0 +1,89 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
+
+The fp64 oracle cannot materialise T x V at these sizes, so (i) outputs the oracle can compute one by
+one — lse, per-token loss, student log-probs and whole grad_hidden rows of sampled tokens — are compared
+directly, and (ii) grad_W is checked through properties that hold at any size:
+   sum_v grad_W[k,v] = 0                       (softmax shift invariance, pin P10)
+   sum_v W[k,v] grad_W[k,v] = sum_t x[t,k] grad_hidden[t,k]   for every k   (both equal <z, G> split by k)
+plus (iii) a few-live-token variant of the 1.7B-class shape where the oracle computes grad_W in full."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import opd_oracle as O
+from paper_2606_24143_b200 import synth
+from tests._util import GRAD_TOL, LOGP_ATOL, LOSS_RTOL, check_grad, compare_all, f64, oracle_for, pick
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+@pytest.fixture(scope="module")
+def handle():
+    from paper_2606_24143_b200 import opd
+    return opd.Handle(0)
+
+
+def sampled_check(handle, cfg, c, mode, n_rows=12):
+    inp = synth.make_inputs(cfg, c=c, device=DEV)
+    idx, lam, old, kk = pick(inp, cfg, mode)
+    r = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, want_lse=True, want_student_logp=True)
+    torch.cuda.synchronize()
+    mask = f64(inp["mask"])
+    live = np.flatnonzero(mask)
+    rng = np.random.default_rng(c)
+    rows = np.sort(np.concatenate([live[:2], rng.choice(live, n_rows - 4, replace=False), live[-2:]]))
+    W = f64(inp["W"])
+    sel = torch.as_tensor(rows, device=DEV)
+    sub = dict(hidden=inp["hidden"][sel], W=inp["W"], mask=inp["mask"][sel])
+    # the oracle on the sampled rows only, with the normaliser of the whole call
+    ref = O.opd_oracle(f64(sub["hidden"]), W, f64(idx[sel]), f64(lam[sel]), f64(old[sel]) if old is not None else None,
+                       f64(sub["mask"]), mode, kk, norm_override=float(live.size), want_grad_W=False)
+    assert np.abs(f64(r["lse"][sel]) - ref["lse"]).max() <= LOGP_ATOL
+    a, b = f64(r["student_logp"][sel]), ref["student_logp"]
+    used = ~np.isnan(b)
+    assert np.abs(a[used] - b[used]).max() <= LOGP_ATOL
+    assert np.abs(f64(r["per_token_kl"][sel]) - ref["per_token_kl"]).max() <= LOSS_RTOL * np.abs(ref["per_token_kl"]).max()
+    gh = r["grad_hidden"]
+    check_grad(f64(gh[sel]), ref["grad_hidden"], "bf16", "grad_hidden rows")
+    assert abs(r["loss"].item() - r["per_token_kl"].double().sum().item() / live.size) <= 1e-5 * max(1.0, abs(r["loss"].item()))
+    if (mask == 0).any():
+        dead = torch.as_tensor(np.flatnonzero(mask == 0), device=DEV)
+        assert not gh[dead].any() and not r["per_token_kl"][dead].any()
+    # grad_W properties (fp64 reductions of the CUDA outputs, done with torch on the GPU: test infrastructure)
+    gw = r["grad_W"]
+    gmax = gw.abs().max().item()
+    colsum = gw.double().sum(dim=1)
+    V = gw.shape[1]
+    assert colsum.abs().max().item() <= 1e-2 * gmax * np.sqrt(V)        # bf16 rounding of G: random-walk bound
+    lhs = (inp["W"].double() * gw.double()).sum(dim=1)
+    rhs = (inp["hidden"].double() * gh.double()).sum(dim=0)
+    assert (lhs - rhs).abs().max().item() <= 2e-2 * max(lhs.abs().max().item(), 1e-30)
+    return r
+
+
+def test_C3_shape_sampled(handle):
+    r = sampled_check(handle, synth.CONFIGS[3], 3, O.RKL_MC)
+    r = sampled_check(handle, synth.CONFIGS[3], 3, O.FKL_TOPK)
+
+
+def test_C4_shape_sampled(handle):
+    sampled_check(handle, synth.CONFIGS[4], 4, O.RKL_MC)
+
+
+def test_C5_shape_sampled_mixed(handle):
+    sampled_check(handle, synth.CONFIGS[5], 5, O.MIXED)
+
+
+def test_C3_shape_few_live_tokens_full_oracle(handle):
+    """d=2048, V=151936 with 160 live tokens scattered over T=16384: every output against the full oracle."""
+    cfg = dict(synth.CONFIGS[3])
+    inp = synth.make_inputs(cfg, c=3, device=DEV)
+    m = torch.zeros_like(inp["mask"])
+    sel = torch.randperm(cfg["T"], generator=torch.Generator().manual_seed(5))[:160].to(DEV)
+    m[sel] = 1
+    inp["mask"] = m
+    idx, lam, old, kk = pick(inp, cfg, O.RKL_MC)
+    r = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, m, O.RKL_MC, kk, want_lse=True, want_student_logp=True)
+    torch.cuda.synchronize()
+    compare_all(r, oracle_for(inp, idx, lam, old, O.RKL_MC, kk, chunk=32), f64(m), "bf16")

@@ -1,0 +1,207 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the fp64 oracle, element by element,
+on the same seeded inputs.  Run with `-m gpu` on a B200."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import opd_oracle as O
+from paper_2606_24143_b200 import synth
+from tests._util import GRAD_TOL, LOGP_ATOL, check_grad, check_loss, compare_all, f64, oracle_for, pick
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+@pytest.fixture(scope="module")
+def opd():
+    from paper_2606_24143_b200 import opd as m
+    return m
+
+
+@pytest.fixture(scope="module")
+def handle(opd):
+    return opd.Handle(0)
+
+
+def run(handle, inp, idx, lam, old, mode, kk, flags=0, layout="dv", **kw):
+    W = inp["W"] if layout == "dv" else inp["W"].t().contiguous().t()     # same logical [d,V], [V,d] storage
+    r = handle.loss_fwd_bwd(inp["hidden"], W, idx, lam, old, inp["mask"], mode, kk, flags=flags, want_lse=True,
+                            want_student_logp=True, **kw)
+    torch.cuda.synchronize()
+    return r
+
+
+# ------------------------------------------------------------------------------------------------
+def test_gemm_core_all_operand_layouts(handle):
+    """The tcgen05 core against torch fp32 matmul for K-major / MN-major A and B, with ragged M, N, K."""
+    torch.manual_seed(1)
+    for (M, N, K) in [(128, 256, 64), (200, 304, 200), (1000, 1000, 520)]:
+        A = torch.randn(M, K, device=DEV).bfloat16()
+        B = torch.randn(N, K, device=DEV).bfloat16()
+        ref = A.double() @ B.double().t()
+        for amn in (False, True):
+            for bmn in (False, True):
+                D = handle.debug_gemm(A.t().contiguous() if amn else A, B.t().contiguous() if bmn else B, amn, bmn)
+                torch.cuda.synchronize()
+                assert (D.double() - ref).abs().max() <= 2e-5 * ref.abs().max()
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "fp32"])
+@pytest.mark.parametrize("layout", ["dv", "vd"])
+def test_gathers_are_bit_exact(handle, dtype, layout):
+    """north_star 'cache gathers bit-exact' (reading Q12): the gathered value is bit-identical to the
+    fp32 logit the same kernel held at (t, a_tj); duplicates in a row give identical values; unsorted caller order."""
+    torch.manual_seed(2)
+    T, d, V, C = 300, 256, 4104, 8
+    dt = torch.bfloat16 if dtype == "bf16" else torch.float32
+    X = torch.randn(T, d, device=DEV).to(dt)
+    W = (torch.randn(d, V, device=DEV) / 16).to(dt)
+    idx = torch.randint(0, V, (T, C), device=DEV, dtype=torch.int32)
+    idx[:, 5] = idx[:, 1]
+    idx[0] = torch.tensor([V - 1, 0, 255, 256, 257, 0, V - 8, 4095], dtype=torch.int32)
+    Wl = W if layout == "dv" else W.t().contiguous().t()
+    logits, gathered = handle.debug_logits(X, Wl, idx)
+    torch.cuda.synchronize()
+    assert torch.equal(gathered, torch.gather(logits, 1, idx.long()))
+    assert torch.equal(gathered[:, 5], gathered[:, 1])
+    z = f64(X) @ f64(W)
+    assert np.abs(f64(logits) - z).max() <= (2e-5 if dtype == "bf16" else 5e-5)
+
+
+@pytest.mark.parametrize("mode,flags,layout", [
+    (O.FKL_TOPK, 0, "dv"), (O.FKL_TOPK, 0, "vd"), (O.RKL_MC, 0, "dv"), (O.RKL_MC, 0, "vd"),
+    (O.FKL_TOPK, O.F_RENORM_STUDENT, "dv"), (O.FKL_TOPK, O.F_NO_RENORM_TEACHER, "dv"),
+    (O.FKL_TOPK, O.F_NO_RENORM_TEACHER | O.F_RENORM_STUDENT, "vd"),
+    (O.RKL_MC, 64, "dv"), (O.RKL_MC, 128, "dv"), (O.RKL_MC, 64 | 128, "dv")])
+def test_C1_fp32(handle, mode, flags, layout):
+    """BASELINE.json configs[0]: fp32, T=256, d=256, V=4096, k=8 / K=4, sigma=0.05, 10% masked."""
+    cfg = synth.CONFIGS[1]
+    inp = synth.make_inputs(cfg, c=1, device=DEV)
+    idx, lam, old, kk = pick(inp, cfg, mode)
+    r = run(handle, inp, idx, lam, old, mode, kk, flags, layout)
+    compare_all(r, oracle_for(inp, idx, lam, old, mode, kk, flags), f64(inp["mask"]), "fp32")
+
+
+@pytest.mark.parametrize("mode", [O.FKL_TOPK, O.RKL_MC])
+def test_C2_bf16(handle, mode):
+    """BASELINE.json configs[1]: bf16, T=4096, d=1024, V=32768, k=16 / K=4, sigma=0.02 (full oracle)."""
+    cfg = synth.CONFIGS[2]
+    inp = synth.make_inputs(cfg, c=2, device=DEV)
+    idx, lam, old, kk = pick(inp, cfg, mode)
+    r = run(handle, inp, idx, lam, old, mode, kk)
+    compare_all(r, oracle_for(inp, idx, lam, old, mode, kk), f64(inp["mask"]), "bf16")
+
+
+RAGGED = dict(dtype="bf16", T=700, d=320, V=2056, k=8, K=5, sigma=0.05, mask="random10")
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "fp32"])
+@pytest.mark.parametrize("mode", [O.FKL_TOPK, O.RKL_MC, O.MIXED])
+@pytest.mark.parametrize("tiles", [None, (256, 512)])
+def test_ragged_shapes_and_super_tiles(handle, dtype, mode, tiles, monkeypatch):
+    """T, V not multiples of the tile sizes, d not a multiple of 256; several backward super-tiles in both
+    directions (OPD_TB / OPD_VB shrink them) must give the same result as one."""
+    if tiles:
+        monkeypatch.setenv("OPD_TB", str(tiles[0]))
+        monkeypatch.setenv("OPD_VB", str(tiles[1]))
+    cfg = dict(RAGGED, dtype=dtype)
+    inp = synth.make_inputs(cfg, c=7, device=DEV)
+    if mode == O.MIXED:
+        m = inp["mask"].clone()
+        m[(torch.arange(cfg["T"], device=DEV) % 3 == 0) & (m != 0)] = 2
+        inp["mask"] = m
+    idx, lam, old, kk = pick(inp, cfg, mode)
+    r = run(handle, inp, idx, lam, old, mode, kk)
+    compare_all(r, oracle_for(inp, idx, lam, old, mode, kk), f64(inp["mask"]), dtype)
+    if tiles:
+        assert handle.launch_stats()["super_rows"] == tiles[0]
+
+
+def test_degenerate_cases(handle, opd):
+    cfg = dict(RAGGED, T=130, k=64, K=64)
+    inp = synth.make_inputs(cfg, c=8, device=DEV)
+    idx, lam, old, kk = pick(inp, cfg, O.RKL_MC)
+    # C = 64 with many duplicates (iid with replacement)
+    r = run(handle, inp, idx, lam, old, O.RKL_MC, kk)
+    compare_all(r, oracle_for(inp, idx, lam, old, O.RKL_MC, kk), f64(inp["mask"]), "bf16")
+    # all K entries the same action == the K=1 result (pin P13 on the GPU)
+    i1, l1, o1 = idx[:, :1].contiguous(), lam[:, :1].contiguous(), old[:, :1].contiguous()
+    a = run(handle, inp, i1, l1, o1, O.RKL_MC, 1)
+    b = run(handle, inp, i1.repeat(1, 7).contiguous(), l1.repeat(1, 7).contiguous(), o1.repeat(1, 7).contiguous(), O.RKL_MC, 7)
+    assert torch.allclose(a["per_token_kl"], b["per_token_kl"], rtol=1e-5, atol=1e-6)
+    # everything masked: N = 0 -> loss 0, all gradients exactly 0
+    z = dict(inp, mask=torch.zeros_like(inp["mask"]))
+    r = run(handle, z, idx, lam, old, O.RKL_MC, kk)
+    assert r["loss"].item() == 0 and not r["grad_hidden"].any() and not r["grad_W"].any() and not r["per_token_kl"].any()
+    # a single live token, and T = 1
+    one = torch.zeros_like(inp["mask"]); one[77] = 1
+    s = dict(inp, mask=one)
+    r = run(handle, s, idx, lam, old, O.RKL_MC, kk)
+    compare_all(r, oracle_for(s, idx, lam, old, O.RKL_MC, kk), f64(one), "bf16")
+    t1 = dict(hidden=inp["hidden"][:1].contiguous(), W=inp["W"], mask=inp["mask"][:1] * 0 + 1)
+    r = run(handle, t1, idx[:1].contiguous(), lam[:1].contiguous(), old[:1].contiguous(), O.RKL_MC, kk)
+    compare_all(r, oracle_for(t1, idx[:1], lam[:1], old[:1], O.RKL_MC, kk), np.ones(1), "bf16")
+
+
+def test_options_strides_and_errors(handle, opd):
+    cfg = RAGGED
+    inp = synth.make_inputs(cfg, c=9, device=DEV)
+    idx, lam, old, kk = pick(inp, cfg, O.RKL_MC)
+    ref = oracle_for(inp, idx, lam, old, O.RKL_MC, kk)
+    T, d, V = cfg["T"], cfg["d"], cfg["V"]
+    # padded row strides of hidden / caches / grads
+    hp = torch.zeros(T, d + 64, device=DEV, dtype=torch.bfloat16); hp[:, :d] = inp["hidden"]
+    ip = torch.full((T, kk + 3), -5, device=DEV, dtype=torch.int32); ip[:, :kk] = idx
+    lp = torch.zeros(T, kk + 3, device=DEV); lp[:, :kk] = lam
+    op = torch.zeros(T, kk + 3, device=DEV); op[:, :kk] = old
+    ghp = torch.full((T, d + 64), 7.0, device=DEV, dtype=torch.bfloat16)
+    gwp = torch.full((d, V + 8), 7.0, device=DEV)
+    r = handle.loss_fwd_bwd(hp[:, :d], inp["W"], ip[:, :kk], lp[:, :kk], op[:, :kk], inp["mask"], O.RKL_MC, kk,
+                            grad_hidden=ghp[:, :d], grad_W=gwp[:, :V])
+    torch.cuda.synchronize()
+    check_loss(r["loss"].item(), ref)
+    check_grad(f64(ghp[:, :d]), ref["grad_hidden"], "bf16")
+    check_grad(f64(gwp[:, :V]), ref["grad_W"], "bf16")
+    assert (ghp[:, d:] == 7).all() and (gwp[:, V:] == 7).all()            # padding untouched
+    # norm_override and GRADW_ACCUM (two micro-batches accumulate)
+    gw = torch.zeros(d, V, device=DEV)
+    for _ in range(2):
+        r2 = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], O.RKL_MC, kk, flags=opd.F_GRADW_ACCUM,
+                                 norm_override=2.0 * ref["N"], grad_W=gw)
+    torch.cuda.synchronize()
+    assert abs(r2["loss"].item() - ref["loss"] / 2) <= 2e-3 * abs(ref["loss"])
+    check_grad(f64(gw), ref["grad_W"], "bf16")
+    # forward only
+    r3 = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], O.RKL_MC, kk, flags=opd.F_FWD_ONLY)
+    assert r3["grad_W"] is None and abs(r3["loss"].item() - r["loss"].item()) < 1e-6
+    # index validation
+    bad = idx.clone(); bad[5, 0] = V
+    live5 = inp["mask"][5].item() != 0
+    if live5:
+        with pytest.raises(opd.OpdError) as e:
+            handle.loss_fwd_bwd(inp["hidden"], inp["W"], bad, lam, old, inp["mask"], O.RKL_MC, kk, flags=opd.F_VALIDATE_IDX)
+        assert e.value.status == opd.ERR_BAD_INDEX
+    # argument errors are reported, not crashed on
+    for kwargs, code in [(dict(k_or_K=0), opd.ERR_BAD_SHAPE), (dict(k_or_K=65), opd.ERR_BAD_SHAPE), (dict(flags=1 << 20), opd.ERR_BAD_ARG)]:
+        with pytest.raises(opd.OpdError) as e:
+            handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], O.RKL_MC,
+                                kwargs.get("k_or_K", kk), flags=kwargs.get("flags", 0))
+        assert e.value.status == code
+    with pytest.raises(opd.OpdError):
+        handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, None, inp["mask"], O.RKL_MC, kk)
+    # the host-buffer entry point gives the same numbers
+    hr = handle.loss_fwd_bwd_host(inp["hidden"].cpu(), inp["W"].cpu(), idx.cpu(), lam.cpu(), old.cpu(), inp["mask"].cpu(), O.RKL_MC, kk)
+    assert abs(hr["loss"].item() - r["loss"].item()) < 1e-6
+    check_grad(f64(hr["grad_W"]), ref["grad_W"], "bf16")
+    assert hr["h2d_bytes"] > 0 and hr["d2h_bytes"] > 0
+
+
+def test_no_logits_sized_workspace(handle, opd):
+    """'full logits never touch HBM' (i): no T x V sized buffer exists."""
+    for c in (3, 4, 5):
+        cfg = synth.CONFIGS[c]
+        C = max(cfg["k"], cfg["K"])
+        ws = handle.workspace_bytes(cfg["T"], cfg["d"], cfg["V"], C, opd.BF16, opd.RKL_MC, 0)
+        assert ws < 0.06 * cfg["T"] * cfg["V"] * 2, (c, ws)
