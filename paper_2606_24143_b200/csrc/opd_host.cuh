@@ -86,7 +86,9 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags) {
     p.T = T; p.d = d; p.V = V; p.C = C; p.planes = fp32 ? 3 : 1;
     p.t_pad = ceil_div(T, BM) * BM;
     p.num_n = ceil_div(V, BN);
-    const int tb = env_int("OPD_TB", 4096), vb = env_int("OPD_VB", 4096);
+    // Super-tile of the backward: 37 row tiles x 16 column tiles = 592 = 4 x 148 tiles per launch on a 148-SM B200
+    // (whole waves for the G and grad_hidden GEMMs); 4736 x 4096 bf16 = 37 MiB stays resident in the 126 MB L2.
+    const int tb = env_int("OPD_TB", 37 * BM), vb = env_int("OPD_VB", 4096);
     p.Tb = std::min(p.t_pad, std::max(BM, tb / BM * BM));
     p.Vb = std::min(p.num_n * BN, std::max(BN, vb / BN * BN));
     p.est_blocks = ceil_div(T, 128);
