@@ -94,103 +94,122 @@ struct GEpi {
     }
 };
 
+// ------------------------------------------------------------------------------------------ fp32 accumulate via TMA
+// One warp stages its 32 rows x 32 fp32 columns (128-byte rows, SWIZZLE_128B) into one of its two 4 KiB smem
+// buffers and one lane issues a TMA store or reduce-add: the read-modify-write of the fp32 accumulators happens in
+// L2, the epilogue never waits on a load.  `wbuf` is this warp's 8 KiB (1024-byte aligned) region.
+__device__ __forceinline__ void stage_and_send(const CUtensorMap* tm, uint8_t* wbuf, int parity, const float (&v)[32],
+                                               int lane, int col, int row, bool reduce) {
+    uint8_t* buf = wbuf + parity * 4096;
+    if (lane == 0) bulk_wait_read<1>();          // the group that last used this buffer has finished reading it
+    __syncwarp();
+    uint8_t* rowp = buf + lane * 128;
+#pragma unroll
+    for (int q = 0; q < 8; ++q)
+        *reinterpret_cast<float4*>(rowp + ((q ^ (lane & 7)) << 4)) = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+    fence_proxy_async_smem();
+    __syncwarp();
+    if (lane == 0) {
+        if (reduce) tma_reduce_add_2d(tm, buf, col, row); else tma_store_2d(tm, buf, col, row);
+        bulk_commit();
+    }
+}
+// all bulk stores / reductions issued by this warp are complete (globally performed)
+__device__ __forceinline__ void drain_sends(int lane) {
+    if (lane == 0) bulk_wait<0>();
+    __syncwarp();
+}
+
 // ------------------------------------------------------------------------------------------ DxEpi
 // S7: grad_hidden super-tile [Tb][d] = sum over vocabulary super-tiles of  G . W^T.  Partial sums live in an
-// fp32 workspace between super-tiles; the last one emits rows into grad_hidden (dtype of hidden) at the
-// token positions of the compacted rows.
+// fp32 workspace between super-tiles (TMA store for the first, TMA reduce-add after); the last one adds the
+// workspace to its accumulator and emits rows into grad_hidden (dtype of hidden) at the token positions.
 struct DxEpi {
     struct Params {
-        float* acc;              // [Tb_pad][ld_acc] fp32
+        CUtensorMap m_acc;       // fp32 [Tb_pad][d], boxes of 32 x 32
+        float* acc;              // same buffer, for the last super-tile's read
         long ld_acc;
         void* out;               // grad_hidden
         long ld_out;
         int out_fp32;
         const int* live_rows;    // compact row -> token index
-        int first, last;         // first / last vocabulary super-tile of this token super-tile
     };
     struct State { int tok; };
     static __device__ __forceinline__ State prepare(const Params& p, const GemmParams& gp, int m_blk, int,
                                                     int row_in_tile, int M_eff) {
         State st{-1};
         const int lrow = m_blk * BM + row_in_tile;
-        if (p.last && lrow < M_eff) st.tok = p.live_rows[gp.tok_off + lrow];
+        if (gp.last && lrow < M_eff) st.tok = p.live_rows[gp.tok_off + lrow];
         return st;
     }
     static __device__ __forceinline__ void run(const Params& p, const GemmParams& gp, State st, uint32_t taddr,
-                                               int m_blk, int n_blk, int row_in_tile, int M_eff, uint8_t*, int) {
+                                               int m_blk, int n_blk, int row_in_tile, int M_eff, uint8_t* epi_smem, int epi_tid) {
         const int lrow = m_blk * BM + row_in_tile;
         const bool live = lrow < M_eff;
-        float* acc = p.acc + static_cast<size_t>(lrow) * p.ld_acc + n_blk * BN;
+        const int lane = epi_tid & 31;
+        uint8_t* wbuf = epi_smem + (epi_tid >> 5) * 8192;
+        const float* acc = p.acc + static_cast<size_t>(lrow) * p.ld_acc + n_blk * BN;
 #pragma unroll 1
         for (int c = 0; c < BN / 32; ++c) {
             float v[32];
             tmem_ld32(taddr + c * 32, v);
             tmem_ld_wait();
             const int col0 = n_blk * BN + c * 32;
-            if (live && col0 < gp.N) {                                // d % 64 == 0: chunks are all-in or all-out
-            float4* a4 = reinterpret_cast<float4*>(acc + c * 32);
-            if (!p.first) {
+            if (col0 >= gp.N) break;                                  // d % 64 == 0: chunks are all-in or all-out (warp-uniform)
+            if (!gp.last) {
+                stage_and_send(&p.m_acc, wbuf, c & 1, v, lane, col0, lrow - lane, !gp.first);
+            } else if (live) {
+                if (!gp.first) {
+                    const float4* a4 = reinterpret_cast<const float4*>(acc + c * 32);
 #pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    const float4 o = a4[q];
-                    v[4 * q] += o.x; v[4 * q + 1] += o.y; v[4 * q + 2] += o.z; v[4 * q + 3] += o.w;
+                    for (int q = 0; q < 8; ++q) {
+                        const float4 o = __ldcg(a4 + q);              // written through L2 by other SMs: bypass L1
+                        v[4 * q] += o.x; v[4 * q + 1] += o.y; v[4 * q + 2] += o.z; v[4 * q + 3] += o.w;
+                    }
+                }
+                if (p.out_fp32) {
+                    float4* o4 = reinterpret_cast<float4*>(static_cast<float*>(p.out) + static_cast<size_t>(st.tok) * p.ld_out + col0);
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) o4[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+                } else {
+                    uint4* o4 = reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(p.out) + static_cast<size_t>(st.tok) * p.ld_out + col0);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        o4[q] = make_uint4(pack_bf16x2(v[8 * q], v[8 * q + 1]), pack_bf16x2(v[8 * q + 2], v[8 * q + 3]),
+                                           pack_bf16x2(v[8 * q + 4], v[8 * q + 5]), pack_bf16x2(v[8 * q + 6], v[8 * q + 7]));
                 }
             }
-            if (!p.last) {
-#pragma unroll
-                for (int q = 0; q < 8; ++q) a4[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
-            } else if (p.out_fp32) {
-                float4* o4 = reinterpret_cast<float4*>(static_cast<float*>(p.out) + static_cast<size_t>(st.tok) * p.ld_out + col0);
-#pragma unroll
-                for (int q = 0; q < 8; ++q) o4[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
-            } else {
-                uint4* o4 = reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(p.out) + static_cast<size_t>(st.tok) * p.ld_out + col0);
-#pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    o4[q] = make_uint4(pack_bf16x2(v[8 * q], v[8 * q + 1]), pack_bf16x2(v[8 * q + 2], v[8 * q + 3]),
-                                       pack_bf16x2(v[8 * q + 4], v[8 * q + 5]), pack_bf16x2(v[8 * q + 6], v[8 * q + 7]));
-            }
-            }
         }
+        if (!gp.last) drain_sends(lane);
     }
 };
 
 // ------------------------------------------------------------------------------------------ DwEpi
-// S8: grad_W tile += accumulator.  Output element (row, col) of this GEMM lives at gw[row*ld + col] with
-// row = row_off + tile row, col = col_off + tile col (the host maps (d,V) or (V,d) onto rows/cols).
+// S8: grad_W tile += accumulator (TMA reduce-add; grad_W was zeroed or holds the caller's running sum).  Output element
+// (row, col) of this GEMM lives at row = row_off + tile row, col = col_off + tile col of the fp32 tensor the map
+// describes ((d,V) or (V,d)); TMA clips rows / columns outside the tensor.
 struct DwEpi {
     struct Params {
-        float* gw;
-        long ld;
-        int row_off, col_off;
-        int rows_total, cols_total;
+        CUtensorMap m_gw;        // fp32 [rows_total][cols_total] (row stride ld), boxes of 32 x 32
     };
     using State = NoState;
     static __device__ __forceinline__ State prepare(const Params&, const GemmParams&, int, int, int, int) { return {}; }
     static __device__ __forceinline__ void run(const Params& p, const GemmParams& gp, const State&, uint32_t taddr,
-                                               int m_blk, int n_blk, int row_in_tile, int M_eff, uint8_t*, int) {
-        const int row = p.row_off + m_blk * BM + row_in_tile;
-        const bool ok = (m_blk * BM + row_in_tile) < M_eff && row < p.rows_total;
-        float* g = p.gw + static_cast<size_t>(row) * p.ld + p.col_off + n_blk * BN;
+                                               int m_blk, int n_blk, int row_in_tile, int M_eff, uint8_t* epi_smem, int epi_tid) {
+        const int lane = epi_tid & 31;
+        uint8_t* wbuf = epi_smem + (epi_tid >> 5) * 8192;
+        const int lrow0 = m_blk * BM + row_in_tile - lane;           // first tile row of this warp
+        const bool warp_ok = lrow0 < M_eff;                          // extents are multiples of 32 except at tensor edges (clipped)
 #pragma unroll 1
         for (int c = 0; c < BN / 32; ++c) {
             float v[32];
             tmem_ld32(taddr + c * 32, v);
             tmem_ld_wait();
             const int lc0 = n_blk * BN + c * 32;
-            const int col0 = p.col_off + lc0;
-            if (ok && lc0 < gp.N) {
-            float4* g4 = reinterpret_cast<float4*>(g + c * 32);
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                if (col0 + 4 * q < p.cols_total && lc0 + 4 * q < gp.N) {          // extents are multiples of 4
-                    float4 o = g4[q];
-                    o.x += v[4 * q]; o.y += v[4 * q + 1]; o.z += v[4 * q + 2]; o.w += v[4 * q + 3];
-                    g4[q] = o;
-                }
-            }
-            }
+            if (lc0 >= gp.N) break;
+            if (warp_ok) stage_and_send(&p.m_gw, wbuf, c & 1, v, lane, gp.col_off + lc0, gp.row_off + lrow0, true);
         }
+        drain_sends(lane);
     }
 };
 

@@ -21,7 +21,7 @@ constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
 constexpr int MN_BOX = 64;                            // MN-major operands arrive as 64(mn) x 64(k) boxes
 constexpr int MN_BOX_BYTES = MN_BOX * BK * 2;         // 8 KiB
 constexpr int GEMM_THREADS = 192;                     // warp0 TMA, warp1 MMA(+TMEM alloc), warps2-5 epilogue
-constexpr int EPI_SMEM_BYTES = 8192;
+constexpr int EPI_SMEM_BYTES = 32768;                 // 4 epilogue warps x 2 staging buffers x (32 rows x 128 B)
 constexpr int GEMM_SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*barriers*/ + EPI_SMEM_BYTES + 1024 /*align slack*/;
 constexpr int TMEM_COLS = 512;                        // 2 accumulator stages x 256 columns
 
@@ -40,6 +40,9 @@ struct GemmParams {
     int tok_dim;              // which extent counts live tokens (clipped to n_live - tok_off on the device)
     int tok_off;
     const int* n_live;        // device scalar: number of live tokens (compacted rows)
+    // per-launch / per-tile epilogue switches (set by the host for gemm_kernel, per tile by bwd_kernel)
+    int first, last;          // DxEpi: first / last vocabulary super-tile of this token super-tile
+    int row_off, col_off;     // DwEpi: position of this GEMM's output inside grad_W
 };
 
 __device__ __forceinline__ void tile_coords(int tile, int num_m, int num_n, int group_m, int& m_blk, int& n_blk) {
@@ -57,7 +60,7 @@ __device__ __forceinline__ void tile_coords(int tile, int num_m, int num_n, int 
 template <class Epi>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-            const GemmParams gp, const typename Epi::Params ep) {
+            const GemmParams gp, const __grid_constant__ typename Epi::Params ep) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + STAGES * STAGE_BYTES);

@@ -8,7 +8,7 @@
 #include <string>
 
 #include "../../include/opd.h"
-#include "opd_epilogues_bwd.cuh"
+#include "opd_bwd_kernel.cuh"
 #include "opd_estimators.cuh"
 
 struct opd_handle_s {
@@ -61,6 +61,20 @@ inline bool make_map(CUtensorMap* m, const void* base, uint64_t inner, uint64_t 
     return r == CUDA_SUCCESS;
 }
 
+// fp32 matrix [rows][cols] (row stride in bytes), 128-byte swizzled boxes of 32 x 32 (epilogue store / reduce-add)
+inline bool make_map_f32(CUtensorMap* m, const void* base, uint64_t cols, uint64_t rows, uint64_t row_stride_bytes) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return false;
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {row_stride_bytes};
+    cuuint32_t box[2] = {32, 32};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(base), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
@@ -72,7 +86,9 @@ struct Plan {
     int Tb, Vb;           // backward super-tile (rows of tokens x vocabulary columns), multiples of 128 / 256
     int est_blocks;
     size_t off_nlive, off_badidx, off_live_rows, off_xc, off_wsplit, off_sorted, off_perm, off_zc, off_beta,
-           off_partials, off_lse2, off_coef, off_gs, off_dxacc, off_block_sums, total;
+           off_partials, off_lse2, off_coef, off_gs, off_dxacc, off_block_sums, off_counters, total;
+    int n_super;          // number of backward super-tiles (upper bound)
+    int gs_bufs;          // ring depth of the G super-tile buffer
     size_t xc_plane, w_plane, gs_plane;   // elements per plane
 };
 
@@ -110,7 +126,10 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags) {
     p.off_coef = take(sizeof(float) * (size_t)p.t_pad);
     const bool bwd = !(flags & OPD_F_FWD_ONLY);
     p.gs_plane = (size_t)p.Tb * p.Vb;
-    p.off_gs = take(bwd ? 2 * p.gs_plane * p.planes : 0);
+    p.gs_bufs = 2;
+    p.off_gs = take(bwd ? 2 * p.gs_plane * p.planes * p.gs_bufs : 0);
+    p.n_super = ceil_div(p.t_pad, p.Tb) * ceil_div(V, p.Vb);
+    p.off_counters = take(bwd ? sizeof(int) * 2 * (size_t)p.n_super : 0);
     p.off_dxacc = take(bwd ? sizeof(float) * (size_t)p.Tb * d : 0);
     p.off_block_sums = take(sizeof(double) * (size_t)p.est_blocks);
     p.total = o;

@@ -128,8 +128,16 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         ok &= make_map(&m_w_dx, wq, d, V, np, (uint64_t)ldwq * 2, wplane_b, MN_BOX);
     }
     if (!fwd_only) {
-        ok &= make_map(&m_gs_k, gs, p.Vb, p.Tb, np, (uint64_t)p.Vb * 2, p.gs_plane * 2, BM);
-        ok &= make_map(&m_gs_mn, gs, p.Vb, p.Tb, np, (uint64_t)p.Vb * 2, p.gs_plane * 2, MN_BOX);
+        ok &= make_map(&m_gs_k, gs, p.Vb, p.Tb, np * p.gs_bufs, (uint64_t)p.Vb * 2, p.gs_plane * 2, BM);
+        ok &= make_map(&m_gs_mn, gs, p.Vb, p.Tb, np * p.gs_bufs, (uint64_t)p.Vb * 2, p.gs_plane * 2, MN_BOX);
+    }
+    DxEpi::Params dxp{};
+    DwEpi::Params dwp{};
+    if (!fwd_only) {
+        ok &= make_map_f32(&dxp.m_acc, dxacc, d, p.Tb, (uint64_t)d * 4);
+        ok &= make_map_f32(&dwp.m_gw, a.grad_W, wl == 0 ? V : d, wl == 0 ? d : V, (uint64_t)ldgw * 4);
+        dxp.acc = dxacc; dxp.ld_acc = d; dxp.out = a.grad_hidden; dxp.ld_out = a.ld_gh; dxp.out_fp32 = fp32 ? 1 : 0;
+        dxp.live_rows = live_rows;
     }
     if (!ok) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled failed");
 
@@ -173,7 +181,27 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
 
     // ------------------------------------------------------------------ S6-S8 backward, super-tile by super-tile
     phase_mark(h, st, OPD_PHASE_BWD, 0);
-    if (!fwd_only) {
+    if (!fwd_only && !env_int("OPD_BWD_LEGACY", 0)) {
+        // one persistent kernel walks every super-tile: G re-formation, grad_hidden and grad_W tiles interleaved,
+        // ordered by dependency counters in global memory (opd_bwd_kernel.cuh)
+        int* counters = reinterpret_cast<int*>(ws + p.off_counters);
+        OPD_CUDA(h, cudaMemsetAsync(counters, 0, sizeof(int) * 2 * (size_t)p.n_super, st));
+        BwdParams bp{};
+        bp.d = d; bp.V = V; bp.Tb = p.Tb; bp.Vb = p.Vb; bp.nvb = ceil_div(V, p.Vb); bp.wl = wl; bp.planes = p.planes;
+        bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super;
+        bp.g = GEpi::Params{gs, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V};
+        bp.dx = dxp;
+        bp.dw = dwp;
+        static bool attr_set = false;
+        if (!attr_set) {
+            OPD_CUDA(h, cudaFuncSetAttribute(bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BYTES));
+            attr_set = true;
+        }
+        bwd_kernel<<<h->num_sms, GEMM_THREADS, GEMM_SMEM_BYTES, st>>>(m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, bp);
+        h->n_kernels++; h->n_gemm++;
+        OPD_CUDA(h, cudaGetLastError());
+    }
+    if (!fwd_only && env_int("OPD_BWD_LEGACY", 0)) {   // one launch per GEMM and super-tile (kept for A/B timing)
         const int nvb = ceil_div(V, p.Vb);
         for (int tb0 = 0; tb0 < T; tb0 += p.Tb) {
             const int Tb = std::min(p.Tb, p.t_pad - tb0);
@@ -195,26 +223,24 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
                     gp.a_mn = 0; gp.b_mn = (wl == 1); gp.a_off = 0; gp.b_off = 0; gp.ka_off = 0; gp.kb_off = vb0;
                     set_segments(gp, p.planes);
                     gp.tok_dim = TOK_M; gp.tok_off = tb0; gp.n_live = n_live;
-                    DxEpi::Params ep{dxacc, (long)d, a.grad_hidden, a.ld_gh, fp32 ? 1 : 0, live_rows, vi == 0, vi == nvb - 1};
-                    OPD_CUDA(h, launch_gemm<DxEpi>(h, st, m_gs_k, m_w_dx, gp, ep));
+                    gp.first = (vi == 0); gp.last = (vi == nvb - 1);
+                    OPD_CUDA(h, launch_gemm<DxEpi>(h, st, m_gs_k, m_w_dx, gp, dxp));
                 }
                 {   // S8: grad_W[:, vb] += hidden[tb]^T . G
                     GemmParams gp{};
                     gp.group_m = 1 << 20; gp.tok_dim = TOK_K; gp.tok_off = tb0; gp.n_live = n_live; gp.K = Tb;
                     gp.a_mn = 1; gp.b_mn = 1;
                     set_segments(gp, p.planes);
-                    DwEpi::Params ep{};
-                    ep.gw = static_cast<float*>(a.grad_W); ep.ld = ldgw;
                     if (wl == 0) {   // rows = d (A = Xc^T), cols = v (B = G)
                         gp.M = d; gp.N = Vb; gp.num_n = ceil_div(Vb, BN);
                         gp.a_off = 0; gp.ka_off = tb0; gp.b_off = 0; gp.kb_off = 0;
-                        ep.row_off = 0; ep.col_off = vb0; ep.rows_total = d; ep.cols_total = V;
-                        OPD_CUDA(h, launch_gemm<DwEpi>(h, st, m_xc_mn, m_gs_mn, gp, ep));
+                        gp.row_off = 0; gp.col_off = vb0;
+                        OPD_CUDA(h, launch_gemm<DwEpi>(h, st, m_xc_mn, m_gs_mn, gp, dwp));
                     } else {         // rows = v (A = G^T), cols = d (B = Xc)
                         gp.M = Vb; gp.N = d; gp.num_n = ceil_div(d, BN);
                         gp.a_off = 0; gp.ka_off = 0; gp.b_off = 0; gp.kb_off = tb0;
-                        ep.row_off = vb0; ep.col_off = 0; ep.rows_total = V; ep.cols_total = d;
-                        OPD_CUDA(h, launch_gemm<DwEpi>(h, st, m_gs_mn, m_xc_mn, gp, ep));
+                        gp.row_off = vb0; gp.col_off = 0;
+                        OPD_CUDA(h, launch_gemm<DwEpi>(h, st, m_gs_mn, m_xc_mn, gp, dwp));
                     }
                 }
             }
