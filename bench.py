@@ -219,6 +219,7 @@ def main():
             pass
     barrier()
     total_ms = ev[0].elapsed_time(ev[-1])
+    step_ms = [round(ev[i].elapsed_time(ev[i + 1]), 3) for i in range(args.steps)]
     pm = h.phase_times_ms()                      # phases of the last timed step
     h.enable_phase_timing(False)
     clocks = sampler.stop() if sampler else None
@@ -301,7 +302,7 @@ def main():
                             super_tile=[stats["super_rows"], stats["super_cols"]]),
                 pct_of_bf16_peak=dict(executed_8dV_vs_burst=100 * whole / pk["burst"], executed_8dV_vs_sustained=100 * whole / pk["sustained"],
                                       model_6dV_vs_burst=100 * whole * 0.75 / pk["burst"], tflops_executed=whole, peaks=pk),
-                phase_ms=pm, loss=loss_val, clocks=clocks, e2e=e2e, gpu_launches=stats["kernels"] * args.steps,
+                phase_ms=pm, step_ms=step_ms, loss=loss_val, clocks=clocks, e2e=e2e, gpu_launches=stats["kernels"] * args.steps,
                 roofline=roofline, cpu_baseline=cpu)
     print(json.dumps(line), flush=True)
     if dist is not None:

@@ -121,16 +121,22 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags) {
     p.off_perm = take((size_t)p.t_pad * C);
     p.off_zc = take(sizeof(float) * (size_t)p.t_pad * C);
     p.off_beta = take(sizeof(float) * (size_t)p.t_pad * C);
-    p.off_partials = take(sizeof(float2) * (size_t)p.num_n * p.t_pad);
     p.off_lse2 = take(sizeof(float) * (size_t)p.t_pad);
     p.off_coef = take(sizeof(float) * (size_t)p.t_pad);
     const bool bwd = !(flags & OPD_F_FWD_ONLY);
     p.gs_plane = (size_t)p.Tb * p.Vb;
     p.gs_bufs = 2;
-    p.off_gs = take(bwd ? 2 * p.gs_plane * p.planes * p.gs_bufs : 0);
     p.n_super = ceil_div(p.t_pad, p.Tb) * ceil_div(V, p.Vb);
     p.off_counters = take(bwd ? sizeof(int) * 2 * (size_t)p.n_super : 0);
-    p.off_dxacc = take(bwd ? sizeof(float) * (size_t)p.Tb * d : 0);
+    // The per-tile LSE partials are dead once the estimators have run, the G ring and the grad_hidden partial
+    // sums only live in the backward: they share one region.
+    const size_t partial_bytes = align_up(sizeof(float2) * (size_t)p.num_n * p.t_pad, 1024);
+    const size_t gs_bytes = bwd ? align_up(2 * p.gs_plane * p.planes * p.gs_bufs, 1024) : 0;
+    const size_t dx_bytes = bwd ? align_up(sizeof(float) * (size_t)p.Tb * d, 1024) : 0;
+    const size_t region = take(std::max(partial_bytes, gs_bytes + dx_bytes));
+    p.off_partials = region;
+    p.off_gs = region;
+    p.off_dxacc = region + gs_bytes;
     p.off_block_sums = take(sizeof(double) * (size_t)p.est_blocks);
     p.total = o;
     return p;

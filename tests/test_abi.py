@@ -53,9 +53,9 @@ def test_workspace_plan_has_no_logits_sized_buffer(lib):
         cfg = synth.CONFIGS[c]
         ws = lib.opd_workspace_bytes(cfg["T"], cfg["d"], cfg["V"], max(cfg["k"], cfg["K"]), 0, 1, 0)
         # the G super-tile is bounded (<= 32 MiB per plane), so the ratio shrinks with the problem; C2 is small
-        assert 0 < ws < (0.30 if c == 2 else 0.06) * cfg["T"] * cfg["V"] * 2
+        assert 0 < ws < (0.40 if c == 2 else 0.05) * cfg["T"] * cfg["V"] * 2
         fwd = lib.opd_workspace_bytes(cfg["T"], cfg["d"], cfg["V"], max(cfg["k"], cfg["K"]), 0, 1, 32)
-        assert fwd < ws
+        assert fwd <= ws
     assert lib.opd_workspace_bytes(0, 256, 4096, 4, 0, 0, 0) == 0
 
 
