@@ -16,7 +16,8 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
 // Rows past the live count and columns past V are written as zeros: both contractions rely on it.
 struct GEpi {
     struct Params {
-        __nv_bfloat16* gs;       // [planes][Tb_pad][ldg]
+        __nv_bfloat16* gs;       // [planes][rows][ldg]
+        int rows;                // allocated rows per plane (tile rows past it are not stored)
         long ldg;
         long plane_stride;       // elements
         int planes;              // 1 (bf16 path) or 3 (fp32 path: three-term bf16 split of G)
@@ -75,6 +76,7 @@ struct GEpi {
                 for (int i = 0; i < 32; ++i)
                     if (col0 + i >= p.V) v[i] = 0.f;
             }
+            if (lrow >= p.rows) continue;                             // row of a pair tile past the buffer
             for (int pl = 0; pl < p.planes; ++pl) {
                 uint32_t w[16];
 #pragma unroll

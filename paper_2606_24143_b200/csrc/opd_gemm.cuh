@@ -1,29 +1,43 @@
 // Generic persistent warp-specialised GEMM core for sm_100a:  D[M,N] = sum_seg A_seg[M,K] * B_seg[N,K]^T
-//   TMA (SWIZZLE_128B) -> 4-stage smem ring -> tcgen05.mma (cta_group::1, 128x256x16, bf16 -> fp32)
-//   -> double-buffered TMEM accumulators -> per-tile epilogue functor run by 4 epilogue warps.
-// A and B may each be K-major (K contiguous in global memory) or MN-major (M/N contiguous); the
-// majorness is a run-time parameter that only changes the TMA box sequence and the UMMA descriptors.
-// Every GEMM of the OPD path (logits, G re-formation, grad_hidden, grad_W) is this kernel with a
-// different epilogue (see opd_epilogues.cuh).
+//   TMA (SWIZZLE_128B) -> shared-memory ring -> tcgen05.mma (bf16 -> fp32) -> double-buffered TMEM
+//   accumulators -> per-tile epilogue functor run by 4 epilogue warps.
+// Two tile configurations of the same code (template parameter CG = tcgen05 cta_group):
+//   CG = 1   one CTA per tile, 128 x 256 x 16 MMAs, 4 stages of 48 KiB
+//   CG = 2   a CTA pair (cluster of 2, one SM each) per 256 x 256 tile: each CTA loads its own 128 rows of A and
+//            its own 128 of B's 256 columns, the pair leader issues 256 x 256 x 16 MMAs that read both CTAs'
+//            shared memory and write 128 accumulator rows into each CTA's TMEM; 6 stages of 32 KiB.  Per SM this
+//            moves 2/3 of the operand bytes of CG = 1 through L2 -> SMEM and halves the B reads of the MMA.
+// A and B may each be K-major (K contiguous in global memory) or MN-major (M/N contiguous); the majorness is a
+// run-time parameter that only changes the TMA box sequence and the UMMA descriptors.
+// Every GEMM of the OPD path (logits, G re-formation, grad_hidden, grad_W) runs on this core with a different
+// epilogue (opd_epilogues.cuh), either as gemm_kernel (one GEMM per launch) or inside bwd_kernel.
 #pragma once
 #include "opd_ptx.cuh"
 
 namespace opd {
 
-constexpr int BM = 128;              // tile rows   (TMEM lanes)
+constexpr int BM = 128;              // accumulator rows per CTA (TMEM lanes)
 constexpr int BN = 256;              // tile cols   (TMEM columns, fp32)
 constexpr int BK = 64;               // bf16 elements per k-block = one 128-byte swizzle row
 constexpr int UMMA_K = 16;
-constexpr int STAGES = 4;
-constexpr int A_STAGE_BYTES = BM * BK * 2;            // 16 KiB
-constexpr int B_STAGE_BYTES = BN * BK * 2;            // 32 KiB
-constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
 constexpr int MN_BOX = 64;                            // MN-major operands arrive as 64(mn) x 64(k) boxes
 constexpr int MN_BOX_BYTES = MN_BOX * BK * 2;         // 8 KiB
 constexpr int GEMM_THREADS = 192;                     // warp0 TMA, warp1 MMA(+TMEM alloc), warps2-5 epilogue
 constexpr int EPI_SMEM_BYTES = 32768;                 // 4 epilogue warps x 2 staging buffers x (32 rows x 128 B)
-constexpr int GEMM_SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*barriers*/ + EPI_SMEM_BYTES + 1024 /*align slack*/;
 constexpr int TMEM_COLS = 512;                        // 2 accumulator stages x 256 columns
+constexpr int MAX_STAGES = 6;
+
+template <int CG>
+struct Cfg {
+    static constexpr int TILE_M = BM * CG;                // rows of one tile (of the CTA or of the pair)
+    static constexpr int B_ROWS = BN / CG;                // B rows (n) each CTA loads
+    static constexpr int A_STAGE_BYTES = BM * BK * 2;     // 16 KiB
+    static constexpr int B_STAGE_BYTES = B_ROWS * BK * 2; // 32 / 16 KiB
+    static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
+    static constexpr int STAGES = CG == 1 ? 4 : 6;
+    static constexpr int RING_BYTES = STAGES * STAGE_BYTES;
+    static constexpr int SMEM_BYTES = RING_BYTES + 1024 /*barriers*/ + EPI_SMEM_BYTES + 1024 /*align slack*/;
+};
 
 enum TokDim { TOK_NONE = 0, TOK_M = 1, TOK_K = 2 };
 constexpr int MAX_SEG = 6;
@@ -55,21 +69,172 @@ __device__ __forceinline__ void tile_coords(int tile, int num_m, int num_n, int 
     n_blk = r / gm;
 }
 
-// Epi must provide:  struct Params;  static __device__ void run(const Params&, const GemmParams&, uint32_t taddr,
-//                    int m_blk, int n_blk, int row_in_tile, int M_eff, uint8_t* epi_smem, int epi_tid)
-template <class Epi>
+// ------------------------------------------------------------------------------------------------ pipeline
+// Shared-memory carve-up, barriers and TMEM of one CTA.
+//   full[s]    (leader's copy is the live one for CG = 2) TMA bytes of stage s have landed (both CTAs' bytes)
+//   empty[s]   the MMAs that read stage s have completed (commit, multicast to both CTAs for CG = 2)
+//   tfull[a]   accumulator stage a is complete (commit, multicast)
+//   tempty[a]  (leader's copy) all 4*CG epilogue warps have drained accumulator stage a
+template <int CG>
+struct Pipe {
+    using C = Cfg<CG>;
+    uint8_t* smem;
+    uint64_t *full_bar, *empty_bar, *tfull_bar, *tempty_bar;
+    uint32_t* tmem_slot;
+    uint8_t* epi_smem;
+    uint32_t tmem_base;
+    uint32_t rank;            // CTA rank in the pair (0 = leader; always 0 for CG = 1)
+
+    __device__ __forceinline__ void setup(uint8_t* smem_raw, int warp, int lane) {
+        smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+        full_bar = reinterpret_cast<uint64_t*>(smem + C::RING_BYTES);
+        empty_bar = full_bar + MAX_STAGES;
+        tfull_bar = empty_bar + MAX_STAGES;
+        tempty_bar = tfull_bar + 2;
+        tmem_slot = reinterpret_cast<uint32_t*>(tempty_bar + 2);
+        epi_smem = smem + C::RING_BYTES + 1024;
+        rank = CG == 1 ? 0u : cluster_ctarank();
+        if (warp == 0 && lane == 0) {
+            for (int s = 0; s < C::STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+            for (int s = 0; s < 2; ++s) { mbar_init(&tfull_bar[s], 1); mbar_init(&tempty_bar[s], 4 * CG); }
+            fence_mbar_init();
+        }
+        if (warp == 1) {
+            tmem_alloc<CG>(tmem_slot, TMEM_COLS);
+            tmem_relinquish<CG>();
+        }
+        tc_fence_before();
+        if constexpr (CG == 1) __syncthreads(); else cluster_sync_all();
+        tc_fence_after();
+        tmem_base = *tmem_slot;
+    }
+    __device__ __forceinline__ void teardown(int warp) {
+        tc_fence_before();
+        if constexpr (CG == 1) __syncthreads(); else cluster_sync_all();   // the peer may still signal our barriers
+        if (warp == 1) tmem_dealloc<CG>(tmem_base, TMEM_COLS);
+    }
+};
+
+// One tile's operand stream as the TMA producer of ONE CTA sees it.
+struct TileOp {
+    const CUtensorMap* tA;
+    const CUtensorMap* tB;
+    int a_mn, b_mn;
+    int a_c, b_c;             // first M row of A / first N row of B this CTA loads
+    int ka, kb;               // K offsets
+    int K;
+    int nseg;
+    unsigned char pa[MAX_SEG], pb[MAX_SEG];   // plane per segment
+};
+
+// TMA producer (one elected lane): stream all k-blocks of all segments of `t` through the ring.
+template <int CG>
+__device__ __forceinline__ void produce_tile(const Pipe<CG>& P, const TileOp& t, int& it) {
+    using C = Cfg<CG>;
+    const int kblocks = (t.K + BK - 1) / BK;
+    for (int seg = 0; seg < t.nseg; ++seg) {
+        for (int kb_i = 0; kb_i < kblocks; ++kb_i, ++it) {
+            const int s = it % C::STAGES;
+            const uint32_t ph = (it / C::STAGES) & 1;
+            mbar_wait(&P.empty_bar[s], ph ^ 1);
+            uint8_t* sA = P.smem + s * C::STAGE_BYTES;
+            uint8_t* sB = sA + C::A_STAGE_BYTES;
+            const int kca = t.ka + kb_i * BK, kcb = t.kb + kb_i * BK;
+            const int pa = t.pa[seg], pb = t.pb[seg];
+            if constexpr (CG == 1) {
+                uint64_t* bar = &P.full_bar[s];
+                mbar_arrive_expect_tx(bar, C::STAGE_BYTES);
+                if (t.a_mn) {
+                    for (int b = 0; b < BM / MN_BOX; ++b) tma_load_3d(sA + b * MN_BOX_BYTES, t.tA, bar, t.a_c + b * MN_BOX, kca, pa);
+                } else {
+                    tma_load_3d(sA, t.tA, bar, kca, t.a_c, pa);
+                }
+                if (t.b_mn) {
+                    for (int b = 0; b < C::B_ROWS / MN_BOX; ++b) tma_load_3d(sB + b * MN_BOX_BYTES, t.tB, bar, t.b_c + b * MN_BOX, kcb, pb);
+                } else {
+                    tma_load_3d(sB, t.tB, bar, kcb, t.b_c, pb);
+                }
+            } else {
+                // the leader's barrier counts the bytes of both CTAs (expect_tx may trail the peer's complete_tx:
+                // the phase cannot complete before the leader's own arrival)
+                if (P.rank == 0) mbar_arrive_expect_tx(&P.full_bar[s], 2 * C::STAGE_BYTES);
+                const uint32_t bar = mapa_rank(smem_u32(&P.full_bar[s]), 0);
+                if (t.a_mn) {
+                    for (int b = 0; b < BM / MN_BOX; ++b) tma_load_3d_pair(sA + b * MN_BOX_BYTES, t.tA, bar, t.a_c + b * MN_BOX, kca, pa);
+                } else {
+                    tma_load_3d_pair(sA, t.tA, bar, kca, t.a_c, pa);
+                }
+                if (t.b_mn) {
+                    for (int b = 0; b < C::B_ROWS / MN_BOX; ++b) tma_load_3d_pair(sB + b * MN_BOX_BYTES, t.tB, bar, t.b_c + b * MN_BOX, kcb, pb);
+                } else {
+                    tma_load_3d_pair(sB, t.tB, bar, kcb, t.b_c, pb);
+                }
+            }
+        }
+    }
+}
+
+// MMA issuer (one elected lane of the CTA / of the pair leader): all MMAs of one tile into accumulator stage lt & 1.
+template <int CG>
+__device__ __forceinline__ void mma_tile(const Pipe<CG>& P, int a_mn, int b_mn, int kiters, int lt, int& it) {
+    using C = Cfg<CG>;
+    const uint32_t idesc = make_idesc_bf16(C::TILE_M, BN, a_mn, b_mn);
+    const uint32_t a_kstep = a_mn ? (UMMA_K * MN_BOX * 2) : (UMMA_K * 2);   // bytes per UMMA_K step
+    const uint32_t b_kstep = b_mn ? (UMMA_K * MN_BOX * 2) : (UMMA_K * 2);
+    const uint32_t a_lbo = a_mn ? MN_BOX_BYTES : 16;
+    const uint32_t b_lbo = b_mn ? MN_BOX_BYTES : 16;
+    const int as = lt & 1;
+    const uint32_t aph = (lt >> 1) & 1;
+    mbar_wait(&P.tempty_bar[as], aph ^ 1);
+    tc_fence_after();
+    const uint32_t tacc = P.tmem_base + as * BN;
+    for (int ki = 0; ki < kiters; ++ki, ++it) {
+        const int s = it % C::STAGES;
+        const uint32_t ph = (it / C::STAGES) & 1;
+        mbar_wait(&P.full_bar[s], ph);
+        tc_fence_after();
+        const uint32_t a0 = smem_u32(P.smem + s * C::STAGE_BYTES);
+        const uint32_t b0 = a0 + C::A_STAGE_BYTES;
+#pragma unroll
+        for (int k = 0; k < BK / UMMA_K; ++k) {
+            const uint64_t ad = make_smem_desc(a0 + k * a_kstep, a_lbo, 1024);
+            const uint64_t bd = make_smem_desc(b0 + k * b_kstep, b_lbo, 1024);
+            umma_bf16<CG>(tacc, ad, bd, idesc, (ki | k) != 0);
+        }
+        umma_commit<CG>(&P.empty_bar[s]);          // frees the smem slot (in both CTAs) once these MMAs have read it
+    }
+    umma_commit<CG>(&P.tfull_bar[as]);             // accumulator complete -> epilogue warps (of both CTAs)
+}
+
+// Epilogue side: wait for accumulator stage lt & 1; returns this warp's TMEM address (lane quarter in bits 16+).
+template <int CG>
+__device__ __forceinline__ uint32_t epi_acquire(const Pipe<CG>& P, int lt, int quarter) {
+    const int as = lt & 1;
+    mbar_wait(&P.tfull_bar[as], (lt >> 1) & 1);
+    tc_fence_after();
+    return P.tmem_base + as * BN + (static_cast<uint32_t>(quarter * 32) << 16);
+}
+template <int CG>
+__device__ __forceinline__ void epi_release(const Pipe<CG>& P, int lt, int lane) {
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) {
+        if constexpr (CG == 1) mbar_arrive(&P.tempty_bar[lt & 1]);
+        else mbar_arrive_cluster(mapa_rank(smem_u32(&P.tempty_bar[lt & 1]), 0));
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ one GEMM per launch
+// Epi must provide:  struct Params;  struct State;  static State prepare(...);
+//                    static void run(const Params&, const GemmParams&, State, uint32_t taddr, int m_blk, int n_blk,
+//                                    int row_in_tile, int M_eff, uint8_t* epi_smem, int epi_tid)
+// with m_blk counting 128-row blocks (for CG = 2 the pair's tile is row blocks 2*m2 and 2*m2 + 1).
+template <class Epi, int CG>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
             const GemmParams gp, const __grid_constant__ typename Epi::Params ep) {
+    using C = Cfg<CG>;
     extern __shared__ uint8_t smem_raw[];
-    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + STAGES * STAGE_BYTES);
-    uint64_t* empty_bar = full_bar + STAGES;
-    uint64_t* tfull_bar = empty_bar + STAGES;
-    uint64_t* tempty_bar = tfull_bar + 2;
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty_bar + 2);
-    uint8_t* epi_smem = smem + STAGES * STAGE_BYTES + 1024;
-
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
 
@@ -80,95 +245,39 @@ gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         if (gp.tok_dim == TOK_M) M = min(M, live);
         else K = min(K, live);
     }
-    if (M <= 0 || K <= 0) return;
-    const int num_m = (M + BM - 1) / BM;
+    if (M <= 0 || K <= 0) return;                     // uniform over the grid
+    const int num_m = (M + C::TILE_M - 1) / C::TILE_M;
     const int num_n = gp.num_n;
     const int total_tiles = num_m * num_n;
     const int kblocks = (K + BK - 1) / BK;
-    const int kiters = kblocks * gp.nseg;
+    const int first_tile = blockIdx.x / CG, tile_step = gridDim.x / CG;
 
-    if (warp == 0 && lane == 0) {
-        prefetch_tmap(&tmA);
-        prefetch_tmap(&tmB);
-        for (int s = 0; s < STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
-        for (int s = 0; s < 2; ++s) { mbar_init(&tfull_bar[s], 1); mbar_init(&tempty_bar[s], 4); }
-        fence_mbar_init();
-    }
-    if (warp == 1) {
-        tmem_alloc(tmem_slot, TMEM_COLS);
-        tmem_relinquish();
-    }
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem_base = *tmem_slot;
+    if (warp == 0 && lane == 0) { prefetch_tmap(&tmA); prefetch_tmap(&tmB); }
+    Pipe<CG> P;
+    P.setup(smem_raw, warp, lane);
 
     if (warp == 0) {
         // =========================== TMA producer (one elected lane) ===========================
         if (elect_one()) {
+            TileOp t;
+            t.tA = &tmA; t.tB = &tmB; t.a_mn = gp.a_mn; t.b_mn = gp.b_mn; t.ka = gp.ka_off; t.kb = gp.kb_off; t.K = K;
+            t.nseg = gp.nseg;
+            for (int i = 0; i < MAX_SEG; ++i) { t.pa[i] = gp.sa[i]; t.pb[i] = gp.sb[i]; }
             int it = 0;
-            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-                int m_blk, n_blk;
-                tile_coords(tile, num_m, num_n, gp.group_m, m_blk, n_blk);
-                const int a_mn0 = gp.a_off + m_blk * BM;
-                const int b_mn0 = gp.b_off + n_blk * BN;
-                for (int ki = 0; ki < kiters; ++ki, ++it) {
-                    const int s = it % STAGES;
-                    const uint32_t ph = (it / STAGES) & 1;
-                    mbar_wait(&empty_bar[s], ph ^ 1);
-                    const int seg = ki / kblocks;
-                    const int kk = (ki - seg * kblocks) * BK;
-                    const int kca = gp.ka_off + kk, kcb = gp.kb_off + kk;
-                    uint8_t* sA = smem + s * STAGE_BYTES;
-                    uint8_t* sB = sA + A_STAGE_BYTES;
-                    mbar_arrive_expect_tx(&full_bar[s], STAGE_BYTES);
-                    if (gp.a_mn) {
-                        for (int b = 0; b < BM / MN_BOX; ++b)
-                            tma_load_3d(sA + b * MN_BOX_BYTES, &tmA, &full_bar[s], a_mn0 + b * MN_BOX, kca, gp.sa[seg]);
-                    } else {
-                        tma_load_3d(sA, &tmA, &full_bar[s], kca, a_mn0, gp.sa[seg]);
-                    }
-                    if (gp.b_mn) {
-                        for (int b = 0; b < BN / MN_BOX; ++b)
-                            tma_load_3d(sB + b * MN_BOX_BYTES, &tmB, &full_bar[s], b_mn0 + b * MN_BOX, kcb, gp.sb[seg]);
-                    } else {
-                        tma_load_3d(sB, &tmB, &full_bar[s], kcb, b_mn0, gp.sb[seg]);
-                    }
-                }
+            for (int tile = first_tile; tile < total_tiles; tile += tile_step) {
+                int m2, n_blk;
+                tile_coords(tile, num_m, num_n, gp.group_m, m2, n_blk);
+                t.a_c = gp.a_off + (m2 * CG + static_cast<int>(P.rank)) * BM;
+                t.b_c = gp.b_off + n_blk * BN + static_cast<int>(P.rank) * C::B_ROWS;
+                produce_tile<CG>(P, t, it);
             }
         }
     } else if (warp == 1) {
-        // =========================== MMA issuer (one elected lane) ===========================
-        if (elect_one()) {
-            const uint32_t idesc = make_idesc_bf16(BM, BN, gp.a_mn, gp.b_mn);
-            const uint32_t a_kstep = gp.a_mn ? (UMMA_K * MN_BOX * 2) : (UMMA_K * 2);   // bytes per UMMA_K step
-            const uint32_t b_kstep = gp.b_mn ? (UMMA_K * MN_BOX * 2) : (UMMA_K * 2);
-            const uint32_t a_lbo = gp.a_mn ? MN_BOX_BYTES : 16;
-            const uint32_t b_lbo = gp.b_mn ? MN_BOX_BYTES : 16;
+        // =========================== MMA issuer (one elected lane of the leader) ===========================
+        if (P.rank == 0 && elect_one()) {
             int it = 0, lt = 0;
-            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++lt) {
-                const int as = lt & 1;
-                const uint32_t aph = (lt >> 1) & 1;
-                mbar_wait(&tempty_bar[as], aph ^ 1);
-                tc_fence_after();
-                const uint32_t tacc = tmem_base + as * BN;
-                for (int ki = 0; ki < kiters; ++ki, ++it) {
-                    const int s = it % STAGES;
-                    const uint32_t ph = (it / STAGES) & 1;
-                    mbar_wait(&full_bar[s], ph);
-                    tc_fence_after();
-                    const uint32_t a0 = smem_u32(smem + s * STAGE_BYTES);
-                    const uint32_t b0 = a0 + A_STAGE_BYTES;
-#pragma unroll
-                    for (int k = 0; k < BK / UMMA_K; ++k) {
-                        const uint64_t ad = make_smem_desc(a0 + k * a_kstep, a_lbo, 1024);
-                        const uint64_t bd = make_smem_desc(b0 + k * b_kstep, b_lbo, 1024);
-                        umma_bf16(tacc, ad, bd, idesc, (ki | k) != 0);
-                    }
-                    umma_commit(&empty_bar[s]);          // frees the smem slot once these MMAs have read it
-                }
-                umma_commit(&tfull_bar[as]);             // accumulator complete -> epilogue
-            }
+            for (int tile = first_tile; tile < total_tiles; tile += tile_step, ++lt)
+                mma_tile<CG>(P, gp.a_mn, gp.b_mn, kblocks * gp.nseg, lt, it);
         }
     } else {
         // =========================== epilogue warps (TMEM -> registers -> global) ===========================
@@ -176,26 +285,18 @@ gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         const int row_in_tile = quarter * 32 + lane;
         const int epi_tid = (warp - 2) * 32 + lane;
         int lt = 0;
-        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++lt) {
-            int m_blk, n_blk;
-            tile_coords(tile, num_m, num_n, gp.group_m, m_blk, n_blk);
-            const int as = lt & 1;
-            const uint32_t aph = (lt >> 1) & 1;
+        for (int tile = first_tile; tile < total_tiles; tile += tile_step, ++lt) {
+            int m2, n_blk;
+            tile_coords(tile, num_m, num_n, gp.group_m, m2, n_blk);
+            const int m_blk = m2 * CG + static_cast<int>(P.rank);
             // per-row state (scalars, cache cursor) is fetched while the MMAs of this tile are still running
             typename Epi::State st = Epi::prepare(ep, gp, m_blk, n_blk, row_in_tile, M);
-            mbar_wait(&tfull_bar[as], aph);
-            tc_fence_after();
-            const uint32_t taddr = tmem_base + as * BN + (static_cast<uint32_t>(quarter * 32) << 16);
-            Epi::run(ep, gp, st, taddr, m_blk, n_blk, row_in_tile, M, epi_smem, epi_tid);
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&tempty_bar[as]);
+            const uint32_t taddr = epi_acquire<CG>(P, lt, quarter);
+            Epi::run(ep, gp, st, taddr, m_blk, n_blk, row_in_tile, M, P.epi_smem, epi_tid);
+            epi_release<CG>(P, lt, lane);
         }
     }
-
-    tc_fence_before();
-    __syncthreads();
-    if (warp == 1) tmem_dealloc(tmem_base, TMEM_COLS);
+    P.teardown(warp);
 }
 
 }  // namespace opd

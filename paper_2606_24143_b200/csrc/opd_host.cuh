@@ -5,7 +5,9 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
 #include <string>
+#include <utility>
 
 #include "../../include/opd.h"
 #include "opd_bwd_kernel.cuh"
@@ -14,6 +16,7 @@
 struct opd_handle_s {
     int device = 0;
     int num_sms = 0;
+    int cg = 2;                    // tcgen05 cta_group of the GEMM core: 2 = CTA pairs (default), 1 = single CTAs (OPD_CTA_GROUP)
     bool arch_ok = false;
     void* ws = nullptr;            // workspace in use
     size_t ws_bytes = 0;
@@ -97,15 +100,21 @@ inline int env_int(const char* name, int dflt) {
     return (s && *s) ? std::atoi(s) : dflt;
 }
 
+inline int cta_group_setting() {
+    const int cg = env_int("OPD_CTA_GROUP", 2);
+    return cg == 1 ? 1 : 2;
+}
+
 inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags) {
     Plan p{};
     p.T = T; p.d = d; p.V = V; p.C = C; p.planes = fp32 ? 3 : 1;
-    p.t_pad = ceil_div(T, BM) * BM;
+    const int TM = BM * cta_group_setting();              // tile rows of the GEMM core (CTA or CTA pair)
+    p.t_pad = ceil_div(T, TM) * TM;
     p.num_n = ceil_div(V, BN);
-    // Super-tile of the backward: 37 row tiles x 16 column tiles = 592 = 4 x 148 tiles per launch on a 148-SM B200
-    // (whole waves for the G and grad_hidden GEMMs); 4736 x 4096 bf16 = 37 MiB stays resident in the 126 MB L2.
-    const int tb = env_int("OPD_TB", 37 * BM), vb = env_int("OPD_VB", 4096);
-    p.Tb = std::min(p.t_pad, std::max(BM, tb / BM * BM));
+    // Super-tile of the backward: 4608 (4736 for single-CTA tiles) token rows x 4096 vocabulary columns = 288 pair
+    // tiles (592 CTA tiles) per G re-formation; the bf16 G super-tile (36-37 MiB) is consumed out of L2.
+    const int tb = env_int("OPD_TB", TM == 256 ? 18 * 256 : 37 * BM), vb = env_int("OPD_VB", 4096);
+    p.Tb = std::min(p.t_pad, std::max(TM, tb / TM * TM));
     p.Vb = std::min(p.num_n * BN, std::max(BN, vb / BN * BN));
     p.est_blocks = ceil_div(T, 128);
     size_t o = 0;
@@ -143,22 +152,35 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags) {
 }
 
 // ---------------------------------------------------------------- GEMM launcher
+// Launch `kernel` on `grid` CTAs of GEMM_THREADS threads; CG = 2 launches clusters of two CTAs (a pair per tile).
+template <int CG, class... KArgs, class... Args>
+inline cudaError_t launch_cg(void (*kernel)(KArgs...), int grid, cudaStream_t st, Args&&... args) {
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<CG>::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(GEMM_THREADS); cfg.dynamicSmemBytes = Cfg<CG>::SMEM_BYTES; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
+template <class Epi, int CG>
+inline cudaError_t launch_gemm_cg(opd_handle_s* h, cudaStream_t st, const CUtensorMap& tA, const CUtensorMap& tB,
+                                  const GemmParams& gp, const typename Epi::Params& ep) {
+    const long tiles = (long)ceil_div(gp.M, Cfg<CG>::TILE_M) * gp.num_n;
+    const int grid = CG * (int)std::min<long>(tiles, h->num_sms / CG);
+    if (grid <= 0) return cudaSuccess;
+    cudaError_t e = launch_cg<CG>(gemm_kernel<Epi, CG>, grid, st, tA, tB, gp, ep);
+    h->n_kernels++;
+    h->n_gemm++;
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
 template <class Epi>
 inline cudaError_t launch_gemm(opd_handle_s* h, cudaStream_t st, const CUtensorMap& tA, const CUtensorMap& tB,
                                const GemmParams& gp, const typename Epi::Params& ep) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(gemm_kernel<Epi>, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
-    const long tiles = (long)ceil_div(gp.M, BM) * gp.num_n;
-    const int grid = (int)std::min<long>(tiles, h->num_sms);
-    if (grid <= 0) return cudaSuccess;
-    gemm_kernel<Epi><<<grid, GEMM_THREADS, GEMM_SMEM_BYTES, st>>>(tA, tB, gp, ep);
-    h->n_kernels++;
-    h->n_gemm++;
-    return cudaGetLastError();
+    return h->cg == 2 ? launch_gemm_cg<Epi, 2>(h, st, tA, tB, gp, ep) : launch_gemm_cg<Epi, 1>(h, st, tA, tB, gp, ep);
 }
 
 inline void set_segments(GemmParams& gp, int planes) {

@@ -22,10 +22,11 @@ extern "C" opd_status_t opd_debug_gemm(opd_handle_t h, void* cuda_stream, int M,
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     CUtensorMap tA, tB;
     bool ok = true;
+    h->cg = cta_group_setting();
     if (a_mn) ok &= make_map(&tA, A, M, K, 1, (uint64_t)M * 2, (uint64_t)M * K * 2, MN_BOX);
     else      ok &= make_map(&tA, A, K, M, 1, (uint64_t)K * 2, (uint64_t)M * K * 2, BM);
     if (b_mn) ok &= make_map(&tB, B, N, K, 1, (uint64_t)N * 2, (uint64_t)N * K * 2, MN_BOX);
-    else      ok &= make_map(&tB, B, K, N, 1, (uint64_t)K * 2, (uint64_t)N * K * 2, BN);
+    else      ok &= make_map(&tB, B, K, N, 1, (uint64_t)K * 2, (uint64_t)N * K * 2, BN / h->cg);
     if (!ok) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled failed");
     GemmParams gp{};
     gp.M = M; gp.N = N; gp.K = K; gp.num_n = ceil_div(N, BN); gp.group_m = 8;

@@ -63,6 +63,8 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     if (!get_encode_fn()) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
 
     OPD_CUDA(h, cudaSetDevice(h->device));
+    h->cg = cta_group_setting();
+    const uint32_t b_box = BN / h->cg;                    // rows of a K-major B box: each CTA of a pair loads half of N
     const Plan p = make_plan(T, d, V, C, fp32, a.flags | (a.stop_after_fwd ? OPD_F_FWD_ONLY : 0));
     s = ensure_workspace(h, p.total);
     if (s != OPD_OK) return s;
@@ -122,9 +124,9 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     const uint64_t wplane_b = fp32 ? wq_plane * 2 : (uint64_t)ldwq * 2 * (wl == 0 ? d : V);
     if (wl == 0) {   // W [d][V]: logits B is MN-major (n = v contiguous); dX B is K-major (k = v contiguous)
         ok &= make_map(&m_w_fwd, wq, V, d, np, (uint64_t)ldwq * 2, wplane_b, MN_BOX);
-        ok &= make_map(&m_w_dx, wq, V, d, np, (uint64_t)ldwq * 2, wplane_b, BN);
+        ok &= make_map(&m_w_dx, wq, V, d, np, (uint64_t)ldwq * 2, wplane_b, b_box);
     } else {         // W [V][d]: logits B is K-major; dX B is MN-major (n = d contiguous, k = v rows)
-        ok &= make_map(&m_w_fwd, wq, d, V, np, (uint64_t)ldwq * 2, wplane_b, BN);
+        ok &= make_map(&m_w_fwd, wq, d, V, np, (uint64_t)ldwq * 2, wplane_b, b_box);
         ok &= make_map(&m_w_dx, wq, d, V, np, (uint64_t)ldwq * 2, wplane_b, MN_BOX);
     }
     if (!fwd_only) {
@@ -181,7 +183,7 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
 
     // ------------------------------------------------------------------ S6-S8 backward, super-tile by super-tile
     phase_mark(h, st, OPD_PHASE_BWD, 0);
-    if (!fwd_only && !env_int("OPD_BWD_LEGACY", 0)) {
+    if (!fwd_only) {
         // one persistent kernel walks every super-tile: G re-formation, grad_hidden and grad_W tiles interleaved,
         // ordered by dependency counters in global memory (opd_bwd_kernel.cuh)
         int* counters = reinterpret_cast<int*>(ws + p.off_counters);
@@ -189,62 +191,15 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         BwdParams bp{};
         bp.d = d; bp.V = V; bp.Tb = p.Tb; bp.Vb = p.Vb; bp.nvb = ceil_div(V, p.Vb); bp.wl = wl; bp.planes = p.planes;
         bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super;
-        bp.g = GEpi::Params{gs, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V};
+        bp.g = GEpi::Params{gs, p.Tb, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V};
         bp.dx = dxp;
         bp.dw = dwp;
-        static bool attr_set = false;
-        if (!attr_set) {
-            OPD_CUDA(h, cudaFuncSetAttribute(bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM_SMEM_BYTES));
-            attr_set = true;
-        }
-        bwd_kernel<<<h->num_sms, GEMM_THREADS, GEMM_SMEM_BYTES, st>>>(m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, bp);
+        // every CTA (pair) must be resident at once: items wait on earlier items of other CTAs
+        const int grid = h->num_sms / h->cg * h->cg;
+        if (h->cg == 2) OPD_CUDA(h, launch_cg<2>(bwd_kernel<2>, grid, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, bp));
+        else OPD_CUDA(h, launch_cg<1>(bwd_kernel<1>, grid, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, bp));
         h->n_kernels++; h->n_gemm++;
         OPD_CUDA(h, cudaGetLastError());
-    }
-    if (!fwd_only && env_int("OPD_BWD_LEGACY", 0)) {   // one launch per GEMM and super-tile (kept for A/B timing)
-        const int nvb = ceil_div(V, p.Vb);
-        for (int tb0 = 0; tb0 < T; tb0 += p.Tb) {
-            const int Tb = std::min(p.Tb, p.t_pad - tb0);
-            for (int vi = 0; vi < nvb; ++vi) {
-                const int vb0 = vi * p.Vb;
-                const int Vb = std::min(p.Vb, V - vb0);
-                {   // S6: G super-tile = softmax-gradient of the recomputed logits (never leaves L2)
-                    GemmParams gp{};
-                    gp.M = Tb; gp.N = Vb; gp.K = d; gp.num_n = ceil_div(Vb, BN); gp.group_m = 1 << 20;
-                    gp.a_mn = 0; gp.b_mn = (wl == 0); gp.a_off = tb0; gp.b_off = vb0; gp.ka_off = 0; gp.kb_off = 0;
-                    set_segments(gp, p.planes);
-                    gp.tok_dim = TOK_M; gp.tok_off = tb0; gp.n_live = n_live;
-                    GEpi::Params ep{gs, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V};
-                    OPD_CUDA(h, launch_gemm<GEpi>(h, st, m_xc_k, m_w_fwd, gp, ep));
-                }
-                {   // S7: grad_hidden[tb] += G . W[:, vb]^T
-                    GemmParams gp{};
-                    gp.M = Tb; gp.N = d; gp.K = Vb; gp.num_n = ceil_div(d, BN); gp.group_m = 1 << 20;
-                    gp.a_mn = 0; gp.b_mn = (wl == 1); gp.a_off = 0; gp.b_off = 0; gp.ka_off = 0; gp.kb_off = vb0;
-                    set_segments(gp, p.planes);
-                    gp.tok_dim = TOK_M; gp.tok_off = tb0; gp.n_live = n_live;
-                    gp.first = (vi == 0); gp.last = (vi == nvb - 1);
-                    OPD_CUDA(h, launch_gemm<DxEpi>(h, st, m_gs_k, m_w_dx, gp, dxp));
-                }
-                {   // S8: grad_W[:, vb] += hidden[tb]^T . G
-                    GemmParams gp{};
-                    gp.group_m = 1 << 20; gp.tok_dim = TOK_K; gp.tok_off = tb0; gp.n_live = n_live; gp.K = Tb;
-                    gp.a_mn = 1; gp.b_mn = 1;
-                    set_segments(gp, p.planes);
-                    if (wl == 0) {   // rows = d (A = Xc^T), cols = v (B = G)
-                        gp.M = d; gp.N = Vb; gp.num_n = ceil_div(Vb, BN);
-                        gp.a_off = 0; gp.ka_off = tb0; gp.b_off = 0; gp.kb_off = 0;
-                        gp.row_off = 0; gp.col_off = vb0;
-                        OPD_CUDA(h, launch_gemm<DwEpi>(h, st, m_xc_mn, m_gs_mn, gp, dwp));
-                    } else {         // rows = v (A = G^T), cols = d (B = Xc)
-                        gp.M = Vb; gp.N = d; gp.num_n = ceil_div(d, BN);
-                        gp.a_off = 0; gp.ka_off = 0; gp.b_off = 0; gp.kb_off = tb0;
-                        gp.row_off = vb0; gp.col_off = 0;
-                        OPD_CUDA(h, launch_gemm<DwEpi>(h, st, m_gs_mn, m_xc_mn, gp, dwp));
-                    }
-                }
-            }
-        }
     }
     phase_mark(h, st, OPD_PHASE_BWD, 1);
 
