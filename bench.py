@@ -27,6 +27,12 @@ METRIC = "OPD loss fwd+bwd tokens/s on 1 B200; % of dense BF16 tensor peak"
 UNIT = "live tokens/s"
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from one `ncu --set full` capture (not measured live)
+NCU_TRAFFIC = {
+    "C4": dict(bwd_kernel=155_149_744_000, fwd_kernel=38_780_680_000, source="profiles/r01c_ncu_full_c4.md"),
+}
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -163,7 +169,6 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--ref-seconds", type=float, default=12.0)
-    ap.add_argument("--traffic-json", default=os.path.join(ROOT, "profiles", "traffic.json"))
     args = ap.parse_args()
     if args.mode is None:
         args.mode = "mixed" if args.config == 5 else "mc"
@@ -268,21 +273,24 @@ def main():
         return
 
     pk = peaks()
-    gemm_ms = pm["fwd"] + pm["bwd"]
+    # Roofline of the dominant kernel, opd::bwd_kernel (one launch per step: S6 logits recompute + S7 grad_hidden +
+    # S8 grad_W = 3 contractions of 2*d*V flops per live token), timed live with CUDA events on the
+    # launching stream (phase "bwd"); the forward kernel (S1-S3, 2*d*V per token) beside it.
     flops_exec = 8.0 * d * V * n_live            # logits + recomputed logits + dX + dW  (2 d V each)
-    ach = flops_exec / (gemm_ms * 1e-3) / 1e12
-    traffic = None
-    if os.path.exists(args.traffic_json):
-        try:
-            tj = json.load(open(args.traffic_json))
-            traffic = tj.get(f"C{args.config}", {}).get("dram_bytes_per_launch")
-        except Exception:
-            traffic = None
-    roofline = dict(bound="tensor", achieved=ach, peak=pk["sustained"], unit="TFLOP/s", frac=ach / pk["sustained"], traffic=traffic,
-                    kernel="opd::gemm_kernel<*> (logits, G re-formation, grad_hidden, grad_W: one tcgen05 core, four epilogues)",
-                    flops_per_step=flops_exec, gemm_launches_per_step=stats["gemm_kernels"], gemm_ms_per_step=gemm_ms,
+    bwd_flops, fwd_flops = 6.0 * d * V * n_live, 2.0 * d * V * n_live
+    ach = bwd_flops / (pm["bwd"] * 1e-3) / 1e12
+    ach_fwd = fwd_flops / (pm["fwd"] * 1e-3) / 1e12
+    tr = NCU_TRAFFIC.get(f"C{args.config}") if args.mode == "mc" and not args.tokens else None
+    roofline = dict(bound="tensor", achieved=ach, peak=pk["sustained"], unit="TFLOP/s", frac=ach / pk["sustained"],
+                    traffic=tr["bwd_kernel"] if tr else None,
+                    kernel="opd::bwd_kernel<2> (persistent: G re-formation, grad_hidden, grad_W tiles on tcgen05 cta_group::2)",
+                    flops_per_launch=bwd_flops, launches_per_step=1, ms_per_launch=pm["bwd"],
                     peak_kind=f"bf16_tflops_sustained of {pk['src']} (kernel timed inside a long step); burst peak {pk['burst']}",
-                    frac_of_burst=ach / pk["burst"])
+                    frac_of_burst=ach / pk["burst"],
+                    fwd_kernel=dict(kernel="opd::gemm_kernel<FwdEpi,2>", achieved=ach_fwd, frac=ach_fwd / pk["sustained"],
+                                    frac_of_burst=ach_fwd / pk["burst"], flops_per_launch=fwd_flops, ms_per_launch=pm["fwd"],
+                                    traffic=tr["fwd_kernel"] if tr else None),
+                    traffic_source=tr["source"] if tr else None)
     whole = flops_exec / (ms_per_step * 1e-3) / 1e12
     cpu = None
     if not args.no_cpu:

@@ -43,6 +43,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
            "-shared", "-Xcompiler", "-fPIC", "-I", INCLUDE,
            os.path.join(CSRC, "opd_lib.cu"), "-o", LIB]
+    cmd[1:1] = os.environ.get("OPD_NVCC_FLAGS", "").split()
     if verbose:
         cmd[1:1] = ["-Xptxas", "-v"]
     r = subprocess.run(cmd, capture_output=True, text=True)

@@ -24,6 +24,8 @@ struct BwdParams {
     const int* n_live;
     int* g_done;               // [S]
     int* c_done;               // [S]
+    int type_mask;             // timing experiments only: bit t set = run tiles of type t (7 = all; else no dependency waits)
+    unsigned long long hint_x, hint_w, hint_g;   // L2 eviction policies of the Xc / W / G-ring operand loads
     GEpi::Params g;            // gs points at ring buffer 0; buffer b at + b * planes * plane_stride
     DxEpi::Params dx;
     DwEpi::Params dw;
@@ -137,6 +139,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             BwdTile t;
             int it = 0;
             for (long item = first_item; sc.get(item, t); item += item_step) {
+                if (!((bp.type_mask >> t.type) & 1)) continue;
                 TileOp op;
                 int pa_off = 0, pb_off = 0;
                 const int buf = t.s & 1;
@@ -144,22 +147,26 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 if (t.type == T_G) {
                     op.tA = &m_xc_k; op.tB = &m_w_fwd; op.a_mn = 0; op.b_mn = (bp.wl == 0);
                     op.a_c = t.tb0 + a_row; op.b_c = t.vb0 + b_row; op.ka = 0; op.kb = 0; op.K = bp.d;
+                    op.a_hint = bp.hint_x; op.b_hint = bp.hint_w;
                 } else if (t.type == T_DX) {
                     op.tA = &m_gs_k; op.tB = &m_w_dx; op.a_mn = 0; op.b_mn = (bp.wl == 1);
                     op.a_c = a_row; op.b_c = b_row; op.ka = 0; op.kb = t.vb0; op.K = t.Vb_eff; pa_off = buf * bp.planes;
+                    op.a_hint = bp.hint_g; op.b_hint = bp.hint_w;
                 } else if (bp.wl == 0) {
                     op.tA = &m_xc_mn; op.tB = &m_gs_mn; op.a_mn = 1; op.b_mn = 1;
                     op.a_c = a_row; op.b_c = b_row; op.ka = t.tb0; op.kb = 0; op.K = t.Tb_eff; pb_off = buf * bp.planes;
+                    op.a_hint = bp.hint_x; op.b_hint = bp.hint_g;
                 } else {
                     op.tA = &m_gs_mn; op.tB = &m_xc_mn; op.a_mn = 1; op.b_mn = 1;
                     op.a_c = a_row; op.b_c = b_row; op.ka = 0; op.kb = t.tb0; op.K = t.Tb_eff; pa_off = buf * bp.planes;
+                    op.a_hint = bp.hint_g; op.b_hint = bp.hint_x;
                 }
                 op.nseg = nseg;
                 for (int i = 0; i < nseg; ++i) {
                     op.pa[i] = static_cast<unsigned char>(pa_off + (nseg == 1 ? 0 : PA[i]));
                     op.pb[i] = static_cast<unsigned char>(pb_off + (nseg == 1 ? 0 : PB[i]));
                 }
-                if (t.type != T_G) {                        // the G super-tile must be complete before TMA reads it
+                if (t.type != T_G && bp.type_mask == 7) {   // the G super-tile must be complete before TMA reads it
                     wait_counter(bp.g_done + t.s, CG * sc.nG(t.s));
                     fence_proxy_async_all();
                 }
@@ -172,12 +179,14 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             BwdSched<CG> sc; sc.init(bp);
             BwdTile t;
             int it = 0, lt = 0;
-            for (long item = first_item; sc.get(item, t); item += item_step, ++lt) {
+            for (long item = first_item; sc.get(item, t); item += item_step) {
+                if (!((bp.type_mask >> t.type) & 1)) continue;
                 int a_mn, b_mn, K;
                 if (t.type == T_G) { a_mn = 0; b_mn = (bp.wl == 0); K = bp.d; }
                 else if (t.type == T_DX) { a_mn = 0; b_mn = (bp.wl == 1); K = t.Vb_eff; }
                 else { a_mn = 1; b_mn = 1; K = t.Tb_eff; }
                 mma_tile<CG>(P, a_mn, b_mn, ((K + BK - 1) / BK) * nseg, lt, it);
+                ++lt;
             }
         }
     } else {
@@ -188,13 +197,14 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
         BwdSched<CG> sc; sc.init(bp);
         BwdTile t;
         int lt = 0;
-        for (long item = first_item; sc.get(item, t); item += item_step, ++lt) {
+        for (long item = first_item; sc.get(item, t); item += item_step) {
+            if (!((bp.type_mask >> t.type) & 1)) continue;
             const int m_blk = t.m_blk * CG + rank;    // this CTA's 128-row block inside the GEMM
             GemmParams gp{};                      // the fields the epilogues read
             gp.tok_off = t.tb0;
             // wait for the previous writer / readers of what this epilogue is about to write
             const int dep = (t.type == T_G) ? t.s - 2 : t.s - 1;
-            if (dep >= 0) {
+            if (dep >= 0 && bp.type_mask == 7) {
                 if (lane == 0) { wait_counter(bp.c_done + dep, CG * (sc.nDX(dep) + sc.nDW(dep))); fence_proxy_async_all(); }
                 __syncwarp();
             }
@@ -218,6 +228,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 DwEpi::run(bp.dw, gp, NoState{}, taddr, m_blk, t.n_blk, row_in_tile, M_eff, P.epi_smem, epi_tid);
             }
             epi_release<CG>(P, lt, lane);                       // TMEM stage free for the MMA warp
+            ++lt;
             // publish: all 128 epilogue threads' global stores, then one release increment
             __threadfence();
             fence_proxy_async_all();

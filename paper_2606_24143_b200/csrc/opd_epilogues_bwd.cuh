@@ -101,7 +101,7 @@ struct GEpi {
 // buffers and one lane issues a TMA store or reduce-add: the read-modify-write of the fp32 accumulators happens in
 // L2, the epilogue never waits on a load.  `wbuf` is this warp's 8 KiB (1024-byte aligned) region.
 __device__ __forceinline__ void stage_and_send(const CUtensorMap* tm, uint8_t* wbuf, int parity, const float (&v)[32],
-                                               int lane, int col, int row, bool reduce) {
+                                               int lane, int col, int row, bool reduce, uint64_t hint) {
     uint8_t* buf = wbuf + parity * 4096;
     if (lane == 0) bulk_wait_read<1>();          // the group that last used this buffer has finished reading it
     __syncwarp();
@@ -112,7 +112,7 @@ __device__ __forceinline__ void stage_and_send(const CUtensorMap* tm, uint8_t* w
     fence_proxy_async_smem();
     __syncwarp();
     if (lane == 0) {
-        if (reduce) tma_reduce_add_2d(tm, buf, col, row); else tma_store_2d(tm, buf, col, row);
+        if (reduce) tma_reduce_add_2d(tm, buf, col, row, hint); else tma_store_2d(tm, buf, col, row, hint);
         bulk_commit();
     }
 }
@@ -129,6 +129,8 @@ __device__ __forceinline__ void drain_sends(int lane) {
 struct DxEpi {
     struct Params {
         CUtensorMap m_acc;       // fp32 [Tb_pad][d], boxes of 32 x 32
+        uint64_t hint;           // L2 eviction policy of the partial-sum stores / reductions
+        int dbg;                 // timing experiments: 1 = plain stores instead of reductions, 2 = no output
         float* acc;              // same buffer, for the last super-tile's read
         long ld_acc;
         void* out;               // grad_hidden
@@ -158,8 +160,9 @@ struct DxEpi {
             tmem_ld_wait();
             const int col0 = n_blk * BN + c * 32;
             if (col0 >= gp.N) break;                                  // d % 64 == 0: chunks are all-in or all-out (warp-uniform)
+            if (p.dbg == 2) continue;
             if (!gp.last) {
-                stage_and_send(&p.m_acc, wbuf, c & 1, v, lane, col0, lrow - lane, !gp.first);
+                stage_and_send(&p.m_acc, wbuf, c & 1, v, lane, col0, lrow - lane, !gp.first && p.dbg != 1, p.hint);
             } else if (live) {
                 if (!gp.first) {
                     const float4* a4 = reinterpret_cast<const float4*>(acc + c * 32);
@@ -193,6 +196,8 @@ struct DxEpi {
 struct DwEpi {
     struct Params {
         CUtensorMap m_gw;        // fp32 [rows_total][cols_total] (row stride ld), boxes of 32 x 32
+        uint64_t hint;           // L2 eviction policy of the grad_W reductions
+        int dbg;                 // timing experiments: 1 = plain stores instead of reductions, 2 = no output
     };
     using State = NoState;
     static __device__ __forceinline__ State prepare(const Params&, const GemmParams&, int, int, int, int) { return {}; }
@@ -209,7 +214,7 @@ struct DwEpi {
             tmem_ld_wait();
             const int lc0 = n_blk * BN + c * 32;
             if (lc0 >= gp.N) break;
-            if (warp_ok) stage_and_send(&p.m_gw, wbuf, c & 1, v, lane, gp.col_off + lc0, gp.row_off + lrow0, true);
+            if (warp_ok && p.dbg != 2) stage_and_send(&p.m_gw, wbuf, c & 1, v, lane, gp.col_off + lc0, gp.row_off + lrow0, p.dbg != 1, p.hint);
         }
         drain_sends(lane);
     }

@@ -26,6 +26,9 @@ constexpr int GEMM_THREADS = 192;                     // warp0 TMA, warp1 MMA(+T
 constexpr int EPI_SMEM_BYTES = 32768;                 // 4 epilogue warps x 2 staging buffers x (32 rows x 128 B)
 constexpr int TMEM_COLS = 512;                        // 2 accumulator stages x 256 columns
 constexpr int MAX_STAGES = 6;
+#ifndef OPD_PAIR_STAGES
+#define OPD_PAIR_STAGES 6                  // TMA ring depth of the CTA-pair configuration (32 KiB per stage)
+#endif
 
 template <int CG>
 struct Cfg {
@@ -34,7 +37,7 @@ struct Cfg {
     static constexpr int A_STAGE_BYTES = BM * BK * 2;     // 16 KiB
     static constexpr int B_STAGE_BYTES = B_ROWS * BK * 2; // 32 / 16 KiB
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
-    static constexpr int STAGES = CG == 1 ? 4 : 6;
+    static constexpr int STAGES = CG == 1 ? 4 : OPD_PAIR_STAGES;
     static constexpr int RING_BYTES = STAGES * STAGE_BYTES;
     static constexpr int SMEM_BYTES = RING_BYTES + 1024 /*barriers*/ + EPI_SMEM_BYTES + 1024 /*align slack*/;
 };
@@ -55,6 +58,7 @@ struct GemmParams {
     int tok_off;
     const int* n_live;        // device scalar: number of live tokens (compacted rows)
     // per-launch / per-tile epilogue switches (set by the host for gemm_kernel, per tile by bwd_kernel)
+    unsigned long long a_hint, b_hint;   // L2 eviction policy of the operand loads (0 = normal)
     int first, last;          // DxEpi: first / last vocabulary super-tile of this token super-tile
     int row_off, col_off;     // DwEpi: position of this GEMM's output inside grad_W
 };
@@ -125,6 +129,7 @@ struct TileOp {
     int K;
     int nseg;
     unsigned char pa[MAX_SEG], pb[MAX_SEG];   // plane per segment
+    uint64_t a_hint, b_hint;  // L2 eviction policy of the operand loads
 };
 
 // TMA producer (one elected lane): stream all k-blocks of all segments of `t` through the ring.
@@ -145,14 +150,14 @@ __device__ __forceinline__ void produce_tile(const Pipe<CG>& P, const TileOp& t,
                 uint64_t* bar = &P.full_bar[s];
                 mbar_arrive_expect_tx(bar, C::STAGE_BYTES);
                 if (t.a_mn) {
-                    for (int b = 0; b < BM / MN_BOX; ++b) tma_load_3d(sA + b * MN_BOX_BYTES, t.tA, bar, t.a_c + b * MN_BOX, kca, pa);
+                    for (int b = 0; b < BM / MN_BOX; ++b) tma_load_3d(sA + b * MN_BOX_BYTES, t.tA, bar, t.a_c + b * MN_BOX, kca, pa, t.a_hint);
                 } else {
-                    tma_load_3d(sA, t.tA, bar, kca, t.a_c, pa);
+                    tma_load_3d(sA, t.tA, bar, kca, t.a_c, pa, t.a_hint);
                 }
                 if (t.b_mn) {
-                    for (int b = 0; b < C::B_ROWS / MN_BOX; ++b) tma_load_3d(sB + b * MN_BOX_BYTES, t.tB, bar, t.b_c + b * MN_BOX, kcb, pb);
+                    for (int b = 0; b < C::B_ROWS / MN_BOX; ++b) tma_load_3d(sB + b * MN_BOX_BYTES, t.tB, bar, t.b_c + b * MN_BOX, kcb, pb, t.b_hint);
                 } else {
-                    tma_load_3d(sB, t.tB, bar, kcb, t.b_c, pb);
+                    tma_load_3d(sB, t.tB, bar, kcb, t.b_c, pb, t.b_hint);
                 }
             } else {
                 // the leader's barrier counts the bytes of both CTAs (expect_tx may trail the peer's complete_tx:
@@ -160,14 +165,14 @@ __device__ __forceinline__ void produce_tile(const Pipe<CG>& P, const TileOp& t,
                 if (P.rank == 0) mbar_arrive_expect_tx(&P.full_bar[s], 2 * C::STAGE_BYTES);
                 const uint32_t bar = mapa_rank(smem_u32(&P.full_bar[s]), 0);
                 if (t.a_mn) {
-                    for (int b = 0; b < BM / MN_BOX; ++b) tma_load_3d_pair(sA + b * MN_BOX_BYTES, t.tA, bar, t.a_c + b * MN_BOX, kca, pa);
+                    for (int b = 0; b < BM / MN_BOX; ++b) tma_load_3d_pair(sA + b * MN_BOX_BYTES, t.tA, bar, t.a_c + b * MN_BOX, kca, pa, t.a_hint);
                 } else {
-                    tma_load_3d_pair(sA, t.tA, bar, kca, t.a_c, pa);
+                    tma_load_3d_pair(sA, t.tA, bar, kca, t.a_c, pa, t.a_hint);
                 }
                 if (t.b_mn) {
-                    for (int b = 0; b < C::B_ROWS / MN_BOX; ++b) tma_load_3d_pair(sB + b * MN_BOX_BYTES, t.tB, bar, t.b_c + b * MN_BOX, kcb, pb);
+                    for (int b = 0; b < C::B_ROWS / MN_BOX; ++b) tma_load_3d_pair(sB + b * MN_BOX_BYTES, t.tB, bar, t.b_c + b * MN_BOX, kcb, pb, t.b_hint);
                 } else {
-                    tma_load_3d_pair(sB, t.tB, bar, kcb, t.b_c, pb);
+                    tma_load_3d_pair(sB, t.tB, bar, kcb, t.b_c, pb, t.b_hint);
                 }
             }
         }
@@ -262,6 +267,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             TileOp t;
             t.tA = &tmA; t.tB = &tmB; t.a_mn = gp.a_mn; t.b_mn = gp.b_mn; t.ka = gp.ka_off; t.kb = gp.kb_off; t.K = K;
             t.nseg = gp.nseg;
+            t.a_hint = gp.a_hint ? gp.a_hint : L2_EVICT_NORMAL; t.b_hint = gp.b_hint ? gp.b_hint : L2_EVICT_NORMAL;
             for (int i = 0; i < MAX_SEG; ++i) { t.pa[i] = gp.sa[i]; t.pb[i] = gp.sb[i]; }
             int it = 0;
             for (int tile = first_tile; tile < total_tiles; tile += tile_step) {

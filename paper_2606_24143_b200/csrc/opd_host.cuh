@@ -100,6 +100,11 @@ inline int env_int(const char* name, int dflt) {
     return (s && *s) ? std::atoi(s) : dflt;
 }
 
+// 0 = normal, 1 = evict first, 2 = evict last
+inline unsigned long long hint_policy(int code) {
+    return code == 1 ? L2_EVICT_FIRST : (code == 2 ? L2_EVICT_LAST : L2_EVICT_NORMAL);
+}
+
 inline int cta_group_setting() {
     const int cg = env_int("OPD_CTA_GROUP", 2);
     return cg == 1 ? 1 : 2;

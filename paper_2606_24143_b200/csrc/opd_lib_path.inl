@@ -140,6 +140,9 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         ok &= make_map_f32(&dwp.m_gw, a.grad_W, wl == 0 ? V : d, wl == 0 ? d : V, (uint64_t)ldgw * 4);
         dxp.acc = dxacc; dxp.ld_acc = d; dxp.out = a.grad_hidden; dxp.ld_out = a.ld_gh; dxp.out_fp32 = fp32 ? 1 : 0;
         dxp.live_rows = live_rows;
+        dxp.hint = hint_policy(env_int("OPD_HINT_DX", 0));
+        dwp.hint = hint_policy(env_int("OPD_HINT_GW", 0));
+        dxp.dbg = dwp.dbg = env_int("OPD_DBG_ACC", 0);
     }
     if (!ok) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled failed");
 
@@ -151,6 +154,7 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         gp.group_m = std::max(1, env_int("OPD_GROUP_M", 16));
         gp.a_mn = 0; gp.b_mn = (wl == 0); gp.a_off = 0; gp.b_off = 0; gp.ka_off = 0; gp.kb_off = 0;
         set_segments(gp, p.planes);
+        gp.a_hint = hint_policy(env_int("OPD_HINT_FX", 0)); gp.b_hint = hint_policy(env_int("OPD_HINT_FW", 0));
         gp.tok_dim = TOK_M; gp.tok_off = 0; gp.n_live = n_live;
         FwdEpi::Params ep{partials, p.t_pad, sorted_idx, zc, C, V, a.dbg_logits};
         OPD_CUDA(h, launch_gemm<FwdEpi>(h, st, m_xc_k, m_w_fwd, gp, ep));
@@ -194,6 +198,9 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         bp.g = GEpi::Params{gs, p.Tb, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V};
         bp.dx = dxp;
         bp.dw = dwp;
+        bp.hint_x = hint_policy(env_int("OPD_HINT_X", 0)); bp.hint_w = hint_policy(env_int("OPD_HINT_W", 0));
+        bp.hint_g = hint_policy(env_int("OPD_HINT_G", 0));
+        bp.type_mask = env_int("OPD_BWD_TYPES", 7) & 7;
         // every CTA (pair) must be resident at once: items wait on earlier items of other CTAs
         const int grid = h->num_sms / h->cg * h->cg;
         if (h->cg == 2) OPD_CUDA(h, launch_cg<2>(bwd_kernel<2>, grid, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, bp));
