@@ -11,6 +11,9 @@
  *                   (Eq.(15)) with the advantage recomputed at learner
  *                   time A = log q - log p_theta and the unclipped ratio rho = p_theta / p_old
  *                   (Finding 2 PAPER.md:153)
+ *     OPD_RKL_TOPK  sparse top-k reverse KL on a cached (stale) support, KL(p~ || q~) with both distributions
+ *                   renormalised on S and S fixed during the update (App. A.1 Eq.(8)-(10));
+ *                   the baseline the paper compares multi-sample MC against. Purely sparse gradient.
  *   loss = (1/N) sum over live tokens; and the backward into grad_hidden and grad_W, for which the
  *   softmax tiles are re-formed (never read back from memory).
  *
@@ -46,7 +49,7 @@ typedef enum {
     OPD_ERR_CUDA = -6        /* a CUDA runtime/driver call failed; see opd_last_error */
 } opd_status_t;
 
-typedef enum { OPD_FKL_TOPK = 0, OPD_RKL_MC = 1, OPD_MIXED = 2 } opd_mode_t;
+typedef enum { OPD_FKL_TOPK = 0, OPD_RKL_MC = 1, OPD_MIXED = 2, OPD_RKL_TOPK = 3 } opd_mode_t;
 typedef enum { OPD_BF16 = 0, OPD_FP32 = 1 } opd_dtype_t;
 
 enum {
@@ -80,7 +83,7 @@ opd_status_t opd_set_workspace(opd_handle_t h, void* ws, size_t bytes);
  * W        logical W(k,v), k in [0,d), v in [0,V): element (k,v) at W[k*ldw_k + v*ldw_v]; exactly one of
  *          the strides is 1 ([d,V] row-major: ldw_v = 1;  [V,d] row-major lm_head.weight: ldw_k = 1).
  * cache_idx [T,C] int32 in [0,V) (row stride ld_cache, also used for the two float caches);
- * cache_teacher_logp [T,C] log q(a|s); cache_old_logp [T,C] log p_old(a|s) (may be NULL for OPD_FKL_TOPK).
+ * cache_teacher_logp [T,C] log q(a|s); cache_old_logp [T,C] log p_old(a|s) (may be NULL for OPD_FKL_TOPK / OPD_RKL_TOPK).
  * mask     [T] bytes: 0 = masked (row contributes nothing, its cache row is never read).
  *          OPD_MIXED: 1 = FKL_TOPK row, 2 = RKL_MC row; one token-mean over all live rows.
  * k_or_K   cache width C (1..64). OPD_MIXED: k | (K << 16); FKL rows use the first k slots, MC rows the
@@ -123,6 +126,16 @@ opd_status_t opd_loss_fwd_bwd_host(opd_handle_t h,
     opd_mode_t mode, int k_or_K, unsigned flags, float norm_override,
     float* loss_host, float* per_token_kl_host, void* grad_hidden_host, void* grad_W_host,
     size_t* h2d_bytes, size_t* d2h_bytes);
+
+/* Optional per-token diagnostics of the MC estimator, written by the following opd_loss_fwd_bwd calls on this
+ * handle (device pointers, caller-owned; pass NULLs to switch off):
+ *   rho_out [T, ld_rho]  rho_theta(a_tj) = p_theta(a_tj|s_t) / p_old(a_tj|s_t) of every cached draw of a live RKL_MC row
+ *                        (caller slot order; other entries untouched) — the quantity whose p99 tail Fig. 5 reports
+ *                        (PAPER.md:149-151);
+ *   var1_out [T]         unbiased sample variance over the m cached draws of the one-sample estimates
+ *                        -rho_j A_theta,j, i.e. the within-prefix Var(L^MC_1 | s_t) of Eq.(16);
+ *                        0 on masked / non-MC rows and when m = 1. */
+opd_status_t opd_set_diagnostics(opd_handle_t h, float* rho_out, long ld_rho, float* var1_out);
 
 /* debugging / verification aids ----------------------------------------------------------------
  * opd_debug_logits: runs the forward contraction kernel only and dumps the fp32 logit tiles it held in

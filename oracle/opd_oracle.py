@@ -22,6 +22,9 @@ What it computes, in the paper's order and notation (PAPER.md = /root/reference/
           A_j   = lam_j - l_j                 (A_theta recomputed at learner time)
           rho_j = exp(l_j - o_j)              (unclipped old->current ratio)
           L_t   = -(1/m) sum_j rho_j A_j
+  O5b RKL_TOPK (App. A.1 Eq.(8)-(10); the cached support S is fixed)
+          p~_j = exp(l_j - log sum_S exp l),  q~_j = exp(lam_j - log sum_S exp lam)
+          L_t  = sum_j p~_j (log p~_j - log q~_j);   g = sum_j p~_j (log p~_j - log q~_j - L_t) e_{a_j}
   O6  N = sum_t [mask_t != 0] (or norm_override), loss = (1/N) sum_t L_t, per_token_kl = L_t (0 if masked)
   O7  g_tv = dL_t/dz_tv with A frozen (stop-gradient):
           FKL:                g = (sum_j q~_j) p - sum_j q~_j e_{a_j}
@@ -52,6 +55,7 @@ import numpy as np
 FKL_TOPK = 0
 RKL_MC = 1
 MIXED = 2
+RKL_TOPK = 3          # sparse top-k reverse KL on the cached support, App. A.1 Eq.(8)-(10)
 
 F_NO_RENORM_TEACHER = 1
 F_RENORM_STUDENT = 2
@@ -144,7 +148,12 @@ def token_terms(mode: int, lam: np.ndarray, old, ell: np.ndarray, flags: int,
         alpha = c
         beta = -w / m
         return L, alpha, beta
-    raise ValueError("mode must be FKL_TOPK or RKL_MC per token")
+    if mode == RKL_TOPK:
+        # Eq.(10) on the cached support, both distributions renormalised on S (Eq.(9)); the support is fixed during
+        # the update, so dD/dz_v = sum_j dD/dl_j [a_j = v] and the full-vocabulary lse cancels.
+        D, dD = sparse_reverse_kl(lam, ell)
+        return D, 0.0, dD
+    raise ValueError("mode must be FKL_TOPK, RKL_MC or RKL_TOPK per token")
 
 
 def _split_k(mode: int, k_or_K: int):
@@ -187,6 +196,8 @@ def opd_oracle(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, m
     lse_out = np.zeros(T)
     alpha_out = np.zeros(T)
     slp = np.full(idx.shape, np.nan)
+    rho_out = np.full(idx.shape, np.nan)       # diagnostics: rho_theta(a_tj) on MC rows (Fig. 5)
+    var1_out = np.zeros(T)                     # diagnostics: sample variance of the one-sample terms (Eq.(16))
     gh = np.zeros((T, d)) if want_grads else None
     gW = np.zeros((d, V)) if (want_grads and want_grad_W) else None
 
@@ -211,6 +222,8 @@ def opd_oracle(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, m
             lse_out[t] = lse[i]
             alpha_out[t] = alpha
             slp[t, :C] = ell
+            if tmode == RKL_MC:
+                rho_out[t, :C], var1_out[t] = mc_diagnostics(lam_all[t, :C], old, ell)
             if want_grads:
                 g = alpha * p[i]                           # O7 dense part
                 np.add.at(g, a, beta)                      # O7 sparse part (duplicates add)
@@ -221,7 +234,7 @@ def opd_oracle(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, m
                 gW += X[tt].T @ G                          # O9
     loss = float(np.sum(per_token)) * scale                # O6
     return dict(loss=loss, N=N, per_token_kl=per_token, lse=lse_out, student_logp=slp,
-                alpha=alpha_out, grad_hidden=gh, grad_W=gW)
+                alpha=alpha_out, grad_hidden=gh, grad_W=gW, rho=rho_out, var1=var1_out)
 
 
 def grad_W_columns(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K,
@@ -328,6 +341,19 @@ def opd_oracle_loops(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, m
     loss = scale * sum(per_token)
     return dict(loss=loss, N=float(N), per_token_kl=np.array(per_token), grad_hidden=np.array(gh),
                 grad_W=np.array(gW))
+
+
+def mc_diagnostics(lam, old, ell):
+    """Per-token diagnostics of the MC estimator: the importance ratios rho_j = p_theta(a_j)/p_old(a_j) whose tail
+    Fig. 5 reports, and the unbiased sample variance over the m cached draws of the one-sample
+    estimates X_j = -rho_j A_theta,j, i.e. the within-prefix Var(L^MC_1 | s_t) of Eq.(16) (PAPER.md:384-386);
+    Var(L^MC_m | s_t) = Var(L^MC_1 | s_t) / m for iid draws. 0 when m = 1."""
+    lam = np.asarray(lam, dtype=np.float64); old = np.asarray(old, dtype=np.float64); ell = np.asarray(ell, dtype=np.float64)
+    rho = np.exp(ell - old)
+    X = -rho * (lam - ell)
+    m = X.shape[0]
+    var1 = float(np.sum((X - X.mean()) ** 2) / (m - 1)) if m > 1 else 0.0
+    return rho, var1
 
 
 def sparse_reverse_kl(lam: np.ndarray, ell: np.ndarray):

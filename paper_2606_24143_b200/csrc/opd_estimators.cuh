@@ -2,6 +2,7 @@
 //   FKL_TOPK  PAPER.md:57 Eq.(1) on the cached support, renormalisers Eq.(9)
 //   RKL_MC    PAPER.md:191, Eq.(15); A_theta recomputed at learner time, rho unclipped
 //             (PAPER.md:126-130); optional PPO clip / A_old variants of Eq.(6),(7) PAPER.md:132-141
+//   RKL_TOPK  sparse top-k reverse KL on the cached support, App. A.1 Eq.(8)-(10) PAPER.md:289-303
 // Output of S4 for the backward: dL_t/dz_v = alpha_t p_v + sum_j beta_tj [a_tj = v]  (both scaled by 1/N).
 #pragma once
 #include "opd_small_kernels.cuh"
@@ -21,6 +22,7 @@ struct EstParams {
     // outputs
     float* lse2; float* coef; float* beta;               // compact-row order ([T], [T], [T][C])
     float* per_token_kl; float* lse_out; float* slp_out; // caller order; lse_out / slp_out may be null
+    float* rho_out; long ld_rho; float* var1_out;        // optional diagnostics (opd_set_diagnostics), caller order
     double* block_sums;                                  // [gridDim.x]
 };
 
@@ -77,9 +79,28 @@ __global__ void __launch_bounds__(128) k_estimator(const EstParams p) {
                 if (p.slp_out) p.slp_out[static_cast<size_t>(tok) * p.ld_cache + pm[s]] = ell;
             }
             alpha = (p.flags & FL_RENORM_STUDENT) ? 0.f : sq;
+        } else if (tmode == MODE_RKL_TOPK) {
+            // App. A.1 Eq.(8)-(10) PAPER.md:289-303: KL(p~ || q~), both renormalised on the cached (fixed) support;
+            // the full-vocabulary lse cancels and the gradient is purely sparse (alpha = 0).
+            float mq = -INFINITY, mp = -INFINITY;
+            for (int s = 0; s < Cr; ++s) { mq = fmaxf(mq, lam[pm[s]]); mp = fmaxf(mp, zc[s]); }
+            float zq = 0.f, zp = 0.f;
+            for (int s = 0; s < Cr; ++s) { zq += expf(lam[pm[s]] - mq); zp += expf(zc[s] - mp); }
+            const float logZq = mq + logf(zq), logZp = mp + logf(zp);
+            for (int s = 0; s < Cr; ++s) {
+                const float lp = zc[s] - logZp, lq = lam[pm[s]] - logZq;
+                L += expf(lp) * (lp - lq);
+            }
+            for (int s = 0; s < Cr; ++s) {
+                const float lp = zc[s] - logZp, lq = lam[pm[s]] - logZq;
+                beta[s] = rs * expf(lp) * (lp - lq - L);
+                if (p.slp_out) p.slp_out[static_cast<size_t>(tok) * p.ld_cache + pm[s]] = zc[s] - lse;
+            }
+            alpha = 0.f;
         } else {
             const float invm = 1.f / static_cast<float>(Cr);
             float sum_term = 0.f, sum_w = 0.f;
+            float sx = 0.f, sxx = 0.f;                      // one-sample estimates X_j = -rho_j A_theta,j (Eq.(16))
             for (int s = 0; s < Cr; ++s) {
                 const float ell = zc[s] - lse;
                 const float o = old[pm[s]];
@@ -87,6 +108,8 @@ __global__ void __launch_bounds__(128) k_estimator(const EstParams p) {
                 const float rho = expf(ell - o);
                 const float A = (p.flags & FL_SUR_A_OLD) ? (lm - o) : (lm - ell);
                 float term = rho * A, w = rho * A;
+                if (p.rho_out) p.rho_out[static_cast<size_t>(tok) * p.ld_rho + pm[s]] = rho;
+                { const float x = -rho * (lm - ell); sx += x; sxx += x * x; }
                 if (p.flags & FL_SUR_CLIP) {
                     const float rbar = fminf(fmaxf(rho, 1.f - CLIP_EPS), 1.f + CLIP_EPS);
                     const float cl = rbar * A;
@@ -101,6 +124,7 @@ __global__ void __launch_bounds__(128) k_estimator(const EstParams p) {
             }
             L = -sum_term * invm;
             alpha = sum_w * invm;
+            if (p.var1_out) p.var1_out[tok] = Cr > 1 ? fmaxf(0.f, (sxx - sx * sx * invm) / static_cast<float>(Cr - 1)) : 0.f;
         }
         for (int s = Cr; s < p.C; ++s) beta[s] = 0.f;
         p.lse2[i] = lse * LOG2E;

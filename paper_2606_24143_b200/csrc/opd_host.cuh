@@ -29,6 +29,7 @@ struct opd_handle_s {
     // stats of the last call
     int n_kernels = 0, n_gemm = 0, super_rows = 0, super_cols = 0;
     cudaEvent_t* phase_events = nullptr;
+    float* diag_rho = nullptr; long diag_ld_rho = 0; float* diag_var1 = nullptr;   // opd_set_diagnostics
 };
 
 namespace opd {

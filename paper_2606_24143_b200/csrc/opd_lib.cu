@@ -100,5 +100,12 @@ extern "C" opd_status_t opd_set_phase_events(opd_handle_t h, void** events) {
     return OPD_OK;
 }
 
+extern "C" opd_status_t opd_set_diagnostics(opd_handle_t h, float* rho_out, long ld_rho, float* var1_out) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    if (rho_out && ld_rho < 1) OPD_FAIL(h, OPD_ERR_BAD_ARG, "ld_rho must be >= the cache width");
+    h->diag_rho = rho_out; h->diag_ld_rho = ld_rho; h->diag_var1 = var1_out;
+    return OPD_OK;
+}
+
 #include "opd_lib_path.inl"
 #include "opd_lib_extra.inl"

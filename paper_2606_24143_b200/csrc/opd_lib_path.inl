@@ -25,7 +25,7 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     const int T = a.T, d = a.d, V = a.V;
     int kf, Km;
     const int C = cache_width(a.mode, a.k_or_K, &kf, &Km);
-    if (a.mode != OPD_FKL_TOPK && a.mode != OPD_RKL_MC && a.mode != OPD_MIXED) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unknown mode %d", (int)a.mode);
+    if (a.mode != OPD_FKL_TOPK && a.mode != OPD_RKL_MC && a.mode != OPD_MIXED && a.mode != OPD_RKL_TOPK) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unknown mode %d", (int)a.mode);
     if (a.dtype != OPD_BF16 && a.dtype != OPD_FP32) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unknown dtype %d", (int)a.dtype);
     opd_status_t s = check_shape(h, T, d, V, C);
     if (s != OPD_OK) return s;
@@ -39,7 +39,7 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     if (!a.hidden || !a.W || !a.cache_idx || (!a.stop_after_fwd && (!a.lam || !a.loss || !a.per_token_kl)))
         OPD_FAIL(h, OPD_ERR_BAD_ARG, "null input/output pointer");
     if (!a.all_live && !a.mask) OPD_FAIL(h, OPD_ERR_BAD_ARG, "mask is null");
-    if (a.mode != OPD_FKL_TOPK && !a.old && !a.stop_after_fwd) OPD_FAIL(h, OPD_ERR_BAD_ARG, "cache_old_logp is required for RKL_MC / MIXED");
+    if ((a.mode == OPD_RKL_MC || a.mode == OPD_MIXED) && !a.old && !a.stop_after_fwd) OPD_FAIL(h, OPD_ERR_BAD_ARG, "cache_old_logp is required for RKL_MC / MIXED");
     if (!fwd_only && (!a.grad_hidden || !a.grad_W)) OPD_FAIL(h, OPD_ERR_BAD_ARG, "grad pointers are null (use OPD_F_FWD_ONLY)");
     const int wl = (a.ldw_v == 1) ? 0 : ((a.ldw_k == 1) ? 1 : -1);       // 0: [d,V] row-major, 1: [V,d] row-major
     if (wl < 0) OPD_FAIL(h, OPD_ERR_BAD_ARG, "one of ldw_k / ldw_v must be 1");
@@ -178,6 +178,8 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         e.mode = (int)a.mode; e.k_fkl = kf; e.K_mc = Km; e.C = C; e.flags = a.flags; e.norm_override = a.norm_override;
         e.lse2 = lse2; e.coef = coef; e.beta = beta; e.per_token_kl = a.per_token_kl; e.lse_out = a.lse_out; e.slp_out = a.slp_out;
         e.block_sums = block_sums;
+        e.rho_out = h->diag_rho; e.ld_rho = h->diag_ld_rho; e.var1_out = h->diag_var1;
+        if (h->diag_var1) OPD_CUDA(h, cudaMemsetAsync(h->diag_var1, 0, sizeof(float) * T, st));
         k_estimator<<<p.est_blocks, 128, 0, st>>>(e);
         k_loss_final<<<1, 256, 0, st>>>(block_sums, p.est_blocks, n_live, a.norm_override, a.loss);
         h->n_kernels += 2;

@@ -8,7 +8,7 @@
 namespace opd {
 
 // flags / modes restated from include/opd.h (kept numerically identical there)
-constexpr int MODE_FKL = 0, MODE_MC = 1, MODE_MIXED = 2;
+constexpr int MODE_FKL = 0, MODE_MC = 1, MODE_MIXED = 2, MODE_RKL_TOPK = 3;
 constexpr unsigned FL_NO_RENORM_TEACHER = 1, FL_RENORM_STUDENT = 2, FL_SUR_CLIP = 64, FL_SUR_A_OLD = 128;
 constexpr float CLIP_EPS = 0.2f;
 

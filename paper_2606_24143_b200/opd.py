@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libopd.so")
 
 OPD_OK = 0
 ERR_BAD_ARG, ERR_BAD_SHAPE, ERR_BAD_INDEX, ERR_WORKSPACE, ERR_ARCH, ERR_CUDA = -1, -2, -3, -4, -5, -6
-FKL_TOPK, RKL_MC, MIXED = 0, 1, 2
+FKL_TOPK, RKL_MC, MIXED, RKL_TOPK = 0, 1, 2, 3
 BF16, FP32 = 0, 1
 F_NO_RENORM_TEACHER, F_RENORM_STUDENT, F_GRADW_ACCUM, F_VALIDATE_IDX, F_FWD_ONLY = 1, 2, 4, 16, 32
 F_SUR_CLIP, F_SUR_A_OLD = 64, 128
@@ -25,7 +25,7 @@ PHASE_NAMES = ("prep", "fwd", "est", "bwd")
 
 EXPORTS = ("opd_create", "opd_destroy", "opd_last_error", "opd_version", "opd_workspace_bytes", "opd_set_workspace",
            "opd_loss_fwd_bwd", "opd_loss_fwd_bwd_host", "opd_debug_logits", "opd_debug_gemm", "opd_last_launch_stats",
-           "opd_set_phase_events")
+           "opd_set_phase_events", "opd_set_diagnostics")
 
 _lib = None
 
@@ -71,6 +71,8 @@ def load_library():
     lib.opd_debug_gemm.restype = c_int
     lib.opd_last_launch_stats.argtypes = [c_void_p, POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(c_int)]
     lib.opd_last_launch_stats.restype = c_int
+    lib.opd_set_diagnostics.argtypes = [c_void_p, c_void_p, c_long, c_void_p]
+    lib.opd_set_diagnostics.restype = c_int
     lib.opd_set_phase_events.argtypes = [c_void_p, c_void_p]
     lib.opd_set_phase_events.restype = c_int
     _lib = lib
@@ -132,6 +134,12 @@ class Handle:
         a, b, c, e = c_int(), c_int(), c_int(), c_int()
         self.lib.opd_last_launch_stats(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c), ctypes.byref(e))
         return dict(kernels=a.value, gemm_kernels=b.value, super_rows=c.value, super_cols=e.value)
+
+    def set_diagnostics(self, rho_out=None, var1_out=None):
+        """opd_set_diagnostics: rho_out [T,C] / var1_out [T] float32 device tensors written by the following calls."""
+        self._diag = (rho_out, var1_out)          # keep the tensors alive
+        self._check(self.lib.opd_set_diagnostics(self._h, _ptr(rho_out), rho_out.stride(0) if rho_out is not None else 0,
+                                                 _ptr(var1_out)))
 
     # ------------------------------------------------------------------ phase timing
     def enable_phase_timing(self, on: bool = True):

@@ -16,6 +16,7 @@ Recipe (shapes from BASELINE.json configs):
   MC draws       (i=5)   a_j ~ Categorical(p_old) iid WITH replacement, K per token
   top-k cache    idx = TopK(log q, k) chosen by the teacher, lam = log q[idx]
   MC cache       idx = a, lam = log q[a], old = log p_old[a]
+  stale top-k    idx = TopK(log p_old, k) (the rollout-time student support S_old), lam = log q[idx]
 All cache values are fp32, indices int32.  Rollout settings follow PAPER.md:332 (temperature 1,
 no truncation).  These are stand-ins for the paper's Qwen3 workloads: V=151936 and
 d in {2048,2560,4096} are the 1.7B/4B/8B-class student heads.
@@ -83,6 +84,7 @@ def make_inputs(cfg: dict, c: int = 0, device="cpu", keep_teacher_rows: bool = F
     hidden [T,d], W [d,V] (cfg dtype); mask [T] u8;
     topk_idx [T,k] i32, topk_logq [T,k] f32            (teacher-selected support + its log-probs)
     mc_idx [T,K] i32, mc_logq [T,K] f32, mc_logp_old [T,K] f32
+    stopk_idx [T,k] i32, stopk_logq [T,k] f32         (stale student's top-k support S_old + teacher log-probs on it)
     and, if keep_teacher_rows, logq [T,V] / logp_old [T,V] f32 (small configs, for oracle pins).
     """
     T, d, V, k, K = cfg["T"], cfg["d"], cfg["V"], cfg["k"], cfg["K"]
@@ -105,6 +107,8 @@ def make_inputs(cfg: dict, c: int = 0, device="cpu", keep_teacher_rows: bool = F
 
     topk_idx = torch.empty(T, k, dtype=torch.int32, device=dev)
     topk_logq = torch.empty(T, k, dtype=torch.float32, device=dev)
+    stopk_idx = torch.empty(T, k, dtype=torch.int32, device=dev)
+    stopk_logq = torch.empty(T, k, dtype=torch.float32, device=dev)
     mc_idx = torch.empty(T, K, dtype=torch.int32, device=dev)
     mc_logq = torch.empty(T, K, dtype=torch.float32, device=dev)
     mc_old = torch.empty(T, K, dtype=torch.float32, device=dev)
@@ -119,6 +123,9 @@ def make_inputs(cfg: dict, c: int = 0, device="cpu", keep_teacher_rows: bool = F
         tv, ti = torch.topk(logq, k, dim=-1)               # descending
         topk_idx[r0:r1] = ti.to(torch.int32)
         topk_logq[r0:r1] = tv
+        si = torch.topk(logpo, k, dim=-1).indices            # stale student's support S_old = TopK(p_old, k)
+        stopk_idx[r0:r1] = si.to(torch.int32)
+        stopk_logq[r0:r1] = torch.gather(logq, 1, si)
         a = torch.multinomial(torch.exp(logpo), K, replacement=True, generator=g5)
         mc_idx[r0:r1] = a.to(torch.int32)
         mc_logq[r0:r1] = torch.gather(logq, 1, a)
@@ -127,7 +134,8 @@ def make_inputs(cfg: dict, c: int = 0, device="cpu", keep_teacher_rows: bool = F
             logq_all[r0:r1] = logq
             logpold_all[r0:r1] = logpo
     out = dict(hidden=hidden, W=W, mask=make_mask(cfg, c, dev), topk_idx=topk_idx, topk_logq=topk_logq,
-               mc_idx=mc_idx, mc_logq=mc_logq, mc_logp_old=mc_old, cfg=dict(cfg), sigma=sig)
+               mc_idx=mc_idx, mc_logq=mc_logq, mc_logp_old=mc_old, stopk_idx=stopk_idx, stopk_logq=stopk_logq,
+               cfg=dict(cfg), sigma=sig)
     if keep_teacher_rows:
         out["logq"] = logq_all
         out["logp_old"] = logpold_all

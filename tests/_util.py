@@ -30,6 +30,8 @@ def pick(inp, cfg, mode):
         return inp["topk_idx"], inp["topk_logq"], None, cfg["k"]
     if mode == O.RKL_MC:
         return inp["mc_idx"], inp["mc_logq"], inp["mc_logp_old"], cfg["K"]
+    if mode == O.RKL_TOPK:      # teacher scores cached on the STALE student's top-k support S_old
+        return inp["stopk_idx"], inp["stopk_logq"], None, cfg["k"]
     return synth.mixed_cache(inp)
 
 

@@ -346,3 +346,65 @@ def test_sparse_reverse_kl_definition_and_gradient():
         e = np.zeros(5); e[j] = 1e-6
         fd = (O.sparse_reverse_kl(lam, ell + e)[0] - O.sparse_reverse_kl(lam, ell - e)[0]) / 2e-6
         assert abs(fd - g[j]) < 1e-9
+
+
+def _rkl_topk_loss(t, X, W, C, mask):
+    """Eq.(10) PAPER.md:297-301 from scratch: token mean of KL(p~^S || q~^S) on the fixed cached support."""
+    logp, _ = O.log_softmax_rows(X @ W)
+    tot = 0.0
+    for ti in range(X.shape[0]):
+        if mask[ti] == 0:
+            continue
+        a = t["idx"][ti, :C]
+        pt = np.exp(logp[ti, a]); pt = pt / pt.sum()
+        qt = np.exp(t["lam"][ti, :C]); qt = qt / qt.sum()
+        tot += float((pt * (np.log(pt) - np.log(qt))).sum())
+    return tot / np.count_nonzero(mask)
+
+
+def test_rkl_topk_end_to_end():
+    """OPD_RKL_TOPK through opd_oracle: S = V equals dense D_R (Eq.(2)); loss and gradients against central
+    differences of an independently written Eq.(10); non-negative; invariant to a per-token teacher constant."""
+    t = tiny(23, T=4, d=6, V=12, C=4, mask=[1, 0, 1, 1])
+    full = np.tile(np.arange(12), (4, 1))
+    r = O.opd_oracle(t["X"], t["W"], full, t["logq"], None, t["mask"], O.RKL_TOPK, 12)
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    live = t["mask"] != 0
+    assert np.abs(r["per_token_kl"][live] - O.dense_reverse_kl(t["logq"], logp)[live]).max() < 1e-13
+    r = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], None, t["mask"], O.RKL_TOPK, 4)
+    f = lambda X, W: _rkl_topk_loss(t, X, W, 4, t["mask"])
+    assert abs(r["loss"] - f(t["X"], t["W"])) < 1e-14 and np.all(r["per_token_kl"] >= 0)
+    h = 1e-6
+    rng = np.random.default_rng(1)
+    probes = [(int(rng.integers(4)), int(rng.integers(6)), int(rng.integers(12))) for _ in range(10)]
+    probes += [(ti, 2, int(t["idx"][ti, j])) for ti in (0, 2, 3) for j in range(4)]
+    for ti, ki, vi in probes:
+        Xp, Xm = t["X"].copy(), t["X"].copy(); Xp[ti, ki] += h; Xm[ti, ki] -= h
+        assert abs((f(Xp, t["W"]) - f(Xm, t["W"])) / (2 * h) - r["grad_hidden"][ti, ki]) < 2e-8
+        Wp, Wm = t["W"].copy(), t["W"].copy(); Wp[ki, vi] += h; Wm[ki, vi] -= h
+        assert abs((f(t["X"], Wp) - f(t["X"], Wm)) / (2 * h) - r["grad_W"][ki, vi]) < 2e-8
+    assert np.all(r["grad_hidden"][1] == 0)
+    r2 = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"] + 1.7, None, t["mask"], O.RKL_TOPK, 4)
+    assert abs(r2["loss"] - r["loss"]) < 1e-14
+    # columns outside the support get no gradient (purely sparse backward)
+    outside = np.setdiff1d(np.arange(12), np.unique(t["idx"][live]))
+    assert np.all(r["grad_W"][:, outside] == 0)
+
+
+def test_mc_diagnostics():
+    """rho == 1 on-policy (W_old = W); var1 is numpy's unbiased variance of the one-sample estimates
+    written out from Eq.(15); the m-sample estimate is their mean, so its within-prefix variance is var1 / m."""
+    t = tiny(31, T=3, d=5, V=9, C=4, dup=True)
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    on = np.take_along_axis(logp, t["idx"], 1)
+    r = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], on, t["mask"], O.RKL_MC, 4)
+    assert np.abs(r["rho"] - 1).max() < 1e-14
+    r = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], O.RKL_MC, 4)
+    for ti in range(3):
+        ell = logp[ti, t["idx"][ti]]
+        x = [-math.exp(ell[j] - t["old"][ti, j]) * (t["lam"][ti, j] - ell[j]) for j in range(4)]
+        assert abs(r["var1"][ti] - np.var(x, ddof=1)) < 1e-13
+        assert abs(r["per_token_kl"][ti] - np.mean(x)) < 1e-14
+        assert np.abs(r["rho"][ti] - np.exp(ell - t["old"][ti])).max() < 1e-14
+    r1 = O.opd_oracle(t["X"], t["W"], t["idx"][:, :1], t["lam"][:, :1], t["old"][:, :1], t["mask"], O.RKL_MC, 1)
+    assert np.all(r1["var1"] == 0)

@@ -74,7 +74,7 @@ def test_gathers_are_bit_exact(handle, dtype, layout):
     (O.FKL_TOPK, 0, "dv"), (O.FKL_TOPK, 0, "vd"), (O.RKL_MC, 0, "dv"), (O.RKL_MC, 0, "vd"),
     (O.FKL_TOPK, O.F_RENORM_STUDENT, "dv"), (O.FKL_TOPK, O.F_NO_RENORM_TEACHER, "dv"),
     (O.FKL_TOPK, O.F_NO_RENORM_TEACHER | O.F_RENORM_STUDENT, "vd"),
-    (O.RKL_MC, 64, "dv"), (O.RKL_MC, 128, "dv"), (O.RKL_MC, 64 | 128, "dv")])
+    (O.RKL_MC, 64, "dv"), (O.RKL_MC, 128, "dv"), (O.RKL_MC, 64 | 128, "dv"), (O.RKL_TOPK, 0, "dv"), (O.RKL_TOPK, 0, "vd")])
 def test_C1_fp32(handle, mode, flags, layout):
     """BASELINE.json configs[0]: fp32, T=256, d=256, V=4096, k=8 / K=4, sigma=0.05, 10% masked."""
     cfg = synth.CONFIGS[1]
@@ -84,7 +84,7 @@ def test_C1_fp32(handle, mode, flags, layout):
     compare_all(r, oracle_for(inp, idx, lam, old, mode, kk, flags), f64(inp["mask"]), "fp32")
 
 
-@pytest.mark.parametrize("mode", [O.FKL_TOPK, O.RKL_MC])
+@pytest.mark.parametrize("mode", [O.FKL_TOPK, O.RKL_MC, O.RKL_TOPK])
 def test_C2_bf16(handle, mode):
     """BASELINE.json configs[1]: bf16, T=4096, d=1024, V=32768, k=16 / K=4, sigma=0.02 (full oracle)."""
     cfg = synth.CONFIGS[2]
@@ -98,7 +98,7 @@ RAGGED = dict(dtype="bf16", T=700, d=320, V=2056, k=8, K=5, sigma=0.05, mask="ra
 
 
 @pytest.mark.parametrize("dtype", ["bf16", "fp32"])
-@pytest.mark.parametrize("mode", [O.FKL_TOPK, O.RKL_MC, O.MIXED])
+@pytest.mark.parametrize("mode", [O.FKL_TOPK, O.RKL_MC, O.MIXED, O.RKL_TOPK])
 @pytest.mark.parametrize("tiles", [None, (256, 512)])
 def test_ragged_shapes_and_super_tiles(handle, dtype, mode, tiles, monkeypatch):
     """T, V not multiples of the tile sizes, d not a multiple of 256; several backward super-tiles in both
@@ -205,3 +205,30 @@ def test_no_logits_sized_workspace(handle, opd):
         C = max(cfg["k"], cfg["K"])
         ws = handle.workspace_bytes(cfg["T"], cfg["d"], cfg["V"], C, opd.BF16, opd.RKL_MC, 0)
         assert ws < 0.05 * cfg["T"] * cfg["V"] * 2, (c, ws)
+
+
+def test_mc_diagnostics_outputs(handle, opd):
+    """opd_set_diagnostics: rho_theta per cached draw and the one-sample variance of Eq.(16) against the oracle;
+    rows that are masked or not RKL_MC are left untouched / zero."""
+    cfg = dict(RAGGED, K=6)
+    inp = synth.make_inputs(cfg, c=11, device=DEV)
+    m = inp["mask"].clone()
+    m[(torch.arange(cfg["T"], device=DEV) % 2 == 0) & (m != 0)] = 2
+    inp["mask"] = m
+    idx, lam, old, kk = synth.mixed_cache(inp)
+    rho = torch.full(idx.shape, -7.0, device=DEV)
+    var1 = torch.full((cfg["T"],), -7.0, device=DEV)
+    handle.set_diagnostics(rho, var1)
+    try:
+        handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, m, O.MIXED, kk)
+        torch.cuda.synchronize()
+    finally:
+        handle.set_diagnostics(None, None)
+    ref = oracle_for(inp, idx, lam, old, O.MIXED, kk)
+    used = ~np.isnan(ref["rho"])
+    got = f64(rho)
+    assert np.abs(got[used] / ref["rho"][used] - 1).max() <= 2e-4
+    assert np.all(got[~used] == -7.0)
+    v = f64(var1)
+    assert np.abs(v - ref["var1"]).max() <= 1e-3 * max(1e-30, np.abs(ref["var1"]).max())
+    assert np.all(v[f64(m) != 2] == 0)
