@@ -370,3 +370,36 @@ def sparse_reverse_kl(lam: np.ndarray, ell: np.ndarray):
     pt = np.exp(lp)
     D = float(np.sum(pt * (lp - lq)))
     return D, pt * (lp - lq - D)
+
+
+# ------------------------------------------------------------------------------------------------
+# Cache producers: what the scoring / rollout side computes before the learner path.
+def cache_topk(hidden, W, k: int):
+    """Top-k cache of the scoring model (teacher scores are kept on a finite support; Fig. 1: forward KL is
+    teacher-supported):  S_t = TopK(softmax(x_t . W), k), in descending order of probability, ties -> lowest index first
+    (a stable sort of the negated logits), with the full-vocabulary log-probs on S_t.
+    Returns (idx [T,k] int64, logp [T,k], lse [T], logp_all [T,V])."""
+    X = np.asarray(hidden, dtype=np.float64)
+    Wd = np.asarray(W, dtype=np.float64)
+    z = X @ Wd
+    logp, lse = log_softmax_rows(z)
+    idx = np.argsort(-z, axis=1, kind="stable")[:, :k]
+    return idx, np.take_along_axis(logp, idx, 1), lse, logp
+
+
+def cache_sample(hidden, W, uniforms):
+    """Sample cache of the rollout policy (m local next-token samples per prefix; iid WITH
+    replacement from p_old(.|s_t), duplicates allowed), drawn by inverse CDF from given uniforms u_tj in [0,1):
+        a_tj = min { v : sum_{v' <= v} p_t(v') >= u_tj * sum_v p_t(v) }
+    (the textbook categorical draw; vocabulary order).  Returns (idx [T,K] int64, logp [T,K] = log p_t(a_tj), lse [T],
+    cdf [T,V])."""
+    X = np.asarray(hidden, dtype=np.float64)
+    Wd = np.asarray(W, dtype=np.float64)
+    u = np.asarray(uniforms, dtype=np.float64)
+    logp, lse = log_softmax_rows(X @ Wd)
+    cdf = np.cumsum(np.exp(logp), axis=1)
+    T, K = u.shape
+    idx = np.empty((T, K), dtype=np.int64)
+    for t in range(T):
+        idx[t] = np.minimum(np.searchsorted(cdf[t], u[t] * cdf[t, -1], side="left"), cdf.shape[1] - 1)
+    return idx, np.take_along_axis(logp, idx, 1), lse, cdf

@@ -12,6 +12,7 @@
 #include "../../include/opd.h"
 #include "opd_bwd_kernel.cuh"
 #include "opd_estimators.cuh"
+#include "opd_producer.cuh"
 
 struct opd_handle_s {
     int device = 0;
@@ -170,6 +171,22 @@ inline cudaError_t launch_cg(void (*kernel)(KArgs...), int grid, cudaStream_t st
     attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
+// Number of clusters (CG = 2) / CTAs (CG = 1) of `kernel` that can be resident at the same time on the device: the
+// persistent backward sizes its grid with it, because its tiles wait on tiles of other CTAs (all must be resident).
+template <int CG, class... KArgs>
+inline int max_resident_groups(void (*kernel)(KArgs...), int num_sms) {
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<CG>::SMEM_BYTES) != cudaSuccess) return 0;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(num_sms / CG * CG); cfg.blockDim = dim3(GEMM_THREADS); cfg.dynamicSmemBytes = Cfg<CG>::SMEM_BYTES;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, kernel, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return std::min(n, num_sms / CG);
 }
 
 template <class Epi, int CG>

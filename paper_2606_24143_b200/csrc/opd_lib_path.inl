@@ -204,7 +204,11 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         bp.hint_g = hint_policy(env_int("OPD_HINT_G", 0));
         bp.type_mask = env_int("OPD_BWD_TYPES", 7) & 7;
         // every CTA (pair) must be resident at once: items wait on earlier items of other CTAs
-        const int grid = h->num_sms / h->cg * h->cg;
+        static int resident[3] = {0, -1, -1};
+        if (resident[h->cg] < 0)
+            resident[h->cg] = h->cg == 2 ? max_resident_groups<2>(bwd_kernel<2>, h->num_sms) : max_resident_groups<1>(bwd_kernel<1>, h->num_sms);
+        if (resident[h->cg] < 1) OPD_FAIL(h, OPD_ERR_CUDA, "the backward kernel cannot be made resident on device %d", h->device);
+        const int grid = resident[h->cg] * h->cg;
         if (h->cg == 2) OPD_CUDA(h, launch_cg<2>(bwd_kernel<2>, grid, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, bp));
         else OPD_CUDA(h, launch_cg<1>(bwd_kernel<1>, grid, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, bp));
         h->n_kernels++; h->n_gemm++;

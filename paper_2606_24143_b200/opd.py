@@ -25,7 +25,7 @@ PHASE_NAMES = ("prep", "fwd", "est", "bwd")
 
 EXPORTS = ("opd_create", "opd_destroy", "opd_last_error", "opd_version", "opd_workspace_bytes", "opd_set_workspace",
            "opd_loss_fwd_bwd", "opd_loss_fwd_bwd_host", "opd_debug_logits", "opd_debug_gemm", "opd_last_launch_stats",
-           "opd_set_phase_events", "opd_set_diagnostics")
+           "opd_set_phase_events", "opd_set_diagnostics", "opd_cache_workspace_bytes", "opd_cache_topk", "opd_cache_sample")
 
 _lib = None
 
@@ -71,6 +71,14 @@ def load_library():
     lib.opd_debug_gemm.restype = c_int
     lib.opd_last_launch_stats.argtypes = [c_void_p, POINTER(c_int), POINTER(c_int), POINTER(c_int), POINTER(c_int)]
     lib.opd_last_launch_stats.restype = c_int
+    lib.opd_cache_workspace_bytes.argtypes = [c_int, c_int, c_int, c_int, c_int, c_int]
+    lib.opd_cache_workspace_bytes.restype = c_size_t
+    lib.opd_cache_topk.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_long, c_void_p, c_long, c_long, c_int,
+                                   c_void_p, c_long, c_void_p, c_long, c_void_p]
+    lib.opd_cache_topk.restype = c_int
+    lib.opd_cache_sample.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_long, c_void_p, c_long, c_long, c_int,
+                                     c_void_p, c_long, c_void_p, c_long, c_void_p, c_long, c_void_p]
+    lib.opd_cache_sample.restype = c_int
     lib.opd_set_diagnostics.argtypes = [c_void_p, c_void_p, c_long, c_void_p]
     lib.opd_set_diagnostics.restype = c_int
     lib.opd_set_phase_events.argtypes = [c_void_p, c_void_p]
@@ -215,6 +223,37 @@ class Handle:
         self._check(st)
         out["h2d_bytes"], out["d2h_bytes"] = up.value, down.value
         return out
+
+    # ------------------------------------------------------------------ cache producers
+    def cache_topk(self, hidden, W, k):
+        """opd_cache_topk -> (idx [T,k] int32, logp [T,k] float32, lse [T] float32): the scoring model's top-k support."""
+        T, d = hidden.shape
+        V = W.shape[1]
+        ldk, ldv = _w_strides(W, d)
+        dev = hidden.device
+        idx = torch.empty(T, k, dtype=torch.int32, device=dev)
+        logp = torch.empty(T, k, dtype=torch.float32, device=dev)
+        lse = torch.empty(T, dtype=torch.float32, device=dev)
+        s = torch.cuda.current_stream(dev).cuda_stream
+        self._check(self.lib.opd_cache_topk(self._h, c_void_p(s), T, d, V, _dtype_code(hidden), _ptr(hidden), hidden.stride(0), _ptr(W),
+                                            ldk, ldv, k, _ptr(idx), k, _ptr(logp), k, _ptr(lse)))
+        return idx, logp, lse
+
+    def cache_sample(self, hidden, W, uniforms):
+        """opd_cache_sample -> (idx [T,K] int32, logp [T,K] float32, lse [T]): K inverse-CDF draws per row from
+        softmax(hidden . W) for the uniforms [T,K] (float32, in [0,1))."""
+        T, d = hidden.shape
+        V = W.shape[1]
+        K = uniforms.shape[1]
+        ldk, ldv = _w_strides(W, d)
+        dev = hidden.device
+        idx = torch.empty(T, K, dtype=torch.int32, device=dev)
+        logp = torch.empty(T, K, dtype=torch.float32, device=dev)
+        lse = torch.empty(T, dtype=torch.float32, device=dev)
+        s = torch.cuda.current_stream(dev).cuda_stream
+        self._check(self.lib.opd_cache_sample(self._h, c_void_p(s), T, d, V, _dtype_code(hidden), _ptr(hidden), hidden.stride(0), _ptr(W),
+                                              ldk, ldv, K, _ptr(uniforms), uniforms.stride(0), _ptr(idx), K, _ptr(logp), K, _ptr(lse)))
+        return idx, logp, lse
 
     # ------------------------------------------------------------------ debug entries
     def debug_logits(self, hidden, W, cache_idx):

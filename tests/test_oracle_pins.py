@@ -408,3 +408,50 @@ def test_mc_diagnostics():
         assert np.abs(r["rho"][ti] - np.exp(ell - t["old"][ti])).max() < 1e-14
     r1 = O.opd_oracle(t["X"], t["W"], t["idx"][:, :1], t["lam"][:, :1], t["old"][:, :1], t["mask"], O.RKL_MC, 1)
     assert np.all(r1["var1"] == 0)
+
+
+def test_cache_topk_against_library_topk_and_ties():
+    """cache_topk: values equal torch.topk's (library routine), the set is the k largest, k = V is a full
+    descending sort, exact ties resolve to the lowest index."""
+    t = tiny(41, T=5, d=6, V=40)
+    idx, lp, lse, logp = O.cache_topk(t["X"], t["W"], 7)
+    tv, ti = torch.topk(torch.from_numpy(logp), 7, dim=1)
+    assert np.allclose(lp, tv.numpy(), atol=1e-15) and np.array_equal(idx, ti.numpy())
+    for r in range(5):
+        rest = np.delete(logp[r], idx[r])
+        assert rest.max() <= lp[r].min() and np.all(np.diff(lp[r]) <= 0)
+    assert abs(np.exp(O.cache_topk(t["X"], t["W"], 40)[1]).sum(1) - 1).max() < 1e-12
+    W2 = t["W"].copy(); W2[:, 30] = W2[:, 3]; W2[:, 17] = W2[:, 3]          # three exactly tied columns
+    idx2 = O.cache_topk(t["X"], W2, 40)[0]
+    for r in range(5):
+        pos = [int(np.flatnonzero(idx2[r] == c)[0]) for c in (3, 17, 30)]
+        assert pos[1] == pos[0] + 1 and pos[2] == pos[0] + 2
+
+
+def test_cache_sample_is_the_inverse_cdf_draw():
+    """cache_sample against a brute-force scan, the frequency law on a uniform grid (counts of
+    index v = p_v * n up to 1), u -> 0 / 1 edges, and duplicates being allowed."""
+    t = tiny(43, T=3, d=5, V=11)
+    rng = np.random.default_rng(2)
+    u = rng.random((3, 6))
+    idx, lp, lse, cdf = O.cache_sample(t["X"], t["W"], u)
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    p = np.exp(logp)
+    for r in range(3):
+        for j in range(6):
+            acc, v = 0.0, 0
+            while True:
+                acc += p[r, v]
+                if acc >= u[r, j] * p[r].sum() or v == 10:
+                    break
+                v += 1
+            assert v == idx[r, j] and abs(lp[r, j] - logp[r, v]) < 1e-15
+    n = 20000
+    grid = np.tile((np.arange(n) + 0.5) / n, (3, 1))
+    gi = O.cache_sample(t["X"], t["W"], grid)[0]
+    for r in range(3):
+        assert np.abs(np.bincount(gi[r], minlength=11) - p[r] * n).max() <= 1.0 + 1e-9
+    e = O.cache_sample(t["X"], t["W"], np.array([[0.0, 1.0 - 1e-16]] * 3))[0]
+    assert np.all(e[:, 0] == 0) and np.all(e[:, 1] == 10)
+    same = O.cache_sample(t["X"], t["W"], np.full((3, 4), 0.37))[0]
+    assert np.all(same == same[:, :1])
