@@ -54,6 +54,8 @@ def pick_cache(inp, cfg, mode_name):
     from paper_2606_24143_b200 import opd, synth
     if mode_name == "fkl":
         return opd.FKL_TOPK, inp["topk_idx"], inp["topk_logq"], None, cfg["k"]
+    if mode_name == "rtopk":
+        return opd.RKL_TOPK, inp["stopk_idx"], inp["stopk_logq"], None, cfg["k"]
     if mode_name == "mixed":
         idx, lam, old, kk = synth.mixed_cache(inp)
         return opd.MIXED, idx, lam, old, kk
@@ -105,16 +107,32 @@ def to_np(t):
     return t.double().numpy() if t.is_floating_point() else t.numpy()
 
 
-def oracle_sample(inp, mode, idx, lam, old, kk, n_rows: int):
+def oracle_prepare(inp, idx, lam, old, max_rows: int):
+    """fp64 numpy copies of the first rows of the workload (input conversion is not part of the timed oracle run)."""
+    mask = to_np(inp["mask"])
+    rows = np.flatnonzero(mask)[:max_rows]
+    n = int(rows.max()) + 1 if rows.size else 0
+    return dict(X=to_np(inp["hidden"][:n]), W=to_np(inp["W"]), idx=to_np(idx[:n]), lam=to_np(lam[:n]),
+                old=None if old is None else to_np(old[:n]), mask=mask[:n], rows=rows)
+
+
+def oracle_sample(prep, mode, kk, n_rows: int):
     """The fp64 oracle as it stands on the first n_rows live tokens of the workload (full d and V), forward+backward."""
     from oracle import opd_oracle as O
-    mask = to_np(inp["mask"])
-    rows = np.flatnonzero(mask)[:n_rows]
-    X, W = to_np(inp["hidden"][: int(rows.max()) + 1]), to_np(inp["W"])
+    rows = prep["rows"][:n_rows]
     t0 = time.perf_counter()
-    O.opd_oracle(X, W, to_np(idx[: X.shape[0]]), to_np(lam[: X.shape[0]]), None if old is None else to_np(old[: X.shape[0]]),
-                 mask[: X.shape[0]], mode, kk, rows=list(rows))
+    O.opd_oracle(prep["X"], prep["W"], prep["idx"], prep["lam"], prep["old"], prep["mask"], mode, kk, rows=list(rows))
     return len(rows), time.perf_counter() - t0
+
+
+def oracle_rows_for(prep, mode, kk, seconds: float, cap: int = 256) -> int:
+    """Rows per timed oracle run so that it lasts about `seconds`: t(n) = a + b n fitted on 4 and 16 rows."""
+    oracle_sample(prep, mode, kk, 2)
+    n1, t1 = oracle_sample(prep, mode, kk, 4)
+    n2, t2 = oracle_sample(prep, mode, kk, 16)
+    b = max((t2 - t1) / max(n2 - n1, 1), 1e-7)
+    a = max(t1 - b * n1, 0.0)
+    return int(max(2, min(cap, len(prep["rows"]), (seconds - a) / b)))
 
 
 def cpu_threads():
@@ -136,15 +154,13 @@ def run_reference(args, rank, world):
     from paper_2606_24143_b200 import synth
     inp = synth.make_inputs(gen, c=args.config, device=dev)
     mode, idx, lam, old, kk = pick_cache(inp, gen, args.mode)
-    inp = {k: (v.cpu() if isinstance(v, torch.Tensor) else v) for k, v in inp.items()}
-    idx, lam, old = idx.cpu(), lam.cpu(), (None if old is None else old.cpu())
-    n, dt = oracle_sample(inp, mode, idx, lam, old, kk, 2)       # calibration
-    rows = int(max(2, min(256, args.ref_seconds / max(dt / n, 1e-6))))
-    for _ in range(args.warmup if args.warmup < 2 else 1):
-        oracle_sample(inp, mode, idx, lam, old, kk, rows)
+    prep = oracle_prepare(inp, idx, lam, old, 2048)
+    rows = oracle_rows_for(prep, mode, kk, args.ref_seconds, cap=2048)
+    for _ in range(1 if args.warmup >= 1 else 0):
+        oracle_sample(prep, mode, kk, rows)
     tot_t, tot_n = 0.0, 0
     for _ in range(args.steps):
-        n, dt = oracle_sample(inp, mode, idx, lam, old, kk, rows)
+        n, dt = oracle_sample(prep, mode, kk, rows)
         tot_t += dt; tot_n += n
     v = tot_n / tot_t
     sample = f"{rows} live tokens of {cfg['name']} per step (full d={cfg['d']}, V={cfg['V']}), forward+backward incl. grad_W, numpy fp64"
@@ -156,6 +172,55 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def run_producer_bench(args, h, inp, cfg, dev, world, rank, dist):
+    """Cache producers (opd_cache_topk / opd_cache_sample) on the workload's shapes: tokens scored per second.
+    Two streamed contractions per call (pass A: LSE partials, pass B: collect / resolve), 4*d*V flops per token."""
+    T, d, V = cfg["T"], cfg["d"], cfg["V"]
+    n = cfg["k"] if args.op == "topk" else cfg["K"]
+    u = torch.rand(T, n, device=dev, generator=torch.Generator(device=dev).manual_seed(1)) if args.op == "sample" else None
+    # the scoring model's head: an independent seeded matrix of the same shape (synth keeps only W resident)
+    Wt = inp["W"]
+    call = (lambda: h.cache_topk(inp["hidden"], Wt, n)) if args.op == "topk" else (lambda: h.cache_sample(inp["hidden"], Wt, u))
+    for _ in range(max(args.warmup, 3)):
+        call()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(dev.index) if rank == 0 else None
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev[0].record()
+    for _ in range(args.steps):
+        call()
+    ev[1].record()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    total_ms = ev[0].elapsed_time(ev[1])
+    clocks = sampler.stop() if sampler else None
+    if dist is not None:
+        t = torch.tensor([total_ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    if rank != 0:
+        return
+    ms = total_ms / args.steps
+    pk = peaks()
+    ach = 4.0 * d * V * T / (ms * 1e-3) / 1e12
+    st = h.launch_stats()
+    line = dict(metric=f"cache producer ({args.op}) tokens scored/s on 1 B200", value=T * world / (ms * 1e-3), unit="tokens/s", n_gpus=world,
+                steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="bf16" if cfg["dtype"] == "bf16" else "f32(3xbf16)", data="synthetic",
+                config=dict(workload=f"{cfg['name']} opd_cache_{args.op} n={n}", T=T, d=d, V=V,
+                            l2_policy="inputs larger than L2 (W alone is %.0f MB)" % (d * V * 2 / 1e6)),
+                clocks=clocks, e2e=None, gpu_launches=st["kernels"] * args.steps,
+                roofline=dict(bound="tensor", achieved=ach, peak=pk["sustained"], unit="TFLOP/s", frac=ach / pk["sustained"], traffic=None,
+                              kernel="opd::gemm_kernel<FwdEpi,2> + opd::gemm_kernel<%s,2>" % ("CollectEpi" if args.op == "topk" else "SampleEpi"),
+                              flops_per_step=4.0 * d * V * T, frac_of_burst=ach / pk["burst"]),
+                cpu_baseline=None)
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -163,7 +228,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1..5); 4 = the config the metric is quoted on")
-    ap.add_argument("--mode", default=None, choices=["fkl", "mc", "mixed"])
+    ap.add_argument("--mode", default=None, choices=["fkl", "mc", "mixed", "rtopk"])
+    ap.add_argument("--op", default="loss", choices=["loss", "topk", "sample"],
+                    help="loss = the hot path (default, the contract's line); topk / sample = the cache producers (NEXT-3)")
     ap.add_argument("--tokens", type=int, default=0, help="override T (debugging)")
     ap.add_argument("--sigma", type=float, default=None)
     ap.add_argument("--no-e2e", action="store_true")
@@ -196,6 +263,9 @@ def main():
     T, d, V = cfg["T"], cfg["d"], cfg["V"]
     n_live = int((inp["mask"] != 0).sum().item())
     h = opd.Handle(local)
+    if args.op != "loss":
+        run_producer_bench(args, h, inp, cfg, dev, world, rank, dist)
+        return
     gh = torch.empty_like(inp["hidden"])
     gw = torch.empty(d, V, dtype=torch.float32, device=dev)
 
@@ -294,12 +364,10 @@ def main():
     whole = flops_exec / (ms_per_step * 1e-3) / 1e12
     cpu = None
     if not args.no_cpu:
-        cinp = {k: (v.cpu() if isinstance(v, torch.Tensor) else v) for k, v in inp.items() if k in ("hidden", "W", "mask")}
-        cidx, clam, cold = idx[:4096].cpu(), lam[:4096].cpu(), (None if old is None else old[:4096].cpu())
-        cinp["hidden"] = cinp["hidden"][:4096]; cinp["mask"] = cinp["mask"][:4096]
-        n, dt = oracle_sample(cinp, mode, cidx, clam, cold, kk, 2)
-        rows = int(max(2, min(256, args.ref_seconds / max(dt / n, 1e-6))))
-        n, dt = oracle_sample(cinp, mode, cidx, clam, cold, kk, rows)
+        sub = dict(hidden=inp["hidden"][:4096], W=inp["W"], mask=inp["mask"][:4096])
+        prep = oracle_prepare(sub, idx[:4096], lam[:4096], None if old is None else old[:4096], 2048)
+        rows = oracle_rows_for(prep, mode, kk, args.ref_seconds, cap=2048)
+        n, dt = oracle_sample(prep, mode, kk, rows)
         cpu = dict(value=n / dt, unit=UNIT, cores=cpu_threads(), kind="oracle",
                    sample=f"{n} live tokens of this workload (full d, V), forward+backward incl. grad_W, numpy fp64, {dt:.1f} s")
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
