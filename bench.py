@@ -47,6 +47,8 @@ def workload(cfg_id: int, args):
     cfg = dict(synth.CONFIGS[cfg_id])
     if args.tokens:
         cfg["T"] = args.tokens
+    if args.cache_width:
+        cfg["k"] = cfg["K"] = args.cache_width
     return cfg
 
 
@@ -232,7 +234,9 @@ def main():
     ap.add_argument("--op", default="loss", choices=["loss", "topk", "sample"],
                     help="loss = the hot path (default, the contract's line); topk / sample = the cache producers (NEXT-3)")
     ap.add_argument("--tokens", type=int, default=0, help="override T (debugging)")
-    ap.add_argument("--sigma", type=float, default=None)
+    ap.add_argument("--sigma", type=float, default=None, help="staleness of the rollout policy: W_old = W + sigma*N(0,1/d)")
+    ap.add_argument("--cache-width", type=int, default=0, help="override the config's k and K (C4's cost-vs-cache-size sweep)")
+    ap.add_argument("--diag", action="store_true", help="also report rho statistics of the MC cache (opd_set_diagnostics)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--ref-seconds", type=float, default=12.0)
@@ -342,6 +346,17 @@ def main():
             dist.destroy_process_group()
         return
 
+    diag = None
+    if args.diag and mode == opd.RKL_MC:
+        rho = torch.zeros(T, idx.shape[1], device=dev)
+        h.set_diagnostics(rho, None)
+        rr = h.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, flags=opd.F_FWD_ONLY)
+        torch.cuda.synchronize()
+        h.set_diagnostics(None, None)
+        rl = rho[inp["mask"] != 0].flatten()
+        srt = torch.sort(rl).values
+        diag = dict(rho_mean=float(rl.mean()), rho_p99=float(srt[int(0.99 * (srt.numel() - 1))]), rho_max=float(rl.max()),
+                    mean_per_token_kl=float(rr["per_token_kl"].sum() / max(n_live, 1)))
     pk = peaks()
     # Roofline of the dominant kernel, opd::bwd_kernel (one launch per step: S6 logits recompute + S7 grad_hidden +
     # S8 grad_W = 3 contractions of 2*d*V flops per live token), timed live with CUDA events on the
@@ -379,7 +394,7 @@ def main():
                 pct_of_bf16_peak=dict(executed_8dV_vs_burst=100 * whole / pk["burst"], executed_8dV_vs_sustained=100 * whole / pk["sustained"],
                                       model_6dV_vs_burst=100 * whole * 0.75 / pk["burst"], tflops_executed=whole, peaks=pk),
                 phase_ms=pm, step_ms=step_ms, loss=loss_val, clocks=clocks, e2e=e2e, gpu_launches=stats["kernels"] * args.steps,
-                roofline=roofline, cpu_baseline=cpu)
+                roofline=roofline, cpu_baseline=cpu, mc_diagnostics=diag)
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
