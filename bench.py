@@ -236,6 +236,7 @@ def main():
     ap.add_argument("--tokens", type=int, default=0, help="override T (debugging)")
     ap.add_argument("--sigma", type=float, default=None, help="staleness of the rollout policy: W_old = W + sigma*N(0,1/d)")
     ap.add_argument("--cache-width", type=int, default=0, help="override the config's k and K (C4's cost-vs-cache-size sweep)")
+    ap.add_argument("--layout", default="dv", choices=["dv", "vd"], help="storage order of W: [d,V] row-major (BASELINE.json) or [V,d] (lm_head.weight)")
     ap.add_argument("--diag", action="store_true", help="also report rho statistics of the MC cache (opd_set_diagnostics)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -271,7 +272,11 @@ def main():
         run_producer_bench(args, h, inp, cfg, dev, world, rank, dist)
         return
     gh = torch.empty_like(inp["hidden"])
-    gw = torch.empty(d, V, dtype=torch.float32, device=dev)
+    if args.layout == "vd":          # same logical [d,V] matrices, [V,d] storage
+        inp["W"] = inp["W"].t().contiguous().t()
+        gw = torch.empty(V, d, dtype=torch.float32, device=dev).t()
+    else:
+        gw = torch.empty(d, V, dtype=torch.float32, device=dev)
 
     def step():
         return h.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, grad_hidden=gh, grad_W=gw)

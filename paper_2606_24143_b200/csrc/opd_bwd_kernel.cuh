@@ -3,14 +3,14 @@
 //
 //   block 0: G(0)      block b: G(b), DX(b-1), DW(b-1)      block S: DX(S-1), DW(S-1)
 //
-//   G(s)   logits of super-tile s recomputed -> G tile (bf16) into buffer s%2 of the L2-resident G ring
+//   G(s)   logits of super-tile s recomputed -> G tile (bf16) into buffer s%R of the G ring (consumed from L2)
 //   DX(s)  grad_hidden[tb] (+)= G(s) . W[:,vb]^T        DW(s)  grad_W[:,vb] += Xc[tb]^T . G(s)
 //
 // CTAs take items round-robin in list order; an item only depends on earlier items, through two counters
 // per super-tile in global memory (release by the epilogue after its stores, acquire by whoever consumes):
 //   g_done[s] == #G tiles      before the TMA producer loads G(s) for a DX/DW tile
 //   c_done[s-1] complete       before a DX/DW(s) epilogue touches the fp32 accumulators (previous writer)
-//   c_done[s-2] complete       before a G(s) epilogue overwrites ring buffer s%2 (previous readers)
+//   c_done[s-R] complete       before a G(s) epilogue overwrites ring buffer s%R (previous readers; R = ring depth)
 // This removes the ~900 launches, their partial last waves and the pipeline refill of the per-GEMM version.
 #pragma once
 #include "opd_epilogues_bwd.cuh"
@@ -20,6 +20,7 @@ namespace opd {
 struct BwdParams {
     int d, V, Tb, Vb, nvb;     // super-tile rows / cols, vocabulary super-tiles per token super-tile
     int wl;                    // 0: W is [d,V] row-major, 1: [V,d]
+    int gbufs;                 // depth of the G ring (2 or 3)
     int planes;                // 1 (bf16) or 3 (fp32 inputs as three bf16 terms)
     const int* n_live;
     int* g_done;               // [S]
@@ -142,7 +143,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 if (!((bp.type_mask >> t.type) & 1)) continue;
                 TileOp op;
                 int pa_off = 0, pb_off = 0;
-                const int buf = t.s & 1;
+                const int buf = t.s % bp.gbufs;
                 const int a_row = (t.m_blk * CG + rank) * BM, b_row = t.n_blk * BN + rank * C::B_ROWS;
                 if (t.type == T_G) {
                     op.tA = &m_xc_k; op.tB = &m_w_fwd; op.a_mn = 0; op.b_mn = (bp.wl == 0);
@@ -203,7 +204,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             GemmParams gp{};                      // the fields the epilogues read
             gp.tok_off = t.tb0;
             // wait for the previous writer / readers of what this epilogue is about to write
-            const int dep = (t.type == T_G) ? t.s - 2 : t.s - 1;
+            const int dep = (t.type == T_G) ? t.s - bp.gbufs : t.s - 1;
             if (dep >= 0 && bp.type_mask == 7) {
                 if (lane == 0) { wait_counter(bp.c_done + dep, CG * (sc.nDX(dep) + sc.nDW(dep))); fence_proxy_async_all(); }
                 __syncwarp();
@@ -211,7 +212,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             if (t.type == T_G) {
                 gp.b_off = t.vb0; gp.N = t.Vb_eff;
                 GEpi::Params ep = bp.g;
-                ep.gs += static_cast<size_t>(t.s & 1) * bp.planes * ep.plane_stride;
+                ep.gs += static_cast<size_t>(t.s % bp.gbufs) * bp.planes * ep.plane_stride;
                 GEpi::State st = GEpi::prepare(ep, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
                 const uint32_t taddr = epi_acquire<CG>(P, lt, quarter);
                 GEpi::run(ep, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, nullptr, epi_tid);

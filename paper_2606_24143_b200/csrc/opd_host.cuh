@@ -91,7 +91,8 @@ struct Plan {
     int Tb, Vb;           // backward super-tile (rows of tokens x vocabulary columns), multiples of 128 / 256
     int est_blocks;
     size_t off_nlive, off_badidx, off_live_rows, off_xc, off_wsplit, off_sorted, off_perm, off_zc, off_beta,
-           off_partials, off_lse2, off_coef, off_gs, off_dxacc, off_block_sums, off_counters, total;
+           off_partials, off_lse2, off_coef, off_gs, off_dxacc, off_block_sums, off_counters, off_wt, off_gwt, total;
+    bool sparse_bwd;      // alpha == 0 on every row: gradients live on the cached columns only (no dense backward)
     int n_super;          // number of backward super-tiles (upper bound)
     int gs_bufs;          // ring depth of the G super-tile buffer
     size_t xc_plane, w_plane, gs_plane;   // elements per plane
@@ -112,7 +113,7 @@ inline int cta_group_setting() {
     return cg == 1 ? 1 : 2;
 }
 
-inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags) {
+inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int mode = 1) {
     Plan p{};
     p.T = T; p.d = d; p.V = V; p.C = C; p.planes = fp32 ? 3 : 1;
     const int TM = BM * cta_group_setting();              // tile rows of the GEMM core (CTA or CTA pair)
@@ -140,15 +141,19 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags) {
     p.off_lse2 = take(sizeof(float) * (size_t)p.t_pad);
     p.off_coef = take(sizeof(float) * (size_t)p.t_pad);
     const bool bwd = !(flags & OPD_F_FWD_ONLY);
+    p.sparse_bwd = (mode == OPD_RKL_TOPK || (mode == OPD_FKL_TOPK && (flags & OPD_F_RENORM_STUDENT))) && !env_int("OPD_DENSE_BWD", 0);
+    // sparse backward with [d,V] storage works on [V,d] transposes (contiguous d-vectors per cached column)
+    p.off_wt = take(bwd && p.sparse_bwd ? (size_t)d * V * (fp32 ? 4 : 2) : 0);
+    p.off_gwt = take(bwd && p.sparse_bwd ? (size_t)d * V * 4 : 0);
     p.gs_plane = (size_t)p.Tb * p.Vb;
-    p.gs_bufs = 2;
+    p.gs_bufs = std::min(3, std::max(2, env_int("OPD_G_BUFS", 2)));
     p.n_super = ceil_div(p.t_pad, p.Tb) * ceil_div(V, p.Vb);
     p.off_counters = take(bwd ? sizeof(int) * 2 * (size_t)p.n_super : 0);
     // The per-tile LSE partials are dead once the estimators have run, the G ring and the grad_hidden partial
     // sums only live in the backward: they share one region.
     const size_t partial_bytes = align_up(sizeof(float2) * (size_t)p.num_n * p.t_pad, 1024);
-    const size_t gs_bytes = bwd ? align_up(2 * p.gs_plane * p.planes * p.gs_bufs, 1024) : 0;
-    const size_t dx_bytes = bwd ? align_up(sizeof(float) * (size_t)p.Tb * d, 1024) : 0;
+    const size_t gs_bytes = bwd && !p.sparse_bwd ? align_up(2 * p.gs_plane * p.planes * p.gs_bufs, 1024) : 0;
+    const size_t dx_bytes = bwd && !p.sparse_bwd ? align_up(sizeof(float) * (size_t)p.Tb * d, 1024) : 0;
     const size_t region = take(std::max(partial_bytes, gs_bytes + dx_bytes));
     p.off_partials = region;
     p.off_gs = region;

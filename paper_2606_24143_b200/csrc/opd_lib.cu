@@ -62,9 +62,9 @@ static int cache_width(opd_mode_t mode, int k_or_K, int* k, int* K) {
     return k_or_K;
 }
 
-extern "C" size_t opd_workspace_bytes(int T, int d, int V, int C, opd_dtype_t dtype, opd_mode_t, unsigned flags) {
+extern "C" size_t opd_workspace_bytes(int T, int d, int V, int C, opd_dtype_t dtype, opd_mode_t mode, unsigned flags) {
     if (T < 1 || d < 64 || V < 256 || C < 1 || C > 64) return 0;
-    return make_plan(T, d, V, C, dtype == OPD_FP32, flags).total;
+    return make_plan(T, d, V, C, dtype == OPD_FP32, flags, (int)mode).total;
 }
 
 extern "C" opd_status_t opd_set_workspace(opd_handle_t h, void* ws, size_t bytes) {

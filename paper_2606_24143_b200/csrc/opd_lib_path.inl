@@ -65,7 +65,7 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     OPD_CUDA(h, cudaSetDevice(h->device));
     h->cg = cta_group_setting();
     const uint32_t b_box = BN / h->cg;                    // rows of a K-major B box: each CTA of a pair loads half of N
-    const Plan p = make_plan(T, d, V, C, fp32, a.flags | (a.stop_after_fwd ? OPD_F_FWD_ONLY : 0));
+    const Plan p = make_plan(T, d, V, C, fp32, a.flags | (a.stop_after_fwd ? OPD_F_FWD_ONLY : 0), (int)a.mode);
     s = ensure_workspace(h, p.total);
     if (s != OPD_OK) return s;
     h->n_kernels = h->n_gemm = 0;
@@ -189,13 +189,42 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
 
     // ------------------------------------------------------------------ S6-S8 backward, super-tile by super-tile
     phase_mark(h, st, OPD_PHASE_BWD, 0);
-    if (!fwd_only) {
+    // alpha_t == 0 on every row: the gradient lives on the cached columns only, no softmax tile has to be re-formed
+    const bool sparse_bwd = p.sparse_bwd;
+    if (!fwd_only && sparse_bwd) {
+        const void* Wv = a.W;                                   // [V,d] view of W / grad_W: contiguous d-vectors per column
+        float* gwv = static_cast<float*>(a.grad_W);
+        long ldwv = ldw, ldgv = ldgw;
+        if (wl == 0) {
+            void* wt = ws + p.off_wt;
+            gwv = reinterpret_cast<float*>(ws + p.off_gwt);
+            const dim3 tg(ceil_div(V, 32), ceil_div(d, 32));
+            if (fp32) k_transpose<float><<<tg, dim3(32, 8), 0, st>>>(static_cast<const float*>(a.W), ldw, d, V, static_cast<float*>(wt), (long)d, 0);
+            else k_transpose<__nv_bfloat16><<<tg, dim3(32, 8), 0, st>>>(static_cast<const __nv_bfloat16*>(a.W), ldw, d, V,
+                                                                        static_cast<__nv_bfloat16*>(wt), (long)d, 0);
+            OPD_CUDA(h, cudaMemsetAsync(gwv, 0, sizeof(float) * (size_t)d * V, st));
+            Wv = wt; ldwv = d; ldgv = d;
+            h->n_kernels++;
+        }
+        if (fp32) k_sparse_bwd<float><<<p.t_pad, 256, 0, st>>>(a.hidden, a.ld_hidden, Wv, ldwv, d, C, sorted_idx, beta, live_rows, n_live,
+                                                               a.grad_hidden, a.ld_gh, gwv, ldgv);
+        else k_sparse_bwd<__nv_bfloat16><<<p.t_pad, 256, 0, st>>>(a.hidden, a.ld_hidden, Wv, ldwv, d, C, sorted_idx, beta, live_rows, n_live,
+                                                                  a.grad_hidden, a.ld_gh, gwv, ldgv);
+        h->n_kernels++;
+        if (wl == 0) {                                          // grad_W[d,V] += gWt^T
+            const dim3 tg(ceil_div(d, 32), ceil_div(V, 32));
+            k_transpose<float><<<tg, dim3(32, 8), 0, st>>>(gwv, (long)d, V, d, static_cast<float*>(a.grad_W), ldgw, 1);
+            h->n_kernels++;
+        }
+        OPD_CUDA(h, cudaGetLastError());
+    }
+    if (!fwd_only && !sparse_bwd) {
         // one persistent kernel walks every super-tile: G re-formation, grad_hidden and grad_W tiles interleaved,
         // ordered by dependency counters in global memory (opd_bwd_kernel.cuh)
         int* counters = reinterpret_cast<int*>(ws + p.off_counters);
         OPD_CUDA(h, cudaMemsetAsync(counters, 0, sizeof(int) * 2 * (size_t)p.n_super, st));
         BwdParams bp{};
-        bp.d = d; bp.V = V; bp.Tb = p.Tb; bp.Vb = p.Vb; bp.nvb = ceil_div(V, p.Vb); bp.wl = wl; bp.planes = p.planes;
+        bp.d = d; bp.V = V; bp.Tb = p.Tb; bp.Vb = p.Vb; bp.nvb = ceil_div(V, p.Vb); bp.wl = wl; bp.planes = p.planes; bp.gbufs = p.gs_bufs;
         bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super;
         bp.g = GEpi::Params{gs, p.Tb, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V};
         bp.dx = dxp;
