@@ -87,3 +87,42 @@ def test_C3_shape_few_live_tokens_full_oracle(handle):
     r = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, m, O.RKL_MC, kk, want_lse=True, want_student_logp=True)
     torch.cuda.synchronize()
     compare_all(r, oracle_for(inp, idx, lam, old, O.RKL_MC, kk, chunk=32), f64(m), "bf16")
+
+
+def test_C4_shape_sparse_reverse_kl_sampled(handle):
+    """OPD_RKL_TOPK (stale student support, sparse backward) at the C4 shape on sampled rows."""
+    sampled_check(handle, synth.CONFIGS[4], 4, O.RKL_TOPK)
+
+
+def test_producers_at_C3_shape_sampled_rows(handle):
+    """opd_cache_topk / opd_cache_sample at T=16384, d=2048, V=151936 in the launch configuration bench.py --op times:
+    validity of the sampled rows against the fp64 oracle (each row needs only its own logits)."""
+    cfg = synth.CONFIGS[3]
+    inp = synth.make_inputs(cfg, c=3, device=DEV)
+    X, W = inp["hidden"], inp["W"]
+    T, V = cfg["T"], cfg["V"]
+    k = cfg["k"]
+    idx, lp, lse = handle.cache_topk(X, W, k)
+    u = torch.rand(T, cfg["K"], generator=torch.Generator(device=DEV).manual_seed(9), device=DEV)
+    sidx, slp, slse = handle.cache_sample(X, W, u)
+    torch.cuda.synchronize()
+    assert torch.equal(lse, slse)
+    assert int(idx.min()) >= 0 and int(idx.max()) < V and int(sidx.min()) >= 0 and int(sidx.max()) < V
+    rows = np.sort(np.random.default_rng(3).choice(T, 16, replace=False))
+    sel = torch.as_tensor(rows, device=DEV)
+    Xs, Wd = f64(X[sel]), f64(W)
+    ridx, rlp, rlse, logp = O.cache_topk(Xs, Wd, k)
+    gi, gl = idx[sel].cpu().numpy().astype(np.int64), f64(lp[sel])
+    assert np.abs(f64(lse[sel]) - rlse).max() <= LOGP_ATOL
+    srt = -np.sort(-logp, axis=1)
+    for r in range(len(rows)):
+        assert len(set(gi[r])) == k
+        assert np.abs(gl[r] - logp[r, gi[r]]).max() <= LOGP_ATOL
+        assert logp[r, gi[r]].min() >= srt[r, k - 1] - 2e-4 and np.all(np.diff(logp[r, gi[r]]) <= 2e-4)
+    assert np.mean([np.array_equal(gi[r], ridx[r]) for r in range(len(rows))]) >= 0.75
+    _, _, _, cdf = O.cache_sample(Xs, Wd, f64(u[sel]))
+    si, u64 = sidx[sel].cpu().numpy().astype(np.int64), f64(u[sel])
+    hi = np.take_along_axis(cdf, si, 1)
+    lo = np.where(si > 0, np.take_along_axis(cdf, np.maximum(si - 1, 0), 1), 0.0)
+    assert np.all(u64 <= hi + 2e-5) and np.all(u64 >= lo - 2e-5)
+    assert np.abs(f64(slp[sel]) - np.take_along_axis(logp, si, 1)).max() <= LOGP_ATOL
