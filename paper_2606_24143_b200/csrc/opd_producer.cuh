@@ -34,16 +34,24 @@ __global__ void __launch_bounds__(256) k_lse_theta(const float2* __restrict__ pa
     if (lane == 0) lse[row] = M + logf(S);
     if (theta == nullptr) return;
     if (k > num_n) { if (lane == 0) theta[row] = -INFINITY; return; }
-    // rank counting: the tile maximum with exactly k-1 tile maxima ahead of it (ties broken by tile index)
-    for (int i = lane; i < num_n; i += 32) {
-        const float mi = partials[static_cast<size_t>(i) * t_pad + row].x;
-        int rank = 0;
-        for (int j = 0; j < num_n; ++j) {
-            const float mj = partials[static_cast<size_t>(j) * t_pad + row].x;
-            rank += (mj > mi) || (mj == mi && j < i);
+    // k selection passes over the tile maxima in the order (value descending, tile index ascending): pass i finds the
+    // largest entry that comes after the one pass i-1 found; the k-th one is theta.
+    float pv = INFINITY; int pi = -1;
+    for (int it = 0; it < k; ++it) {
+        float bv = -INFINITY; int bi = 0x7fffffff;
+        for (int n = lane; n < num_n; n += 32) {
+            const float m = partials[static_cast<size_t>(n) * t_pad + row].x;
+            const bool after = (m < pv) || (m == pv && n > pi);
+            if (after && (m > bv || (m == bv && n < bi))) { bv = m; bi = n; }
         }
-        if (rank == k - 1) theta[row] = mi;
+        for (int o = 16; o > 0; o >>= 1) {
+            const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+        }
+        pv = bv; pi = bi;
     }
+    if (lane == 0) theta[row] = pv;
 }
 
 // ------------------------------------------------------------------------------------------ CollectEpi (top-k pass B)
@@ -207,21 +215,28 @@ struct SampleEpi {
             const int col0 = n_blk * BN + c * 32;
             if (col0 >= p.V) break;                                   // warp-uniform
             if (!mine) continue;
-#pragma unroll 1
-            for (int i = 0; i < 32 && col0 + i < p.V; ++i) {
-                const float z = select32(v, i);
-                cum += expf(z - st.lse);
-                last_col = col0 + i; last_z = z;
-                while (mine && cum >= res) {
-                    const size_t o = static_cast<size_t>(row);
-                    p.idx_out[o * p.ld_idx + pr[st.cursor]] = col0 + i;
-                    p.logp_out[o * p.ld_logp + pr[st.cursor]] = z - st.lse;
-                    ++st.cursor;
-                    mine = st.cursor < p.K && tt[st.cursor] == n_blk;
-                    res = mine ? tr[st.cursor] : 0.f;
-                }
-                if (!mine) break;
+            const int nv = min(32, p.V - col0);                       // valid columns of this chunk
+            float pre[32];                                            // running mass inside the chunk
+            float run = 0.f;
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {
+                run += (i < nv) ? expf(v[i] - st.lse) : 0.f;
+                pre[i] = run;
             }
+            while (mine && cum + run >= res) {                        // this draw resolves inside the chunk
+                int pos = 32;
+#pragma unroll
+                for (int i = 31; i >= 0; --i) pos = (cum + pre[i] >= res) ? i : pos;
+                pos = min(pos, nv - 1);
+                const float z = select32(v, pos);
+                p.idx_out[static_cast<size_t>(row) * p.ld_idx + pr[st.cursor]] = col0 + pos;
+                p.logp_out[static_cast<size_t>(row) * p.ld_logp + pr[st.cursor]] = z - st.lse;
+                ++st.cursor;
+                mine = st.cursor < p.K && tt[st.cursor] == n_blk;
+                res = mine ? tr[st.cursor] : 0.f;
+            }
+            cum += run;
+            last_col = col0 + nv - 1; last_z = select32(v, nv - 1);
         }
         while (mine) {                                                 // rounding: residual beyond the tile's mass
             p.idx_out[static_cast<size_t>(row) * p.ld_idx + pr[st.cursor]] = last_col;
