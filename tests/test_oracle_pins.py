@@ -455,3 +455,31 @@ def test_cache_sample_is_the_inverse_cdf_draw():
     assert np.all(e[:, 0] == 0) and np.all(e[:, 1] == 10)
     same = O.cache_sample(t["X"], t["W"], np.full((3, 4), 0.37))[0]
     assert np.all(same == same[:, :1])
+
+
+def test_P12_paper_table6_fixed_prefix_ratios_follow_one_over_m():
+    """tests/golden/paper_table6_mc_variance_ratios.txt (Table 6): the paper's measured fixed-prefix
+    ratios R_m^local sit within 7% of 1/m; the oracle's estimator obeys the same law exactly in expectation, which its
+    within-prefix diagnostics reproduce: E[var of the m-sample mean] = var1 / m (mc_diagnostics), here checked by
+    enumeration of all m-tuples of a small categorical."""
+    import itertools
+    import os
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "paper_table6_mc_variance_ratios.txt"))
+            if l.strip() and not l.startswith("#")]
+    table = {int(r[0]): float(r[1]) for r in rows}
+    for m, ratio in table.items():
+        assert abs(ratio * m - 1.0) < 0.07
+    t = tiny(51, T=1, d=4, V=5)
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    po = np.exp(t["logpo"][0])
+    def var_of_mean(m):
+        mean = sq = 0.0
+        for a in itertools.product(range(5), repeat=m):
+            a = np.array(a)
+            pr = float(np.prod(po[a]))
+            L = O.token_terms(O.RKL_MC, t["logq"][0, a], t["logpo"][0, a], logp[0, a], 0)[0]
+            mean += pr * L; sq += pr * L * L
+        return sq - mean * mean
+    v1 = var_of_mean(1)
+    for m in (2, 4):
+        assert abs(var_of_mean(m) / v1 - 1.0 / m) < 1e-10
