@@ -127,6 +127,21 @@ opd_status_t opd_loss_fwd_bwd_host(opd_handle_t h,
     float* loss_host, float* per_token_kl_host, void* grad_hidden_host, void* grad_W_host,
     size_t* h2d_bytes, size_t* d2h_bytes);
 
+/* Pipelined form of the host entry point: two staging slots (0, 1) and separate copy-in / compute / copy-out streams.
+ * _submit enqueues the H2D copies, the kernels and the D2H copies of one step on `slot` and returns; _wait blocks until
+ * that slot's results are in the host buffers (which must stay valid, and should be pinned, until then). Alternating
+ * the slots overlaps the copies of neighbouring steps with the kernels of the current one:
+ *     submit(0, step 0); for i >= 1: submit(i % 2, step i); wait((i - 1) % 2);   ...  wait(last % 2)
+ * A slot must be waited for before it is submitted to again (OPD_ERR_BAD_ARG otherwise). */
+opd_status_t opd_loss_fwd_bwd_host_submit(opd_handle_t h, int slot,
+    int T, int d, int V, opd_dtype_t dtype,
+    const void* hidden_host, const void* W_host,
+    const int* cache_idx_host, const float* cache_teacher_logp_host, const float* cache_old_logp_host,
+    const unsigned char* mask_host,
+    opd_mode_t mode, int k_or_K, unsigned flags, float norm_override,
+    float* loss_host, float* per_token_kl_host, void* grad_hidden_host, void* grad_W_host);
+opd_status_t opd_loss_fwd_bwd_host_wait(opd_handle_t h, int slot, size_t* h2d_bytes, size_t* d2h_bytes);
+
 /* cache producers -------------------------------------------------------------------------------
  * The steps either side of the learner path that build the finite caches it consumes, on the same
  * streamed contraction (the logits are never stored).  hidden / W / dtype / strides as for opd_loss_fwd_bwd; every row

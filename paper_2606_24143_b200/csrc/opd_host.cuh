@@ -24,9 +24,12 @@ struct opd_handle_s {
     bool ws_owned = false;
     std::string err;
     // host-entry staging buffers (opd_loss_fwd_bwd_host)
-    void* stage = nullptr;
-    size_t stage_bytes = 0;
-    cudaStream_t host_stream = nullptr;
+    void* stage[2] = {nullptr, nullptr};
+    size_t stage_bytes[2] = {0, 0};
+    cudaStream_t host_stream = nullptr, host_in = nullptr, host_out = nullptr;   // compute, copy-in, copy-out
+    cudaEvent_t ev_in[2] = {}, ev_c[2] = {}, ev_out[2] = {};
+    size_t slot_h2d[2] = {0, 0}, slot_d2h[2] = {0, 0};
+    bool slot_busy[2] = {false, false};
     // stats of the last call
     int n_kernels = 0, n_gemm = 0, super_rows = 0, super_cols = 0;
     cudaEvent_t* phase_events = nullptr;

@@ -37,8 +37,11 @@ extern "C" opd_status_t opd_create(opd_handle_t* out, int device) {
 extern "C" opd_status_t opd_destroy(opd_handle_t h) {
     if (!h) return OPD_ERR_BAD_ARG;
     if (h->ws_owned && h->ws) cudaFree(h->ws);
-    if (h->stage) cudaFree(h->stage);
-    if (h->host_stream) cudaStreamDestroy(h->host_stream);
+    for (int s = 0; s < 2; ++s) {
+        if (h->stage[s]) cudaFree(h->stage[s]);
+        if (h->ev_in[s]) { cudaEventDestroy(h->ev_in[s]); cudaEventDestroy(h->ev_c[s]); cudaEventDestroy(h->ev_out[s]); }
+    }
+    if (h->host_stream) { cudaStreamDestroy(h->host_stream); cudaStreamDestroy(h->host_in); cudaStreamDestroy(h->host_out); }
     delete h;
     return OPD_OK;
 }

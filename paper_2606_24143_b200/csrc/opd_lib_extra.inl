@@ -39,20 +39,37 @@ extern "C" opd_status_t opd_debug_gemm(opd_handle_t h, void* cuda_stream, int M,
     return OPD_OK;
 }
 
-// ---------------------------------------------------------------- host-buffer entry point
-extern "C" opd_status_t opd_loss_fwd_bwd_host(opd_handle_t h, int T, int d, int V, opd_dtype_t dtype,
+// ---------------------------------------------------------------- host-buffer entry points
+// Two staging slots, three streams (copy-in, compute, copy-out): a caller that alternates slots overlaps the H2D copy of
+// step i+1 and the D2H copy of step i-1 with the kernels of step i.  opd_loss_fwd_bwd_host = submit + wait on slot 0.
+static opd_status_t host_streams(opd_handle_s* h) {
+    if (h->host_stream) return OPD_OK;
+    OPD_CUDA(h, cudaStreamCreateWithFlags(&h->host_stream, cudaStreamNonBlocking));
+    OPD_CUDA(h, cudaStreamCreateWithFlags(&h->host_in, cudaStreamNonBlocking));
+    OPD_CUDA(h, cudaStreamCreateWithFlags(&h->host_out, cudaStreamNonBlocking));
+    for (int s = 0; s < 2; ++s) {
+        OPD_CUDA(h, cudaEventCreateWithFlags(&h->ev_in[s], cudaEventDisableTiming));
+        OPD_CUDA(h, cudaEventCreateWithFlags(&h->ev_c[s], cudaEventDisableTiming));
+        OPD_CUDA(h, cudaEventCreateWithFlags(&h->ev_out[s], cudaEventDisableTiming));
+    }
+    return OPD_OK;
+}
+
+extern "C" opd_status_t opd_loss_fwd_bwd_host_submit(opd_handle_t h, int slot, int T, int d, int V, opd_dtype_t dtype,
     const void* hidden_h, const void* W_h, const int* idx_h, const float* lam_h, const float* old_h, const unsigned char* mask_h,
     opd_mode_t mode, int k_or_K, unsigned flags, float norm_override,
-    float* loss_h, float* ptk_h, void* gh_h, void* gw_h, size_t* h2d_bytes, size_t* d2h_bytes) {
+    float* loss_h, float* ptk_h, void* gh_h, void* gw_h) {
     if (!h) return OPD_ERR_BAD_ARG;
+    if (slot < 0 || slot > 1) OPD_FAIL(h, OPD_ERR_BAD_ARG, "slot must be 0 or 1");
+    if (h->slot_busy[slot]) OPD_FAIL(h, OPD_ERR_BAD_ARG, "slot %d is in flight: call opd_loss_fwd_bwd_host_wait first", slot);
     if (!hidden_h || !W_h || !idx_h || !lam_h || !mask_h) OPD_FAIL(h, OPD_ERR_BAD_ARG, "null host input");
     int kf, Km;
     const int C = cache_width(mode, k_or_K, &kf, &Km);
     opd_status_t s = check_shape(h, T, d, V, C);
     if (s != OPD_OK) return s;
     OPD_CUDA(h, cudaSetDevice(h->device));
-    if (!h->host_stream) OPD_CUDA(h, cudaStreamCreateWithFlags(&h->host_stream, cudaStreamNonBlocking));
-    cudaStream_t st = h->host_stream;
+    s = host_streams(h);
+    if (s != OPD_OK) return s;
     const size_t esz = dtype == OPD_FP32 ? 4 : 2;
     const bool bwd = !(flags & OPD_F_FWD_ONLY);
     size_t o = 0;
@@ -60,35 +77,63 @@ extern "C" opd_status_t opd_loss_fwd_bwd_host(opd_handle_t h, int T, int d, int 
     const size_t o_hid = take((size_t)T * d * esz), o_w = take((size_t)d * V * esz), o_idx = take((size_t)T * C * 4),
                  o_lam = take((size_t)T * C * 4), o_old = take((size_t)T * C * 4), o_mask = take(T), o_loss = take(4),
                  o_ptk = take((size_t)T * 4), o_gh = take(bwd ? (size_t)T * d * esz : 0), o_gw = take(bwd ? (size_t)d * V * 4 : 0);
-    if (h->stage_bytes < o) {
-        if (h->stage) cudaFree(h->stage);
-        h->stage = nullptr; h->stage_bytes = 0;
-        cudaError_t e = cudaMalloc(&h->stage, o);
+    if (h->stage_bytes[slot] < o) {
+        if (h->stage[slot]) cudaFree(h->stage[slot]);
+        h->stage[slot] = nullptr; h->stage_bytes[slot] = 0;
+        cudaError_t e = cudaMalloc(&h->stage[slot], o);
         if (e != cudaSuccess) OPD_FAIL(h, OPD_ERR_WORKSPACE, "cudaMalloc(%zu) for host staging failed: %s", o, cudaGetErrorString(e));
-        h->stage_bytes = o;
+        h->stage_bytes[slot] = o;
     }
-    uint8_t* sb = static_cast<uint8_t*>(h->stage);
+    uint8_t* sb = static_cast<uint8_t*>(h->stage[slot]);
     size_t up = 0, down = 0;
-    auto h2d = [&](size_t off, const void* src, size_t b) { up += b; return cudaMemcpyAsync(sb + off, src, b, cudaMemcpyHostToDevice, st); };
+    cudaStream_t sin = h->host_in, sc = h->host_stream, sout = h->host_out;
+    auto h2d = [&](size_t off, const void* src, size_t b) { up += b; return cudaMemcpyAsync(sb + off, src, b, cudaMemcpyHostToDevice, sin); };
     OPD_CUDA(h, h2d(o_hid, hidden_h, (size_t)T * d * esz));
     OPD_CUDA(h, h2d(o_w, W_h, (size_t)d * V * esz));
     OPD_CUDA(h, h2d(o_idx, idx_h, (size_t)T * C * 4));
     OPD_CUDA(h, h2d(o_lam, lam_h, (size_t)T * C * 4));
     if (old_h) OPD_CUDA(h, h2d(o_old, old_h, (size_t)T * C * 4));
     OPD_CUDA(h, h2d(o_mask, mask_h, T));
-    s = opd_loss_fwd_bwd(h, st, T, d, V, dtype, sb + o_hid, d, sb + o_w, V, 1, reinterpret_cast<int*>(sb + o_idx), C,
+    OPD_CUDA(h, cudaEventRecord(h->ev_in[slot], sin));
+    OPD_CUDA(h, cudaStreamWaitEvent(sc, h->ev_in[slot], 0));
+    s = opd_loss_fwd_bwd(h, sc, T, d, V, dtype, sb + o_hid, d, sb + o_w, V, 1, reinterpret_cast<int*>(sb + o_idx), C,
                          reinterpret_cast<float*>(sb + o_lam), old_h ? reinterpret_cast<float*>(sb + o_old) : nullptr, sb + o_mask,
                          mode, k_or_K, flags & ~OPD_F_GRADW_ACCUM, norm_override, reinterpret_cast<float*>(sb + o_loss),
                          reinterpret_cast<float*>(sb + o_ptk), nullptr, nullptr, bwd ? sb + o_gh : nullptr, d,
                          bwd ? sb + o_gw : nullptr, V, 1);
     if (s != OPD_OK) return s;
-    auto d2h = [&](void* dst, size_t off, size_t b) { down += b; return cudaMemcpyAsync(dst, sb + off, b, cudaMemcpyDeviceToHost, st); };
+    OPD_CUDA(h, cudaEventRecord(h->ev_c[slot], sc));
+    OPD_CUDA(h, cudaStreamWaitEvent(sout, h->ev_c[slot], 0));
+    auto d2h = [&](void* dst, size_t off, size_t b) { down += b; return cudaMemcpyAsync(dst, sb + off, b, cudaMemcpyDeviceToHost, sout); };
     if (loss_h) OPD_CUDA(h, d2h(loss_h, o_loss, 4));
     if (ptk_h) OPD_CUDA(h, d2h(ptk_h, o_ptk, (size_t)T * 4));
     if (bwd && gh_h) OPD_CUDA(h, d2h(gh_h, o_gh, (size_t)T * d * esz));
     if (bwd && gw_h) OPD_CUDA(h, d2h(gw_h, o_gw, (size_t)d * V * 4));
-    OPD_CUDA(h, cudaStreamSynchronize(st));
-    if (h2d_bytes) *h2d_bytes = up;
-    if (d2h_bytes) *d2h_bytes = down;
+    OPD_CUDA(h, cudaEventRecord(h->ev_out[slot], sout));
+    // the next copy-in into THIS slot must not start before these kernels have consumed it: the caller waits on the slot
+    h->slot_h2d[slot] = up; h->slot_d2h[slot] = down; h->slot_busy[slot] = true;
     return OPD_OK;
+}
+
+extern "C" opd_status_t opd_loss_fwd_bwd_host_wait(opd_handle_t h, int slot, size_t* h2d_bytes, size_t* d2h_bytes) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    if (slot < 0 || slot > 1) OPD_FAIL(h, OPD_ERR_BAD_ARG, "slot must be 0 or 1");
+    if (!h->slot_busy[slot]) OPD_FAIL(h, OPD_ERR_BAD_ARG, "nothing was submitted on slot %d", slot);
+    OPD_CUDA(h, cudaEventSynchronize(h->ev_out[slot]));
+    h->slot_busy[slot] = false;
+    if (h2d_bytes) *h2d_bytes = h->slot_h2d[slot];
+    if (d2h_bytes) *d2h_bytes = h->slot_d2h[slot];
+    return OPD_OK;
+}
+
+extern "C" opd_status_t opd_loss_fwd_bwd_host(opd_handle_t h, int T, int d, int V, opd_dtype_t dtype,
+    const void* hidden_h, const void* W_h, const int* idx_h, const float* lam_h, const float* old_h, const unsigned char* mask_h,
+    opd_mode_t mode, int k_or_K, unsigned flags, float norm_override,
+    float* loss_h, float* ptk_h, void* gh_h, void* gw_h, size_t* h2d_bytes, size_t* d2h_bytes) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    if (h->slot_busy[0]) OPD_FAIL(h, OPD_ERR_BAD_ARG, "slot 0 has a submitted call that was not waited for");
+    opd_status_t s = opd_loss_fwd_bwd_host_submit(h, 0, T, d, V, dtype, hidden_h, W_h, idx_h, lam_h, old_h, mask_h, mode, k_or_K, flags,
+                                                  norm_override, loss_h, ptk_h, gh_h, gw_h);
+    if (s != OPD_OK) return s;
+    return opd_loss_fwd_bwd_host_wait(h, 0, h2d_bytes, d2h_bytes);
 }

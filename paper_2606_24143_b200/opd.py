@@ -24,7 +24,7 @@ N_PHASES = 4
 PHASE_NAMES = ("prep", "fwd", "est", "bwd")
 
 EXPORTS = ("opd_create", "opd_destroy", "opd_last_error", "opd_version", "opd_workspace_bytes", "opd_set_workspace",
-           "opd_loss_fwd_bwd", "opd_loss_fwd_bwd_host", "opd_debug_logits", "opd_debug_gemm", "opd_last_launch_stats",
+           "opd_loss_fwd_bwd", "opd_loss_fwd_bwd_host", "opd_loss_fwd_bwd_host_submit", "opd_loss_fwd_bwd_host_wait", "opd_debug_logits", "opd_debug_gemm", "opd_last_launch_stats",
            "opd_set_phase_events", "opd_set_diagnostics", "opd_cache_workspace_bytes", "opd_cache_topk", "opd_cache_sample")
 
 _lib = None
@@ -64,6 +64,11 @@ def load_library():
                                           c_void_p, c_int, c_int, c_uint, c_float, c_void_p, c_void_p, c_void_p, c_void_p,
                                           POINTER(c_size_t), POINTER(c_size_t)]
     lib.opd_loss_fwd_bwd_host.restype = c_int
+    lib.opd_loss_fwd_bwd_host_submit.argtypes = [c_void_p, c_int, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p, c_void_p,
+                                                 c_void_p, c_void_p, c_int, c_int, c_uint, c_float, c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.opd_loss_fwd_bwd_host_submit.restype = c_int
+    lib.opd_loss_fwd_bwd_host_wait.argtypes = [c_void_p, c_int, POINTER(c_size_t), POINTER(c_size_t)]
+    lib.opd_loss_fwd_bwd_host_wait.restype = c_int
     lib.opd_debug_logits.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_long, c_void_p, c_long, c_long,
                                      c_void_p, c_long, c_int, c_void_p, c_void_p]
     lib.opd_debug_logits.restype = c_int
@@ -223,6 +228,26 @@ class Handle:
         self._check(st)
         out["h2d_bytes"], out["d2h_bytes"] = up.value, down.value
         return out
+
+    def host_submit(self, slot, hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K, out, flags=0,
+                    norm_override=0.0):
+        """opd_loss_fwd_bwd_host_submit: enqueue one step on staging slot 0/1 (host tensors; `out` = dict of host tensors
+        loss, per_token_kl, grad_hidden, grad_W that receive the results once host_wait(slot) has returned)."""
+        T, d = hidden.shape
+        V = W.shape[1]
+        self._pending = getattr(self, "_pending", {})
+        self._pending[slot] = (hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, out)     # keep alive
+        self._check(self.lib.opd_loss_fwd_bwd_host_submit(
+            self._h, slot, T, d, V, _dtype_code(hidden), _ptr(hidden), _ptr(W), _ptr(cache_idx), _ptr(cache_teacher_logp),
+            _ptr(cache_old_logp), _ptr(mask), mode, k_or_K, flags, float(norm_override), _ptr(out["loss"]),
+            _ptr(out["per_token_kl"]), _ptr(out.get("grad_hidden")), _ptr(out.get("grad_W"))))
+
+    def host_wait(self, slot):
+        """opd_loss_fwd_bwd_host_wait -> (out dict of the step submitted on `slot`, h2d bytes, d2h bytes)."""
+        up, down = c_size_t(), c_size_t()
+        self._check(self.lib.opd_loss_fwd_bwd_host_wait(self._h, slot, ctypes.byref(up), ctypes.byref(down)))
+        out = self._pending.pop(slot)[-1]
+        return out, up.value, down.value
 
     # ------------------------------------------------------------------ cache producers
     def cache_topk(self, hidden, W, k):

@@ -232,3 +232,36 @@ def test_mc_diagnostics_outputs(handle, opd):
     v = f64(var1)
     assert np.abs(v - ref["var1"]).max() <= 1e-3 * max(1e-30, np.abs(ref["var1"]).max())
     assert np.all(v[f64(m) != 2] == 0)
+
+
+def test_pipelined_host_entry(handle, opd):
+    """opd_loss_fwd_bwd_host_submit / _wait: two steps in flight on the two staging slots give the results of the
+    synchronous call; a busy slot refuses a second submit; waiting on an idle slot is an error."""
+    cfg = RAGGED
+    hosts, refs = [], []
+    for c in (12, 13, 14):
+        inp = synth.make_inputs(cfg, c=c, device=DEV)
+        idx, lam, old, kk = pick(inp, cfg, O.RKL_MC)
+        r = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], O.RKL_MC, kk)
+        torch.cuda.synchronize()
+        refs.append({k: r[k].cpu() for k in ("loss", "per_token_kl", "grad_hidden", "grad_W")})
+        hosts.append([t.cpu().pin_memory() for t in (inp["hidden"], inp["W"], idx, lam, old, inp["mask"])] + [kk])
+    T, d, V = cfg["T"], cfg["d"], cfg["V"]
+    new_out = lambda: dict(loss=torch.empty(1).pin_memory(), per_token_kl=torch.empty(T).pin_memory(),
+                           grad_hidden=torch.empty(T, d, dtype=torch.bfloat16).pin_memory(), grad_W=torch.empty(d, V).pin_memory())
+    outs = [new_out() for _ in range(3)]
+    sub = lambda i: handle.host_submit(i % 2, *hosts[i][:6], O.RKL_MC, hosts[i][6], outs[i])
+    sub(0); sub(1)
+    with pytest.raises(opd.OpdError):
+        sub(2)                                              # slot 0 is still in flight
+    o0, up, down = handle.host_wait(0)
+    sub(2)
+    handle.host_wait(1); handle.host_wait(0)
+    with pytest.raises(opd.OpdError):
+        handle.host_wait(1)
+    assert up > 0 and down > 0
+    for i in range(3):
+        assert abs(outs[i]["loss"].item() - refs[i]["loss"].item()) <= 1e-6
+        assert torch.equal(outs[i]["per_token_kl"], refs[i]["per_token_kl"])
+        check_grad(f64(outs[i]["grad_hidden"]), f64(refs[i]["grad_hidden"]), "bf16")
+        check_grad(f64(outs[i]["grad_W"]), f64(refs[i]["grad_W"]), "bf16")
