@@ -72,8 +72,11 @@ const char* opd_version(void);
 /* workspace ------------------------------------------------------------------------------------
  * Bytes of device scratch one opd_loss_fwd_bwd call with these arguments needs. No buffer of size
  * O(T*V) exists: the largest items are the compacted copy of hidden (T*d), the per-tile (max,sumexp)
- * partials (T*ceil(V/256)*8 B) and a bounded super-tile of re-formed softmax gradients G
- * (<= 32 MiB per operand plane) that lives in L2 between the three backward contractions. */
+ * partials (T*ceil(V/256)*8 B) and, aliased with them, a two-deep ring of bounded super-tiles of re-formed softmax
+ * gradients G (4608 x 4096 bf16 each) plus fp32 grad_hidden partial sums of one token super-tile, consumed out of L2 by
+ * the backward contractions (C4: 431 MB in total, 4.3% of the bf16 logits). The modes whose gradient is purely sparse
+ * (OPD_RKL_TOPK; OPD_FKL_TOPK with OPD_F_RENORM_STUDENT) instead need 6*d*V bytes for [V,d] transposes when W is
+ * stored [d,V]. */
 size_t opd_workspace_bytes(int T, int d, int V, int C, opd_dtype_t dtype, opd_mode_t mode, unsigned flags);
 /* Optional: use caller memory (256-byte aligned) instead of the handle's own allocation. */
 opd_status_t opd_set_workspace(opd_handle_t h, void* ws, size_t bytes);

@@ -1,5 +1,5 @@
-// Tile epilogues of the OPD path.  Each runs on the 4 epilogue warps of gemm_kernel: thread = one
-// row of the 128x256 fp32 accumulator tile, read from TMEM in 8 chunks of 32 columns.
+// Tile epilogues of the OPD path.  Each runs on the 4 epilogue warps of a CTA: thread = one row of the CTA's
+// 128 x 256 fp32 accumulator (half of a pair's 256 x 256 tile), read from TMEM in 8 chunks of 32 columns.
 //   FwdEpi   z tile -> per-row (max, sum exp) partial of the tile + gather of the cached columns   (S2, S3)
 //   GEpi     z tile -> G = (1/N)(alpha p + sum_j beta_j e_{a_j}) as bf16 into the L2-resident super-tile (S6)
 //   DxEpi    grad_hidden super-tile accumulate / emit                                               (S7)

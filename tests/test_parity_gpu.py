@@ -265,3 +265,27 @@ def test_pipelined_host_entry(handle, opd):
         assert torch.equal(outs[i]["per_token_kl"], refs[i]["per_token_kl"])
         check_grad(f64(outs[i]["grad_hidden"]), f64(refs[i]["grad_hidden"]), "bf16")
         check_grad(f64(outs[i]["grad_W"]), f64(refs[i]["grad_W"]), "bf16")
+
+
+def test_call_is_cuda_graph_capturable(handle):
+    """opd_loss_fwd_bwd only enqueues work on the caller's stream (no allocation once the workspace exists, no sync):
+    it can be captured into a CUDA graph and replayed; the replay reproduces the eager result on new input values."""
+    cfg = dict(RAGGED, T=512)
+    inp = synth.make_inputs(cfg, c=15, device=DEV)
+    idx, lam, old, kk = pick(inp, cfg, O.RKL_MC)
+    X = inp["hidden"].clone()
+    gh, gw = torch.empty_like(X), torch.empty(cfg["d"], cfg["V"], device=DEV)
+    handle.loss_fwd_bwd(X, inp["W"], idx, lam, old, inp["mask"], O.RKL_MC, kk, grad_hidden=gh, grad_W=gw)   # sizes the workspace
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        r = handle.loss_fwd_bwd(X, inp["W"], idx, lam, old, inp["mask"], O.RKL_MC, kk, grad_hidden=gh, grad_W=gw)
+    X.copy_(inp["hidden"].flip(0))                        # new values in the captured input buffer
+    g.replay()
+    torch.cuda.synchronize()
+    loss_g, gh_g, gw_g = r["loss"].clone(), gh.clone(), gw.clone()
+    e = handle.loss_fwd_bwd(X, inp["W"], idx, lam, old, inp["mask"], O.RKL_MC, kk)
+    torch.cuda.synchronize()
+    assert abs(loss_g.item() - e["loss"].item()) <= 1e-6 * abs(e["loss"].item())
+    check_grad(f64(gh_g), f64(e["grad_hidden"]), "bf16")
+    check_grad(f64(gw_g), f64(e["grad_W"]), "bf16")
