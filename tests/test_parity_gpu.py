@@ -289,3 +289,20 @@ def test_call_is_cuda_graph_capturable(handle):
     assert abs(loss_g.item() - e["loss"].item()) <= 1e-6 * abs(e["loss"].item())
     check_grad(f64(gh_g), f64(e["grad_hidden"]), "bf16")
     check_grad(f64(gw_g), f64(e["grad_W"]), "bf16")
+
+
+@pytest.mark.parametrize("knobs", [dict(OPD_CTA_GROUP="1"), dict(OPD_G_BUFS="3", OPD_TB="256", OPD_VB="256"),
+                                   dict(OPD_GROUP_M="3", OPD_HINT_GW="1", OPD_HINT_G="2")])
+def test_tuning_knobs_do_not_change_results(handle, knobs, monkeypatch):
+    """The single-CTA tile configuration, a 3-deep G ring with the smallest super-tiles, another raster group and L2
+    hints give the same outputs as the defaults (within summation-order noise) and match the oracle."""
+    cfg = RAGGED
+    inp = synth.make_inputs(cfg, c=16, device=DEV)
+    idx, lam, old, kk = pick(inp, cfg, O.RKL_MC)
+    base = run(handle, inp, idx, lam, old, O.RKL_MC, kk)
+    for k, v in knobs.items():
+        monkeypatch.setenv(k, v)
+    r = run(handle, inp, idx, lam, old, O.RKL_MC, kk)
+    compare_all(r, oracle_for(inp, idx, lam, old, O.RKL_MC, kk), f64(inp["mask"]), "bf16")
+    assert abs(r["loss"].item() - base["loss"].item()) <= 1e-6
+    assert torch.equal(r["student_logp"].nan_to_num(), base["student_logp"].nan_to_num())
