@@ -306,3 +306,24 @@ def test_tuning_knobs_do_not_change_results(handle, knobs, monkeypatch):
     compare_all(r, oracle_for(inp, idx, lam, old, O.RKL_MC, kk), f64(inp["mask"]), "bf16")
     assert abs(r["loss"].item() - base["loss"].item()) <= 1e-6
     assert torch.equal(r["student_logp"].nan_to_num(), base["student_logp"].nan_to_num())
+
+
+def test_autograd_entry(handle):
+    """opd_loss(...).backward() on a [V,d] lm_head parameter (transposed view used in place) against the oracle."""
+    from paper_2606_24143_b200.autograd import opd_loss
+    cfg = dict(RAGGED, T=384)
+    inp = synth.make_inputs(cfg, c=17, device=DEV)
+    idx, lam, old, kk = pick(inp, cfg, O.RKL_MC)
+    hidden = inp["hidden"].clone().requires_grad_(True)
+    weight = inp["W"].t().contiguous().requires_grad_(True)               # [V,d] like nn.Linear(d, V).weight
+    loss, ptk = opd_loss(hidden, weight.t(), idx, lam, old, inp["mask"], O.RKL_MC, kk, return_per_token=True)
+    (2.0 * loss).backward()
+    torch.cuda.synchronize()
+    ref = oracle_for(inp, idx, lam, old, O.RKL_MC, kk)
+    check_loss(loss.item(), ref)
+    assert weight.grad.shape == weight.shape and weight.grad.dtype == weight.dtype
+    check_grad(f64(hidden.grad), 2.0 * ref["grad_hidden"], "bf16")
+    check_grad(f64(weight.grad).T, 2.0 * ref["grad_W"], "bf16")
+    with torch.no_grad():
+        l2 = opd_loss(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], O.RKL_MC, kk)
+    assert abs(l2.item() - loss.item()) <= 1e-6
