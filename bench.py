@@ -182,7 +182,21 @@ def run_producer_bench(args, h, inp, cfg, dev, world, rank, dist):
     u = torch.rand(T, n, device=dev, generator=torch.Generator(device=dev).manual_seed(1)) if args.op == "sample" else None
     # the scoring model's head: an independent seeded matrix of the same shape (synth keeps only W resident)
     Wt = inp["W"]
-    call = (lambda: h.cache_topk(inp["hidden"], Wt, n)) if args.op == "topk" else (lambda: h.cache_sample(inp["hidden"], Wt, u))
+    flops = 4.0 * d * V * T
+    n_tok = T
+    if args.op == "dense":      # dense two-head forward KL: teacher hidden states and head of the student's shapes (dT = d)
+        g = torch.Generator(device=dev).manual_seed(2)
+        th = torch.randn(T, d, device=dev, generator=g).to(inp["hidden"].dtype)
+        wt = (torch.randn(d, V, device=dev, generator=g) * d ** -0.5).to(inp["W"].dtype)
+        gh = torch.empty_like(inp["hidden"]); gw = torch.empty(d, V, dtype=torch.float32, device=dev)
+        call = lambda: h.dense_kl_fwd_bwd(inp["hidden"], inp["W"], th, wt, inp["mask"], grad_hidden=gh, grad_W=gw)
+        n_tok = int((inp["mask"] != 0).sum().item())
+        flops = 12.0 * d * V * n_tok    # two forward heads, Q and G re-formation, grad_hidden, grad_W: 2 d V each
+        n = 0
+    elif args.op == "topk":
+        call = lambda: h.cache_topk(inp["hidden"], Wt, n)
+    else:
+        call = lambda: h.cache_sample(inp["hidden"], Wt, u)
     for _ in range(max(args.warmup, 3)):
         call()
     torch.cuda.synchronize()
@@ -208,17 +222,20 @@ def run_producer_bench(args, h, inp, cfg, dev, world, rank, dist):
         return
     ms = total_ms / args.steps
     pk = peaks()
-    ach = 4.0 * d * V * T / (ms * 1e-3) / 1e12
+    ach = flops / (ms * 1e-3) / 1e12
     st = h.launch_stats()
-    line = dict(metric=f"cache producer ({args.op}) tokens scored/s on 1 B200", value=T * world / (ms * 1e-3), unit="tokens/s", n_gpus=world,
+    line = dict(metric=(f"cache producer ({args.op}) tokens scored/s on 1 B200" if args.op != "dense" else
+                        "dense two-head forward KL fwd+bwd tokens/s on 1 B200"), value=n_tok * world / (ms * 1e-3), unit="live tokens/s" if args.op == "dense" else "tokens/s", n_gpus=world,
                 steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="bf16" if cfg["dtype"] == "bf16" else "f32(3xbf16)", data="synthetic",
-                config=dict(workload=f"{cfg['name']} opd_cache_{args.op} n={n}", T=T, d=d, V=V,
+                config=dict(workload=(f"{cfg['name']} opd_cache_{args.op} n={n}" if args.op != "dense" else f"{cfg['name']} opd_dense_kl_fwd_bwd dT=d"),
+                            T=T, d=d, V=V,
                             l2_policy="inputs larger than L2 (W alone is %.0f MB)" % (d * V * 2 / 1e6)),
                 clocks=clocks, e2e=None, gpu_launches=st["kernels"] * args.steps,
                 roofline=dict(bound="tensor", achieved=ach, peak=pk["sustained"], unit="TFLOP/s", frac=ach / pk["sustained"], traffic=None,
-                              kernel="opd::gemm_kernel<FwdEpi,2> + opd::gemm_kernel<%s,2>" % ("CollectEpi" if args.op == "topk" else "SampleEpi"),
-                              flops_per_step=4.0 * d * V * T, frac_of_burst=ach / pk["burst"]),
+                              kernel=("opd::gemm_kernel<FwdEpi,2> + opd::gemm_kernel<%s,2>" % ("CollectEpi" if args.op == "topk" else "SampleEpi")
+                                      if args.op != "dense" else "2 x opd::gemm_kernel<FwdEpi,2> + opd::bwd_kernel<2,true>"),
+                              flops_per_step=flops, frac_of_burst=ach / pk["burst"]),
                 cpu_baseline=None)
     print(json.dumps(line), flush=True)
 
@@ -231,7 +248,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1..5); 4 = the config the metric is quoted on")
     ap.add_argument("--mode", default=None, choices=["fkl", "mc", "mixed", "rtopk"])
-    ap.add_argument("--op", default="loss", choices=["loss", "topk", "sample"],
+    ap.add_argument("--op", default="loss", choices=["loss", "topk", "sample", "dense"],
                     help="loss = the hot path (default, the contract's line); topk / sample = the cache producers (NEXT-3)")
     ap.add_argument("--tokens", type=int, default=0, help="override T (debugging)")
     ap.add_argument("--sigma", type=float, default=None, help="staleness of the rollout policy: W_old = W + sigma*N(0,1/d)")

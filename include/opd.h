@@ -168,6 +168,23 @@ opd_status_t opd_cache_sample(opd_handle_t h, void* cuda_stream, int T, int d, i
     const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, int K, const float* uniforms, long ld_u,
     int* idx_out, long ld_idx, float* logp_out, long ld_logp, float* lse_out);
 
+/* dense two-head KL -------------------------------------------------------------------------------
+ * Dense full-vocabulary forward KL with the teacher's distribution recomputed from TRANSMITTED TEACHER HIDDEN STATES
+ * (the direction the paper names as future work; objective and gradient: Eq.(1)):
+ *     q_t = softmax(teacher_hidden_t . W_T),  p_t = softmax(hidden_t . W),
+ *     per_token_kl[t] = sum_v q_tv (log q_tv - log p_tv),   loss = (1/N) sum over live tokens,   dL_t/dz_tv = p_tv - q_tv.
+ * Both heads are streamed tile by tile; neither set of logits is stored (bounded L2-resident rings of q and of the
+ * gradient tiles only). teacher_hidden [T,dT] (row stride ld_th) and W_T (logical [dT,V], strides ldt_k / ldt_v, either
+ * storage order) have the dtype of hidden / W; dT % 64 == 0. mask [T]: 0 = masked. flags: OPD_F_GRADW_ACCUM,
+ * OPD_F_FWD_ONLY. With bf16 inputs q is rounded to bf16 before use (in the loss AND the gradient, consistently).
+ * Other arguments and outputs as for opd_loss_fwd_bwd. */
+size_t opd_dense_kl_workspace_bytes(int T, int d, int dT, int V, opd_dtype_t dtype, unsigned flags);
+opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, int T, int d, int dT, int V, opd_dtype_t dtype,
+    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v,
+    const void* teacher_hidden, long ld_th, const void* W_T, long ldt_k, long ldt_v,
+    const unsigned char* mask, unsigned flags, float norm_override,
+    float* loss, float* per_token_kl, void* grad_hidden, long ld_gh, void* grad_W, long ldgw_k, long ldgw_v);
+
 /* Optional per-token diagnostics of the MC estimator, written by the following opd_loss_fwd_bwd calls on this
  * handle (device pointers, caller-owned; pass NULLs to switch off):
  *   rho_out [T, ld_rho]  rho_theta(a_tj) = p_theta(a_tj|s_t) / p_old(a_tj|s_t) of every cached draw of a live RKL_MC row

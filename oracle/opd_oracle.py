@@ -403,3 +403,40 @@ def cache_sample(hidden, W, uniforms):
     for t in range(T):
         idx[t] = np.minimum(np.searchsorted(cdf[t], u[t] * cdf[t, -1], side="left"), cdf.shape[1] - 1)
     return idx, np.take_along_axis(logp, idx, 1), lse, cdf
+
+
+# ------------------------------------------------------------------------------------------------
+# Dense two-head forward KL: the teacher's distribution recomputed from transmitted teacher
+# hidden states (the direction PAPER.md:240 names as future work), objective Eq.(1), gradient PAPER.md:59.
+def dense_kl_oracle(hidden, W, teacher_hidden, W_T, mask, norm_override: float = 0.0, q_round=None, chunk: int = 512):
+    """q_t = softmax(h^T_t . W_T), p_t = softmax(x_t . W);  L_t = sum_v q_tv (log q_tv - log p_tv)  (Eq.(1));
+    loss = (1/N) sum_t m_t L_t;  dL_t/dz_tv = (sum_v q_tv) p_tv - q_tv  (= p - q, PAPER.md:59);
+    grad_hidden / grad_W by the chain rule (O8, O9).  ``q_round``: optional function applied to q before it is used
+    (the bf16 CUDA path rounds q to bf16 — the tests compare against both the exact and the rounded definition).
+    Returns dict(loss, N, per_token_kl[T], grad_hidden[T,d], grad_W[d,V])."""
+    X = np.asarray(hidden, dtype=np.float64)
+    Wd = np.asarray(W, dtype=np.float64)
+    XT = np.asarray(teacher_hidden, dtype=np.float64)
+    WT = np.asarray(W_T, dtype=np.float64)
+    msk = np.asarray(mask).astype(np.int64)
+    T, d = X.shape
+    V = Wd.shape[1]
+    N = float(np.count_nonzero(msk))
+    norm = float(norm_override) if norm_override > 0 else N
+    scale = 0.0 if norm == 0 else 1.0 / norm
+    per_token = np.zeros(T)
+    gh = np.zeros((T, d))
+    gW = np.zeros((d, V))
+    live = np.flatnonzero(msk)
+    for s in range(0, live.size, chunk):
+        tt = live[s:s + chunk]
+        logp, _ = log_softmax_rows(X[tt] @ Wd)
+        logq, _ = log_softmax_rows(XT[tt] @ WT)
+        q = np.exp(logq)
+        if q_round is not None:
+            q = q_round(q)
+        per_token[tt] = np.sum(q * (logq - logp), axis=1)
+        G = (np.sum(q, axis=1, keepdims=True) * np.exp(logp) - q) * scale
+        gh[tt] = G @ Wd.T
+        gW += X[tt].T @ G
+    return dict(loss=float(np.sum(per_token)) * scale, N=N, per_token_kl=per_token, grad_hidden=gh, grad_W=gW)

@@ -13,7 +13,7 @@
 //   c_done[s-R] complete       before a G(s) epilogue overwrites ring buffer s%R (previous readers; R = ring depth)
 // This removes the ~900 launches, their partial last waves and the pipeline refill of the per-GEMM version.
 #pragma once
-#include "opd_epilogues_bwd.cuh"
+#include "opd_dense.cuh"
 
 namespace opd {
 
@@ -25,21 +25,32 @@ struct BwdParams {
     const int* n_live;
     int* g_done;               // [S]
     int* c_done;               // [S]
-    int type_mask;             // timing experiments only: bit t set = run tiles of type t (7 = all; else no dependency waits)
+    int type_mask;             // bit t set = run tiles of type t.  All types of the variant = the normal run; a tile waits
+                               // on a counter only if every tile type that increments it is enabled (dense forward-only
+                               // runs Q + G; other subsets are timing experiments and give wrong gradients)
     unsigned long long hint_x, hint_w, hint_g;   // L2 eviction policies of the Xc / W / G-ring operand loads
     GEpi::Params g;            // gs points at ring buffer 0; buffer b at + b * planes * plane_stride
     DxEpi::Params dx;
     DwEpi::Params dw;
+    // dense two-head variant (opd_dense.cuh): teacher contraction depth / layout, Q ring and its counter
+    int dT, wl_t, qbytes;      // qbytes: element size of the Q ring (2 bf16, 4 fp32)
+    int* q_done;               // [S]
+    QEpi::Params q;            // qs points at Q ring buffer 0; buffer b at + b * q_buf_bytes
+    size_t q_buf_bytes;
+    GDenseEpi::Params gd;
 };
 
-enum { T_G = 0, T_DX = 1, T_DW = 2 };
+enum { T_G = 0, T_DX = 1, T_DW = 2, T_Q = 3 };
 
 struct BwdTile {
     int type, s, tb0, vb0, Tb_eff, Vb_eff, vi, m_blk, n_blk;
 };
 
-template <int CG>
+// DENSE: block b holds Q(b), G(b-1), DX(b-2), DW(b-2) (the Q tiles of a super-tile run one block ahead of its G tiles);
+// otherwise block b holds G(b), DX(b-1), DW(b-1).
+template <int CG, bool DENSE>
 struct BwdSched {
+    static constexpr int GOFF = DENSE ? 1 : 0;
     static constexpr int TM = Cfg<CG>::TILE_M;
     int S, nvb, Tb, Vb, V, d, wl, n_live;
     int blk;        // current block
@@ -65,22 +76,31 @@ struct BwdSched {
         return wl == 0 ? ((d + TM - 1) / TM) * nt : ((b + TM - 1) / TM) * ((d + BN - 1) / BN);
     }
     __device__ __forceinline__ int block_size(int b) const {
-        return (b < S ? nG(b) : 0) + (b >= 1 ? nDX(b - 1) + nDW(b - 1) : 0);
+        const int g = b - GOFF, c = b - GOFF - 1;
+        return (DENSE && b < S ? nG(b) : 0) + (g >= 0 && g < S ? nG(g) : 0) + (c >= 0 && c < S ? nDX(c) + nDW(c) : 0);
     }
     // decode `item` (monotonically increasing between calls); false when the list is exhausted
     __device__ __forceinline__ bool get(long item, BwdTile& t) {
-        while (blk <= S) {
+        while (blk <= S + GOFF) {
             const int sz = block_size(blk);
             if (item < base + sz) break;
             base += sz; ++blk;
         }
-        if (blk > S) return false;
+        if (blk > S + GOFF) return false;
         int r = static_cast<int>(item - base);
         int rows;
-        if (blk < S && r < nG(blk)) { t.type = T_G; t.s = blk; }
-        else {
-            if (blk < S) r -= nG(blk);
-            t.s = blk - 1;
+        const int g = blk - GOFF;
+        t.type = -1;
+        if (DENSE && blk < S) {
+            const int nq = nG(blk);
+            if (r < nq) { t.type = T_Q; t.s = blk; } else r -= nq;
+        }
+        if (t.type < 0 && g >= 0 && g < S) {
+            const int ng = nG(g);
+            if (r < ng) { t.type = T_G; t.s = g; } else r -= ng;
+        }
+        if (t.type < 0) {
+            t.s = g - 1;
             const int ndx = nDX(t.s);
             if (r < ndx) t.type = T_DX; else { t.type = T_DW; r -= ndx; }
         }
@@ -107,11 +127,14 @@ __device__ __forceinline__ void wait_counter(const int* c, int expected) {
 __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
 // Counters count CTA-level epilogues: a tile of a CTA pair (CG = 2) contributes 2.
-template <int CG>
+// DENSE adds the teacher-head Q tiles of the dense two-head KL (opd_dense.cuh); m_tx_k / m_wt_fwd are then the teacher's
+// compacted hidden states and head (unused copies of the student's maps otherwise).
+template <int CG, bool DENSE>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ CUtensorMap m_w_fwd,
            const __grid_constant__ CUtensorMap m_gs_k, const __grid_constant__ CUtensorMap m_w_dx,
            const __grid_constant__ CUtensorMap m_xc_mn, const __grid_constant__ CUtensorMap m_gs_mn,
+           const __grid_constant__ CUtensorMap m_tx_k, const __grid_constant__ CUtensorMap m_wt_fwd,
            const __grid_constant__ BwdParams bp) {
     using C = Cfg<CG>;
     extern __shared__ uint8_t smem_raw[];
@@ -123,10 +146,13 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
     if (warp == 0 && lane == 0) {
         prefetch_tmap(&m_xc_k); prefetch_tmap(&m_w_fwd); prefetch_tmap(&m_gs_k);
         prefetch_tmap(&m_w_dx); prefetch_tmap(&m_xc_mn); prefetch_tmap(&m_gs_mn);
+        if constexpr (DENSE) { prefetch_tmap(&m_tx_k); prefetch_tmap(&m_wt_fwd); }
     }
     Pipe<CG> P;
     P.setup(smem_raw, warp, lane);
     const int rank = static_cast<int>(P.rank);
+    const int mask = bp.type_mask;
+    auto on = [mask](int type) { return ((mask >> type) & 1) != 0; };
 
     // segment tables of the three-term split (planes == 3), see set_segments()
     const int nseg = bp.planes == 1 ? 1 : 6;
@@ -136,11 +162,11 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
     if (warp == 0) {
         // =========================== TMA producer ===========================
         if (elect_one()) {
-            BwdSched<CG> sc; sc.init(bp);
+            BwdSched<CG, DENSE> sc; sc.init(bp);
             BwdTile t;
             int it = 0;
             for (long item = first_item; sc.get(item, t); item += item_step) {
-                if (!((bp.type_mask >> t.type) & 1)) continue;
+                if (!on(t.type)) continue;
                 TileOp op;
                 int pa_off = 0, pb_off = 0;
                 const int buf = t.s % bp.gbufs;
@@ -148,6 +174,10 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 if (t.type == T_G) {
                     op.tA = &m_xc_k; op.tB = &m_w_fwd; op.a_mn = 0; op.b_mn = (bp.wl == 0);
                     op.a_c = t.tb0 + a_row; op.b_c = t.vb0 + b_row; op.ka = 0; op.kb = 0; op.K = bp.d;
+                    op.a_hint = bp.hint_x; op.b_hint = bp.hint_w;
+                } else if (DENSE && t.type == T_Q) {
+                    op.tA = &m_tx_k; op.tB = &m_wt_fwd; op.a_mn = 0; op.b_mn = (bp.wl_t == 0);
+                    op.a_c = t.tb0 + a_row; op.b_c = t.vb0 + b_row; op.ka = 0; op.kb = 0; op.K = bp.dT;
                     op.a_hint = bp.hint_x; op.b_hint = bp.hint_w;
                 } else if (t.type == T_DX) {
                     op.tA = &m_gs_k; op.tB = &m_w_dx; op.a_mn = 0; op.b_mn = (bp.wl == 1);
@@ -167,7 +197,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                     op.pa[i] = static_cast<unsigned char>(pa_off + (nseg == 1 ? 0 : PA[i]));
                     op.pb[i] = static_cast<unsigned char>(pb_off + (nseg == 1 ? 0 : PB[i]));
                 }
-                if (t.type != T_G && bp.type_mask == 7) {   // the G super-tile must be complete before TMA reads it
+                if ((t.type == T_DX || t.type == T_DW) && on(T_G)) {   // the G super-tile must be complete before TMA reads it
                     wait_counter(bp.g_done + t.s, CG * sc.nG(t.s));
                     fence_proxy_async_all();
                 }
@@ -177,13 +207,14 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
     } else if (warp == 1) {
         // =========================== MMA issuer ===========================
         if (rank == 0 && elect_one()) {
-            BwdSched<CG> sc; sc.init(bp);
+            BwdSched<CG, DENSE> sc; sc.init(bp);
             BwdTile t;
             int it = 0, lt = 0;
             for (long item = first_item; sc.get(item, t); item += item_step) {
-                if (!((bp.type_mask >> t.type) & 1)) continue;
+                if (!on(t.type)) continue;
                 int a_mn, b_mn, K;
                 if (t.type == T_G) { a_mn = 0; b_mn = (bp.wl == 0); K = bp.d; }
+                else if (DENSE && t.type == T_Q) { a_mn = 0; b_mn = (bp.wl_t == 0); K = bp.dT; }
                 else if (t.type == T_DX) { a_mn = 0; b_mn = (bp.wl == 1); K = t.Vb_eff; }
                 else { a_mn = 1; b_mn = 1; K = t.Tb_eff; }
                 mma_tile<CG>(P, a_mn, b_mn, ((K + BK - 1) / BK) * nseg, lt, it);
@@ -195,21 +226,43 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
         const int quarter = warp & 3;
         const int row_in_tile = quarter * 32 + lane;
         const int epi_tid = (warp - 2) * 32 + lane;
-        BwdSched<CG> sc; sc.init(bp);
+        BwdSched<CG, DENSE> sc; sc.init(bp);
         BwdTile t;
         int lt = 0;
+        auto wait_for = [&](const int* counter, int expected) {      // warp-level acquire of a dependency counter
+            if (lane == 0) { wait_counter(counter, expected); fence_proxy_async_all(); }
+            __syncwarp();
+        };
         for (long item = first_item; sc.get(item, t); item += item_step) {
-            if (!((bp.type_mask >> t.type) & 1)) continue;
+            if (!on(t.type)) continue;
             const int m_blk = t.m_blk * CG + rank;    // this CTA's 128-row block inside the GEMM
             GemmParams gp{};                      // the fields the epilogues read
             gp.tok_off = t.tb0;
-            // wait for the previous writer / readers of what this epilogue is about to write
-            const int dep = (t.type == T_G) ? t.s - bp.gbufs : t.s - 1;
-            if (dep >= 0 && bp.type_mask == 7) {
-                if (lane == 0) { wait_counter(bp.c_done + dep, CG * (sc.nDX(dep) + sc.nDW(dep))); fence_proxy_async_all(); }
-                __syncwarp();
+            // wait for the previous writer / readers of what this epilogue is about to write (and, dense, for its Q tile)
+            if (t.type == T_Q) {
+                if (t.s >= 2 && on(T_G)) wait_for(bp.g_done + t.s - 2, CG * sc.nG(t.s - 2));
+            } else {
+                const int dep = (t.type == T_G) ? t.s - bp.gbufs : t.s - 1;
+                if (dep >= 0 && on(T_DX) && on(T_DW)) wait_for(bp.c_done + dep, CG * (sc.nDX(dep) + sc.nDW(dep)));
+                if (DENSE && t.type == T_G && on(T_Q)) wait_for(bp.q_done + t.s, CG * sc.nG(t.s));
             }
-            if (t.type == T_G) {
+            if (DENSE && t.type == T_Q) {
+                gp.b_off = t.vb0; gp.N = t.Vb_eff;
+                QEpi::Params ep = bp.q;
+                ep.qs = static_cast<uint8_t*>(ep.qs) + static_cast<size_t>(t.s & 1) * bp.q_buf_bytes;
+                QEpi::State st = QEpi::prepare(ep, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
+                const uint32_t taddr = epi_acquire<CG>(P, lt, quarter);
+                QEpi::run(ep, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, nullptr, epi_tid);
+            } else if (DENSE && t.type == T_G) {
+                gp.b_off = t.vb0; gp.N = t.Vb_eff;
+                GDenseEpi::Params ep = bp.gd;
+                ep.gs += static_cast<size_t>(t.s % bp.gbufs) * bp.planes * ep.plane_stride;
+                ep.qs = static_cast<const uint8_t*>(ep.qs) + static_cast<size_t>(t.s & 1) * bp.q_buf_bytes;
+                if (!on(T_DX)) ep.rows = 0;                     // forward-only: nothing consumes G
+                GDenseEpi::State st = GDenseEpi::prepare(ep, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
+                const uint32_t taddr = epi_acquire<CG>(P, lt, quarter);
+                GDenseEpi::run(ep, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, nullptr, epi_tid);
+            } else if (t.type == T_G) {
                 gp.b_off = t.vb0; gp.N = t.Vb_eff;
                 GEpi::Params ep = bp.g;
                 ep.gs += static_cast<size_t>(t.s % bp.gbufs) * bp.planes * ep.plane_stride;
@@ -234,7 +287,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             __threadfence();
             fence_proxy_async_all();
             asm volatile("bar.sync 1, 128;" ::: "memory");
-            if (epi_tid == 0) atomicAdd((t.type == T_G ? bp.g_done : bp.c_done) + t.s, 1);
+            if (epi_tid == 0) atomicAdd((t.type == T_G ? bp.g_done : (t.type == T_Q ? bp.q_done : bp.c_done)) + t.s, 1);
         }
     }
     P.teardown(warp);

@@ -113,3 +113,4 @@ extern "C" opd_status_t opd_set_diagnostics(opd_handle_t h, float* rho_out, long
 #include "opd_lib_path.inl"
 #include "opd_lib_extra.inl"
 #include "opd_lib_producer.inl"
+#include "opd_lib_dense.inl"

@@ -16,6 +16,23 @@ struct PathIO {
     float* dbg_logits; float* dbg_gathered; bool stop_after_fwd; bool all_live;
 };
 
+// Launch the persistent backward kernel on as many CTAs (pairs) as can be resident at once: its tiles wait on tiles of
+// other CTAs through counters in global memory, so every CTA of the grid must be running.
+template <bool DENSE>
+static opd_status_t launch_bwd(opd_handle_s* h, cudaStream_t st, const CUtensorMap& m_xc_k, const CUtensorMap& m_w_fwd,
+                               const CUtensorMap& m_gs_k, const CUtensorMap& m_w_dx, const CUtensorMap& m_xc_mn,
+                               const CUtensorMap& m_gs_mn, const CUtensorMap& m_tx_k, const CUtensorMap& m_wt_fwd, const BwdParams& bp) {
+    static int resident[3] = {0, -1, -1};
+    if (resident[h->cg] < 0)
+        resident[h->cg] = h->cg == 2 ? max_resident_groups<2>(bwd_kernel<2, DENSE>, h->num_sms)
+                                     : max_resident_groups<1>(bwd_kernel<1, DENSE>, h->num_sms);
+    if (resident[h->cg] < 1) OPD_FAIL(h, OPD_ERR_CUDA, "the backward kernel cannot be made resident on device %d", h->device);
+    const int grid = resident[h->cg] * h->cg;
+    if (h->cg == 2) OPD_CUDA(h, launch_cg<2>(bwd_kernel<2, DENSE>, grid, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
+    else OPD_CUDA(h, launch_cg<1>(bwd_kernel<1, DENSE>, grid, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
+    return OPD_OK;
+}
+
 static void phase_mark(opd_handle_s* h, cudaStream_t st, int phase, int end) {
     if (h->phase_events) cudaEventRecord(h->phase_events[2 * phase + end], st);
 }
@@ -233,13 +250,8 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         bp.hint_g = hint_policy(env_int("OPD_HINT_G", 0));
         bp.type_mask = env_int("OPD_BWD_TYPES", 7) & 7;
         // every CTA (pair) must be resident at once: items wait on earlier items of other CTAs
-        static int resident[3] = {0, -1, -1};
-        if (resident[h->cg] < 0)
-            resident[h->cg] = h->cg == 2 ? max_resident_groups<2>(bwd_kernel<2>, h->num_sms) : max_resident_groups<1>(bwd_kernel<1>, h->num_sms);
-        if (resident[h->cg] < 1) OPD_FAIL(h, OPD_ERR_CUDA, "the backward kernel cannot be made resident on device %d", h->device);
-        const int grid = resident[h->cg] * h->cg;
-        if (h->cg == 2) OPD_CUDA(h, launch_cg<2>(bwd_kernel<2>, grid, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, bp));
-        else OPD_CUDA(h, launch_cg<1>(bwd_kernel<1>, grid, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, bp));
+        opd_status_t ls = launch_bwd<false>(h, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_xc_k, m_w_fwd, bp);
+        if (ls != OPD_OK) return ls;
         h->n_kernels++; h->n_gemm++;
         OPD_CUDA(h, cudaGetLastError());
     }

@@ -25,7 +25,8 @@ PHASE_NAMES = ("prep", "fwd", "est", "bwd")
 
 EXPORTS = ("opd_create", "opd_destroy", "opd_last_error", "opd_version", "opd_workspace_bytes", "opd_set_workspace",
            "opd_loss_fwd_bwd", "opd_loss_fwd_bwd_host", "opd_loss_fwd_bwd_host_submit", "opd_loss_fwd_bwd_host_wait", "opd_debug_logits", "opd_debug_gemm", "opd_last_launch_stats",
-           "opd_set_phase_events", "opd_set_diagnostics", "opd_cache_workspace_bytes", "opd_cache_topk", "opd_cache_sample")
+           "opd_set_phase_events", "opd_set_diagnostics", "opd_cache_workspace_bytes", "opd_cache_topk", "opd_cache_sample",
+           "opd_dense_kl_workspace_bytes", "opd_dense_kl_fwd_bwd")
 
 _lib = None
 
@@ -84,6 +85,12 @@ def load_library():
     lib.opd_cache_sample.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_long, c_void_p, c_long, c_long, c_int,
                                      c_void_p, c_long, c_void_p, c_long, c_void_p, c_long, c_void_p]
     lib.opd_cache_sample.restype = c_int
+    lib.opd_dense_kl_workspace_bytes.argtypes = [c_int, c_int, c_int, c_int, c_int, c_uint]
+    lib.opd_dense_kl_workspace_bytes.restype = c_size_t
+    lib.opd_dense_kl_fwd_bwd.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_int, c_void_p, c_long, c_void_p, c_long, c_long,
+                                         c_void_p, c_long, c_void_p, c_long, c_long, c_void_p, c_uint, c_float,
+                                         c_void_p, c_void_p, c_void_p, c_long, c_void_p, c_long, c_long]
+    lib.opd_dense_kl_fwd_bwd.restype = c_int
     lib.opd_set_diagnostics.argtypes = [c_void_p, c_void_p, c_long, c_void_p]
     lib.opd_set_diagnostics.restype = c_int
     lib.opd_set_phase_events.argtypes = [c_void_p, c_void_p]
@@ -279,6 +286,32 @@ class Handle:
         self._check(self.lib.opd_cache_sample(self._h, c_void_p(s), T, d, V, _dtype_code(hidden), _ptr(hidden), hidden.stride(0), _ptr(W),
                                               ldk, ldv, K, _ptr(uniforms), uniforms.stride(0), _ptr(idx), K, _ptr(logp), K, _ptr(lse)))
         return idx, logp, lse
+
+    # ------------------------------------------------------------------ dense two-head KL
+    def dense_kl_fwd_bwd(self, hidden, W, teacher_hidden, W_T, mask, flags=0, norm_override=0.0, grad_hidden=None, grad_W=None):
+        """opd_dense_kl_fwd_bwd -> dict(loss, per_token_kl, grad_hidden, grad_W): dense forward KL(q || p) with
+        q = softmax(teacher_hidden . W_T), p = softmax(hidden . W); W / W_T are the logical [d,V] / [dT,V] heads."""
+        T, d = hidden.shape
+        dT = teacher_hidden.shape[1]
+        V = W.shape[1]
+        ldk, ldv = _w_strides(W, d)
+        tk, tv = _w_strides(W_T, dT)
+        dev = hidden.device
+        fwd_only = bool(flags & F_FWD_ONLY)
+        loss = torch.empty(1, dtype=torch.float32, device=dev)
+        ptk = torch.empty(T, dtype=torch.float32, device=dev)
+        if not fwd_only:
+            if grad_hidden is None:
+                grad_hidden = torch.empty_like(hidden)
+            if grad_W is None:
+                grad_W = torch.empty_strided(tuple(W.shape), (ldk, ldv), dtype=torch.float32, device=dev)
+        gk, gv = (grad_W.stride(0), grad_W.stride(1)) if grad_W is not None else (0, 0)
+        s = torch.cuda.current_stream(dev).cuda_stream
+        self._check(self.lib.opd_dense_kl_fwd_bwd(
+            self._h, c_void_p(s), T, d, dT, V, _dtype_code(hidden), _ptr(hidden), hidden.stride(0), _ptr(W), ldk, ldv,
+            _ptr(teacher_hidden), teacher_hidden.stride(0), _ptr(W_T), tk, tv, _ptr(mask), flags, float(norm_override),
+            _ptr(loss), _ptr(ptk), _ptr(grad_hidden), grad_hidden.stride(0) if grad_hidden is not None else 0, _ptr(grad_W), gk, gv))
+        return dict(loss=loss, per_token_kl=ptk, grad_hidden=grad_hidden, grad_W=grad_W)
 
     # ------------------------------------------------------------------ debug entries
     def debug_logits(self, hidden, W, cache_idx):

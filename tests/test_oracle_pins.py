@@ -483,3 +483,35 @@ def test_P12_paper_table6_fixed_prefix_ratios_follow_one_over_m():
     v1 = var_of_mean(1)
     for m in (2, 4):
         assert abs(var_of_mean(m) / v1 - 1.0 / m) < 1e-10
+
+
+def test_dense_two_head_kl_pins():
+    """dense_kl_oracle (Eq.(1)): equals torch's kl_div (library) and its autograd gradients; equals the
+    top-k forward KL at k = V fed with the teacher's full log-probs (pin P1's relation, through opd_oracle); zero when
+    the two heads coincide; central finite differences; masked rows contribute nothing."""
+    t = tiny(61, T=5, d=6, V=13, mask=[1, 1, 0, 1, 1])
+    rng = np.random.default_rng(4)
+    XT = rng.normal(size=(5, 8)); WT = rng.normal(size=(8, 13)) / math.sqrt(8)
+    r = O.dense_kl_oracle(t["X"], t["W"], XT, WT, t["mask"])
+    X = torch.tensor(t["X"], requires_grad=True); W = torch.tensor(t["W"], requires_grad=True)
+    logp = torch.log_softmax(X @ W, dim=1)
+    logq = torch.log_softmax(torch.tensor(XT) @ torch.tensor(WT), dim=1)
+    m = torch.tensor(t["mask"] != 0)
+    per = torch.nn.functional.kl_div(logp, logq, reduction="none", log_target=True).sum(1)
+    loss = per[m].sum() / m.sum()
+    loss.backward()
+    assert abs(r["loss"] - loss.item()) < 1e-14 and np.abs(r["per_token_kl"][m.numpy()] - per[m].detach().numpy()).max() < 1e-14
+    assert np.abs(r["grad_hidden"] - X.grad.numpy()).max() < 1e-14 and np.abs(r["grad_W"] - W.grad.numpy()).max() < 1e-14
+    assert np.all(r["grad_hidden"][2] == 0) and r["per_token_kl"][2] == 0
+    full = np.tile(np.arange(13), (5, 1))
+    r2 = O.opd_oracle(t["X"], t["W"], full, logq.numpy(), None, t["mask"], O.FKL_TOPK, 13)
+    assert abs(r2["loss"] - r["loss"]) < 1e-13 and np.abs(r2["grad_W"] - r["grad_W"]).max() < 1e-14
+    z = O.dense_kl_oracle(t["X"], t["W"], t["X"], t["W"], t["mask"])
+    assert abs(z["loss"]) < 1e-15 and np.abs(z["grad_W"]).max() < 1e-15
+    f = lambda Xa, Wa: O.dense_kl_oracle(Xa, Wa, XT, WT, t["mask"])["loss"]
+    h = 1e-6
+    for ti, ki, vi in [(0, 1, 2), (3, 5, 12), (4, 0, 7)]:
+        Xp, Xm = t["X"].copy(), t["X"].copy(); Xp[ti, ki] += h; Xm[ti, ki] -= h
+        assert abs((f(Xp, t["W"]) - f(Xm, t["W"])) / (2 * h) - r["grad_hidden"][ti, ki]) < 2e-8
+        Wp, Wm = t["W"].copy(), t["W"].copy(); Wp[ki, vi] += h; Wm[ki, vi] -= h
+        assert abs((f(t["X"], Wp) - f(t["X"], Wm)) / (2 * h) - r["grad_W"][ki, vi]) < 2e-8
