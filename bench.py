@@ -29,7 +29,7 @@ UNIT = "live tokens/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from one `ncu --set full` capture (not measured live)
 NCU_TRAFFIC = {
-    "C4": dict(bwd_kernel=155_149_744_000, fwd_kernel=38_780_680_000, source="profiles/r01c_ncu_full_c4.md"),
+    "C4": dict(bwd_kernel=157_306_721_000, fwd_kernel=37_047_861_000, source="profiles/r01d_final_c4.md"),
 }
 
 
@@ -408,7 +408,7 @@ def main():
     tr = NCU_TRAFFIC.get(f"C{args.config}") if args.mode == "mc" and not args.tokens else None
     roofline = dict(bound="tensor", achieved=ach, peak=pk["sustained"], unit="TFLOP/s", frac=ach / pk["sustained"],
                     traffic=tr["bwd_kernel"] if tr else None,
-                    kernel="opd::bwd_kernel<2> (persistent: G re-formation, grad_hidden, grad_W tiles on tcgen05 cta_group::2)",
+                    kernel="opd::bwd_kernel<2,false> (persistent: G re-formation, grad_hidden, grad_W tiles on tcgen05 cta_group::2)",
                     flops_per_launch=bwd_flops, launches_per_step=1, ms_per_launch=pm["bwd"],
                     peak_kind=f"bf16_tflops_sustained of {pk['src']} (kernel timed inside a long step); burst peak {pk['burst']}",
                     frac_of_burst=ach / pk["burst"],
