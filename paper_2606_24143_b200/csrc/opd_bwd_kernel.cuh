@@ -11,7 +11,8 @@
 //   g_done[s] == #G tiles      before the TMA producer loads G(s) for a DX/DW tile
 //   c_done[s-1] complete       before a DX/DW(s) epilogue touches the fp32 accumulators (previous writer)
 //   c_done[s-R] complete       before a G(s) epilogue overwrites ring buffer s%R (previous readers; R = ring depth)
-// This removes the ~900 launches, their partial last waves and the pipeline refill of the per-GEMM version.
+// One launch instead of one per GEMM and super-tile (about 900 at C4): no partial last waves, no pipeline refills.
+// Every CTA (pair) of the grid must be resident at once (the host sizes the grid with cudaOccupancyMaxActiveClusters).
 #pragma once
 #include "opd_dense.cuh"
 
