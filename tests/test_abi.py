@@ -75,3 +75,37 @@ def test_null_handle_is_an_error(lib):
     assert lib.opd_destroy(None) == -1
     assert lib.opd_set_workspace(None, None, 0) == -1
     assert lib.opd_last_error(None) == b"null handle"
+
+
+def test_header_is_plain_c_and_links_from_c(tmp_path):
+    """include/opd.h compiles as C99 (no C++ / torch types on the boundary) and a C program can link libopd.so and call the
+    entry points that need no GPU."""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("gcc not available")
+    from paper_2606_24143_b200 import build, opd
+    lib = build.build()
+    src = tmp_path / "use_opd.c"
+    src.write_text(r'''
+#include <stdio.h>
+#include "opd.h"
+int main(void) {
+    size_t ws = opd_workspace_bytes(32768, 4096, 151936, 16, OPD_BF16, OPD_RKL_MC, 0);
+    size_t pw = opd_cache_workspace_bytes(1024, 1024, 32768, OPD_BF16, 16, 0);
+    size_t dw = opd_dense_kl_workspace_bytes(1024, 1024, 2048, 32768, OPD_BF16, 0);
+    opd_status_t (*f)(opd_handle_t, void*, int, int, int, opd_dtype_t, const void*, long, const void*, long, long, const int*, long,
+                      const float*, const float*, const unsigned char*, opd_mode_t, int, unsigned, float, float*, float*, float*,
+                      float*, void*, long, void*, long, long) = opd_loss_fwd_bwd;
+    printf("%s|%zu|%zu|%zu|%d\n", opd_version(), ws, pw, dw, f != 0 && opd_destroy(0) == OPD_ERR_BAD_ARG);
+    return 0;
+}
+''')
+    exe = tmp_path / "use_opd"
+    inc = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(opd.__file__))), "include")
+    subprocess.run([gcc, "-std=c99", "-Wall", "-Werror", "-I", inc, str(src), "-o", str(exe), lib, f"-Wl,-rpath,{os.path.dirname(lib)}"],
+                   check=True, capture_output=True, text=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.strip().split("|")
+    assert out[0].startswith("opd-b200") and int(out[1]) == opd.load_library().opd_workspace_bytes(32768, 4096, 151936, 16, 0, 1, 0)
+    assert int(out[2]) > 0 and int(out[3]) > 0 and out[4] == "1"
