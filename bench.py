@@ -27,10 +27,17 @@ METRIC = "OPD loss fwd+bwd tokens/s on 1 B200; % of dense BF16 tensor peak"
 UNIT = "live tokens/s"
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from one `ncu --set full` capture (not measured live)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from one committed `ncu --set full` capture of this
+# workload (a citation: bench.py never runs under a profiler, so the line carries "traffic_measured": false)
 NCU_TRAFFIC = {
     "C4": dict(bwd_kernel=157_306_721_000, fwd_kernel=37_047_861_000, source="profiles/r01d_final_c4.md"),
 }
+
+
+def config_dict(cfg, mode_name, C, sigma):
+    """The workload description both arms print (identical dicts: the driver compares them)."""
+    return dict(workload=f"{cfg['name']} {mode_name} C={C} sigma={sigma}", T=cfg["T"], d=cfg["d"], V=cfg["V"],
+                l2_policy="inputs larger than L2 (W alone is %.0f MB)" % (cfg["d"] * cfg["V"] * 2 / 1e6))
 
 
 def peaks():
@@ -154,7 +161,7 @@ def run_reference(args, rank, world):
     gen = dict(cfg)
     gen["T"] = min(cfg["T"], 2048)                 # the oracle only sees a bounded sample of the workload's rows
     from paper_2606_24143_b200 import synth
-    inp = synth.make_inputs(gen, c=args.config, device=dev)
+    inp = synth.make_inputs(gen, c=args.config, device=dev, sigma=args.sigma)
     mode, idx, lam, old, kk = pick_cache(inp, gen, args.mode)
     prep = oracle_prepare(inp, idx, lam, old, 2048)
     rows = oracle_rows_for(prep, mode, kk, args.ref_seconds, cap=2048)
@@ -168,7 +175,7 @@ def run_reference(args, rank, world):
     sample = f"{rows} live tokens of {cfg['name']} per step (full d={cfg['d']}, V={cfg['V']}), forward+backward incl. grad_W, numpy fp64"
     line = dict(impl="reference", metric=METRIC, value=v, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
                 ms_per_step=1e3 * tot_t / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
-                data="synthetic", config=dict(workload=f"{cfg['name']} {args.mode}", T=cfg["T"], d=cfg["d"], V=cfg["V"]),
+                data="synthetic", config=config_dict(cfg, args.mode, idx.shape[1], inp["sigma"]),
                 cpu_baseline=dict(value=v, unit=UNIT, cores=cpu_threads(), kind="oracle", sample=sample),
                 e2e=dict(value=v, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
     print(json.dumps(line), flush=True)
@@ -307,22 +314,22 @@ def main():
         r = step()
     barrier()
     stats = h.launch_stats()
-    h.enable_phase_timing(True)
-    phase_ms = {k: 0.0 for k in opd.PHASE_NAMES}
+    phase_sets = [h.new_phase_events() for _ in range(args.steps)]      # one set of phase events per timed step
     sampler = ClockSampler(local) if rank == 0 else None
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
     ev[0].record()
     for i in range(args.steps):
+        h.use_phase_events(phase_sets[i])
         r = step()
         ev[i + 1].record()
-        if i == args.steps - 1:
-            pass
     barrier()
+    h.use_phase_events(None)
     total_ms = ev[0].elapsed_time(ev[-1])
     step_ms = [round(ev[i].elapsed_time(ev[i + 1]), 3) for i in range(args.steps)]
-    pm = h.phase_times_ms()                      # phases of the last timed step
-    h.enable_phase_timing(False)
+    per_step = [h.phase_times_ms(ps) for ps in phase_sets]               # every timed step, CUDA events on the launching stream
+    pm = {k: float(np.mean([q[k] for q in per_step])) for k in opd.PHASE_NAMES}          # average over the timed steps
+    phase_steps = {k: [round(q[k], 3) for q in per_step] for k in opd.PHASE_NAMES}
     clocks = sampler.stop() if sampler else None
     loss_val = float(r["loss"].item())
     if dist is not None:
@@ -407,7 +414,7 @@ def main():
     ach_fwd = fwd_flops / (pm["fwd"] * 1e-3) / 1e12
     tr = NCU_TRAFFIC.get(f"C{args.config}") if args.mode == "mc" and not args.tokens else None
     roofline = dict(bound="tensor", achieved=ach, peak=pk["sustained"], unit="TFLOP/s", frac=ach / pk["sustained"],
-                    traffic=tr["bwd_kernel"] if tr else None,
+                    traffic=tr["bwd_kernel"] if tr else None, traffic_measured=False,
                     kernel="opd::bwd_kernel<2,false> (persistent: G re-formation, grad_hidden, grad_W tiles on tcgen05 cta_group::2)",
                     flops_per_launch=bwd_flops, launches_per_step=1, ms_per_launch=pm["bwd"],
                     peak_kind=f"bf16_tflops_sustained of {pk['src']} (kernel timed inside a long step); burst peak {pk['burst']}",
@@ -428,12 +435,11 @@ def main():
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="bf16" if cfg["dtype"] == "bf16" else "f32(3xbf16)", data="synthetic",
-                config=dict(workload=f"{cfg['name']} {args.mode} C={idx.shape[1]} sigma={inp['sigma']}", T=T, d=d, V=V,
-                            live_tokens_per_gpu=n_live, l2_policy="inputs larger than L2 (W alone is %.0f MB)" % (d * V * 2 / 1e6),
-                            super_tile=[stats["super_rows"], stats["super_cols"]]),
+                config=config_dict(cfg, args.mode, idx.shape[1], inp["sigma"]),
+                launch=dict(live_tokens_per_gpu=n_live, super_tile=[stats["super_rows"], stats["super_cols"]], layout=args.layout),
                 pct_of_bf16_peak=dict(executed_8dV_vs_burst=100 * whole / pk["burst"], executed_8dV_vs_sustained=100 * whole / pk["sustained"],
                                       model_6dV_vs_burst=100 * whole * 0.75 / pk["burst"], tflops_executed=whole, peaks=pk),
-                phase_ms=pm, step_ms=step_ms, loss=loss_val, clocks=clocks, e2e=e2e, gpu_launches=stats["kernels"] * args.steps,
+                phase_ms=pm, phase_ms_per_step=phase_steps, step_ms=step_ms, loss=loss_val, clocks=clocks, e2e=e2e, gpu_launches=stats["kernels"] * args.steps,
                 roofline=roofline, cpu_baseline=cpu, mc_diagnostics=diag)
     print(json.dumps(line), flush=True)
     if dist is not None:

@@ -56,6 +56,8 @@ enum {
     OPD_F_NO_RENORM_TEACHER = 1, /* FKL: do not renormalise the cached teacher scores on S (truncated sum)      */
     OPD_F_RENORM_STUDENT = 2,    /* FKL: renormalise the student on S too (paper-literal Eq.(9); sparse backward) */
     OPD_F_GRADW_ACCUM = 4,       /* grad_W += ... instead of overwrite (micro-batches)                           */
+    OPD_F_GRADW_BF16 = 8,        /* grad_W is a bf16 array: sums are kept in fp32 scratch and rounded once at the end
+                                    (reading Q15: the paper does not fix the gradient dtype); +4*d*V bytes of workspace */
     OPD_F_VALIDATE_IDX = 16,     /* check cache indices of live rows; makes the call synchronous                 */
     OPD_F_FWD_ONLY = 32,         /* loss / per-token outputs only; grad pointers may be NULL                     */
     /* reverse-KL surrogate of the 2x2 ablation, Eq.(6),(7) PAPER.md:132-141 (default: A_theta, no clip = Eq.(15)) */
@@ -76,7 +78,10 @@ const char* opd_version(void);
  * gradients G (4608 x 4096 bf16 each) plus fp32 grad_hidden partial sums of one token super-tile, consumed out of L2 by
  * the backward contractions (C4: 431 MB in total, 4.3% of the bf16 logits). The modes whose gradient is purely sparse
  * (OPD_RKL_TOPK; OPD_FKL_TOPK with OPD_F_RENORM_STUDENT) instead need 6*d*V bytes for [V,d] transposes when W is
- * stored [d,V]. */
+ * stored [d,V]; OPD_F_GRADW_BF16 adds 4*d*V bytes (fp32 sums behind the bf16 grad_W).
+ * The handle-owned workspace only grows: a call that needs more than any earlier call on the handle frees and reallocates
+ * it, which synchronises the device (that one call is not asynchronous) and is refused inside a stream capture
+ * (OPD_ERR_WORKSPACE: run the shapes once eagerly first, or provide the memory with opd_set_workspace). */
 size_t opd_workspace_bytes(int T, int d, int V, int C, opd_dtype_t dtype, opd_mode_t mode, unsigned flags);
 /* Optional: use caller memory (256-byte aligned) instead of the handle's own allocation. */
 opd_status_t opd_set_workspace(opd_handle_t h, void* ws, size_t bytes);
@@ -95,8 +100,8 @@ opd_status_t opd_set_workspace(opd_handle_t h, void* ws, size_t bytes);
  * loss [1], per_token_kl [T] (0 on masked rows); optional lse_out [T], student_logp_out [T,C] (row stride
  *          ld_cache; log p_theta(a_tj|s_t), written on live rows' used slots only).
  * grad_hidden [T,d] dtype of hidden, row stride ld_gh, masked rows exactly 0.
- * grad_W   fp32, same logical layout as W: element (k,v) at grad_W[k*ldgw_k + v*ldgw_v], the unit stride
- *          must be the same one as W's.
+ * grad_W   fp32 (bf16 with OPD_F_GRADW_BF16), same logical layout as W: element (k,v) at grad_W[k*ldgw_k + v*ldgw_v], the
+ *          unit stride must be the same one as W's. Overwritten (no need to zero it) unless OPD_F_GRADW_ACCUM.
  * Supported shapes: 1 <= T < 2^24, d % 64 == 0, 64 <= d <= 16384, V % 8 == 0, 256 <= V < 2^24, 1 <= C <= 64;
  *          hidden / W / grad bases 16-byte aligned; non-unit strides multiples of 8 (bf16) / 4 (fp32) elements.
  * Precision: bf16 inputs are used as they are, accumulation is fp32; fp32 inputs are split into three
@@ -120,7 +125,9 @@ opd_status_t opd_loss_fwd_bwd(opd_handle_t h, void* cuda_stream,
 /* Same computation with HOST buffers (pinned or pageable): copies the inputs to handle-owned device
  * buffers, runs opd_loss_fwd_bwd, copies loss / per_token_kl / grad_hidden / grad_W back and
  * synchronises. All arrays are dense (ld = inner extent); W is [d,V] row-major. Pointers that are NULL
- * among the outputs are skipped. *h2d_bytes / *d2h_bytes (may be NULL) receive the bytes copied. */
+ * among the outputs are skipped. *h2d_bytes / *d2h_bytes (may be NULL) receive the bytes copied.
+ * OPD_F_GRADW_BF16: grad_W_host is bf16 (halves the largest copy back). OPD_F_GRADW_ACCUM is refused (OPD_ERR_BAD_ARG): the
+ * device copy of grad_W is per call. The caller's current device is left unchanged by every entry point. */
 opd_status_t opd_loss_fwd_bwd_host(opd_handle_t h,
     int T, int d, int V, opd_dtype_t dtype,
     const void* hidden_host, const void* W_host,
@@ -186,14 +193,29 @@ opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, int T, int 
     float* loss, float* per_token_kl, void* grad_hidden, long ld_gh, void* grad_W, long ldgw_k, long ldgw_v);
 
 /* Optional per-token diagnostics of the MC estimator, written by the following opd_loss_fwd_bwd calls on this
- * handle (device pointers, caller-owned; pass NULLs to switch off):
+ * handle (device pointers, caller-owned; pass NULLs to switch off). rows / cols: the capacity of the arrays (token rows;
+ * slots per row of rho_out, <= ld_rho): a later call with T > rows or C > cols is refused (OPD_ERR_BAD_ARG), never written
+ * out of bounds:
  *   rho_out [T, ld_rho]  rho_theta(a_tj) = p_theta(a_tj|s_t) / p_old(a_tj|s_t) of every cached draw of a live RKL_MC row
  *                        (caller slot order; other entries untouched) — the quantity whose p99 tail Fig. 5 reports
  *                        (PAPER.md:149-151);
  *   var1_out [T]         unbiased sample variance over the m cached draws of the one-sample estimates
  *                        -rho_j A_theta,j, i.e. the within-prefix Var(L^MC_1 | s_t) of Eq.(16);
  *                        0 on masked / non-MC rows and when m = 1. */
-opd_status_t opd_set_diagnostics(opd_handle_t h, float* rho_out, long ld_rho, float* var1_out);
+opd_status_t opd_set_diagnostics(opd_handle_t h, int rows, int cols, float* rho_out, long ld_rho, float* var1_out);
+
+/* Sequence-level diagnostics of App. E (Eq.(17); Table 6, second column): "the same
+ * estimator averaged over generated timesteps". cu_seqlens [n_seq + 1] (device int32): sequence n owns the token rows
+ * [cu_seqlens[n], cu_seqlens[n+1]). The following OPD_RKL_MC / OPD_MIXED calls on this handle write, per sequence n
+ * (device float arrays of n_seq entries, caller-owned; T_n = its live RKL_MC rows; 0 where T_n = 0):
+ *   seq_mean_m[n] = (1/T_n) sum_t L^MC_m(theta; s_t)         the m-sample estimator of Eq.(15) averaged over timesteps
+ *   seq_mean_1[n] = (1/T_n) sum_t L^MC_1(theta; s_t)         the same with the first cached draw of every row only
+ *   seq_var_m[n]  = (1/T_n^2) sum_t Var^(L^MC_1 | s_t) / m   the variance of seq_mean_m over the local draws with the prefix
+ *                   path fixed, from the within-prefix sample variances of Eq.(16) (draws are iid)
+ * R_m^seq is a ratio of variances of these sequence means (m-sample over one-sample) which the caller forms over its
+ * sequences or batches. Pass n_seq = 0 to switch off. */
+opd_status_t opd_set_seq_diagnostics(opd_handle_t h, int n_seq, const int* cu_seqlens,
+                                     float* seq_mean_m, float* seq_mean_1, float* seq_var_m);
 
 /* debugging / verification aids ----------------------------------------------------------------
  * opd_debug_logits: runs the forward contraction kernel only and dumps the fp32 logit tiles it held in
@@ -206,6 +228,9 @@ opd_status_t opd_debug_logits(opd_handle_t h, void* cuda_stream, int T, int d, i
  * A is [M,K] (a_mn_major = 0) or stored as [K,M] (a_mn_major = 1); B is [N,K] or stored as [K,N]. bf16. */
 opd_status_t opd_debug_gemm(opd_handle_t h, void* cuda_stream, int M, int N, int K,
     const void* A, int a_mn_major, const void* B, int b_mn_major, float* D);
+/* opd_debug_occupy: enqueue a kernel of n_ctas CTAs (one per SM: each takes 200 KB of shared memory) that spin for
+ * `milliseconds`. A test aid: the persistent backward kernel must complete while such a kernel holds SMs. */
+opd_status_t opd_debug_occupy(opd_handle_t h, void* cuda_stream, int n_ctas, float milliseconds);
 /* Launch statistics of the last opd_loss_fwd_bwd on this handle: kernels launched, GEMM-kernel launches,
  * super-tile rows/cols used by the backward. Any pointer may be NULL. */
 opd_status_t opd_last_launch_stats(opd_handle_t h, int* n_kernels, int* n_gemm_kernels, int* super_rows, int* super_cols);

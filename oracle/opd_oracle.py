@@ -38,7 +38,8 @@ Readings of the paper where it is silent or ambiguous are listed in DESIGN.md ("
 Pins (tests/test_oracle_pins.py): k=V equals dense D_F; k=1 equals library cross-entropy; K=V uniform
 proposal equals dense D_R; Eq.(5) by enumeration; on-policy unbiasedness; 1/m variance law; KL >= 0;
 zero cases; central finite differences; softmax-shift invariance; mask/permutation invariance;
-duplicates.  No function here is "parity unpinned".
+duplicates; the four PPO-style surrogates against Eq.(4)/(6)/(7) written out; the sequence-level diagnostics by
+enumeration.  No function here is "parity unpinned".
 
 Everything is float64.  A library matmul (numpy) serves as the O1 step; tokens are processed in
 row chunks only to bound memory (rows are independent).  ``opd_oracle_loops`` is the same
@@ -198,6 +199,7 @@ def opd_oracle(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, m
     slp = np.full(idx.shape, np.nan)
     rho_out = np.full(idx.shape, np.nan)       # diagnostics: rho_theta(a_tj) on MC rows (Fig. 5)
     var1_out = np.zeros(T)                     # diagnostics: sample variance of the one-sample terms (Eq.(16))
+    first_out = np.zeros(T)                    # diagnostics: L^MC_1 from the first cached draw, -rho_1 A_theta,1 (Eq.(15), m = 1)
     gh = np.zeros((T, d)) if want_grads else None
     gW = np.zeros((d, V)) if (want_grads and want_grad_W) else None
 
@@ -224,6 +226,7 @@ def opd_oracle(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, m
             slp[t, :C] = ell
             if tmode == RKL_MC:
                 rho_out[t, :C], var1_out[t] = mc_diagnostics(lam_all[t, :C], old, ell)
+                first_out[t] = -rho_out[t, 0] * (lam_all[t, 0] - ell[0])
             if want_grads:
                 g = alpha * p[i]                           # O7 dense part
                 np.add.at(g, a, beta)                      # O7 sparse part (duplicates add)
@@ -234,7 +237,7 @@ def opd_oracle(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, m
                 gW += X[tt].T @ G                          # O9
     loss = float(np.sum(per_token)) * scale                # O6
     return dict(loss=loss, N=N, per_token_kl=per_token, lse=lse_out, student_logp=slp,
-                alpha=alpha_out, grad_hidden=gh, grad_W=gW, rho=rho_out, var1=var1_out)
+                alpha=alpha_out, grad_hidden=gh, grad_W=gW, rho=rho_out, var1=var1_out, first_draw=first_out)
 
 
 def grad_W_columns(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K,
@@ -356,6 +359,38 @@ def mc_diagnostics(lam, old, ell):
     return rho, var1
 
 
+def seq_diagnostics(per_token_mc, first_draw, var1, mask, cu_seqlens, m: int, mc_code=None):
+    """Sequence-level diagnostics of App. E, Eq.(17) (Table 6 second column PAPER.md:412-419): "the same
+    estimator averaged over generated timesteps".  For every sequence n = token rows [cu[n], cu[n+1]) with T_n live MC rows:
+
+        mean_m[n] = (1/T_n) sum_t L^MC_m(theta; s_t)          (per_token_mc[t], Eq.(15))
+        mean_1[n] = (1/T_n) sum_t L^MC_1(theta; s_t)          (first_draw[t] = -rho_t1 A_theta,t1, the first cached draw)
+        var_m[n]  = (1/T_n^2) sum_t var1[t] / m               variance of mean_m over the local draws with the prefix path
+                                                              fixed: draws are iid across and within prefixes,
+                                                              so Var(mean_m) = (1/T_n^2) sum_t Var(L^MC_1 | s_t) / m, with the
+                                                              within-prefix variances estimated as in Eq.(16) (mc_diagnostics)
+    mc_code: if given (MIXED batches), only rows with mask == mc_code take part; else every live row.
+    R_m^seq of Eq.(17) is the ratio of the variances of mean_m and mean_1, which a caller forms over its sequences / batches
+    (reading Q19 in DESIGN.md: with the path fixed and iid draws the ratio of the var_m's is exactly 1/m; the paper's measured
+    0.338 / 0.152 / 0.112 are above 1/m, i.e. its variance also contains variation that more draws do not remove)."""
+    L = np.asarray(per_token_mc, dtype=np.float64)
+    L1 = np.asarray(first_draw, dtype=np.float64)
+    v1 = np.asarray(var1, dtype=np.float64)
+    msk = np.asarray(mask).astype(np.int64)
+    cu = np.asarray(cu_seqlens).astype(np.int64)
+    n_seq = cu.shape[0] - 1
+    mean_m, mean_1, var_m = np.zeros(n_seq), np.zeros(n_seq), np.zeros(n_seq)
+    for n in range(n_seq):
+        rows = [t for t in range(cu[n], cu[n + 1]) if msk[t] != 0 and (mc_code is None or msk[t] == mc_code)]
+        Tn = len(rows)
+        if Tn == 0:
+            continue
+        mean_m[n] = sum(L[t] for t in rows) / Tn
+        mean_1[n] = sum(L1[t] for t in rows) / Tn
+        var_m[n] = sum(v1[t] for t in rows) / (Tn * Tn * m)
+    return mean_m, mean_1, var_m
+
+
 def sparse_reverse_kl(lam: np.ndarray, ell: np.ndarray):
     """App. A.1 Eq.(8)-(10) for ONE token on a fixed cached support S.
 
@@ -408,11 +443,10 @@ def cache_sample(hidden, W, uniforms):
 # ------------------------------------------------------------------------------------------------
 # Dense two-head forward KL: the teacher's distribution recomputed from transmitted teacher
 # hidden states (the direction PAPER.md:240 names as future work), objective Eq.(1), gradient PAPER.md:59.
-def dense_kl_oracle(hidden, W, teacher_hidden, W_T, mask, norm_override: float = 0.0, q_round=None, chunk: int = 512):
+def dense_kl_oracle(hidden, W, teacher_hidden, W_T, mask, norm_override: float = 0.0, chunk: int = 512):
     """q_t = softmax(h^T_t . W_T), p_t = softmax(x_t . W);  L_t = sum_v q_tv (log q_tv - log p_tv)  (Eq.(1));
     loss = (1/N) sum_t m_t L_t;  dL_t/dz_tv = (sum_v q_tv) p_tv - q_tv  (= p - q, PAPER.md:59);
-    grad_hidden / grad_W by the chain rule (O8, O9).  ``q_round``: optional function applied to q before it is used
-    (the bf16 CUDA path rounds q to bf16 — the tests compare against both the exact and the rounded definition).
+    grad_hidden / grad_W by the chain rule (O8, O9).
     Returns dict(loss, N, per_token_kl[T], grad_hidden[T,d], grad_W[d,V])."""
     X = np.asarray(hidden, dtype=np.float64)
     Wd = np.asarray(W, dtype=np.float64)
@@ -433,8 +467,6 @@ def dense_kl_oracle(hidden, W, teacher_hidden, W_T, mask, norm_override: float =
         logp, _ = log_softmax_rows(X[tt] @ Wd)
         logq, _ = log_softmax_rows(XT[tt] @ WT)
         q = np.exp(logq)
-        if q_round is not None:
-            q = q_round(q)
         per_token[tt] = np.sum(q * (logq - logp), axis=1)
         G = (np.sum(q, axis=1, keepdims=True) * np.exp(logp) - q) * scale
         gh[tt] = G @ Wd.T

@@ -4,8 +4,8 @@
     loss.backward()        # hidden.grad / lm_head_weight.grad come from the library's fused backward
 
 Marshalling only: forward calls opd_loss_fwd_bwd once (loss AND both gradients are produced by that call, the
-logits are never materialised); backward hands the stored gradients to autograd, scaled in place by the incoming
-scalar gradient.  There is no PyTorch fallback: without libopd.so / off sm_100 the call raises.
+logits are never materialised); backward hands the stored gradients to autograd, scaled (out of place: a second
+backward with retain_graph=True sees the same saved tensors) by the incoming scalar gradient.  There is no PyTorch fallback: without libopd.so / off sm_100 the call raises.
 """
 from __future__ import annotations
 
@@ -33,9 +33,9 @@ class _OpdLoss(torch.autograd.Function):
         if not ctx.need_grad:
             return (None,) * 10
         gh, gw = ctx.saved_tensors
-        if g_loss is not None:                  # chain rule with the incoming scalar, in place, without a host sync
-            gh.mul_(g_loss.to(gh.dtype))
-            gw.mul_(g_loss.to(gw.dtype))
+        if g_loss is not None:                  # chain rule with the incoming scalar: out of place, without a host sync
+            gh = gh * g_loss.to(gh.dtype)
+            gw = gw * g_loss.to(gw.dtype)
         gw = gw if gw.dtype == ctx.w_dtype else gw.to(ctx.w_dtype)
         return gh, gw, None, None, None, None, None, None, None, None
 

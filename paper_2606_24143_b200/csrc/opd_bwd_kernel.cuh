@@ -6,13 +6,17 @@
 //   G(s)   logits of super-tile s recomputed -> G tile (bf16) into buffer s%R of the G ring (consumed from L2)
 //   DX(s)  grad_hidden[tb] (+)= G(s) . W[:,vb]^T        DW(s)  grad_W[:,vb] += Xc[tb]^T . G(s)
 //
-// CTAs take items round-robin in list order; an item only depends on earlier items, through two counters
-// per super-tile in global memory (release by the epilogue after its stores, acquire by whoever consumes):
+// CTA pairs claim items dynamically, in list order, from a global ticket counter (ticket_claim / ticket_read in
+// opd_gemm.cuh); an item only depends on earlier items, through two counters per super-tile in global memory
+// (release by the epilogue after its stores, acquire by whoever consumes):
 //   g_done[s] == #G tiles      before the TMA producer loads G(s) for a DX/DW tile
 //   c_done[s-1] complete       before a DX/DW(s) epilogue touches the fp32 accumulators (previous writer)
 //   c_done[s-R] complete       before a G(s) epilogue overwrites ring buffer s%R (previous readers; R = ring depth)
 // One launch instead of one per GEMM and super-tile (about 900 at C4): no partial last waves, no pipeline refills.
-// Every CTA (pair) of the grid must be resident at once (the host sizes the grid with cudaOccupancyMaxActiveClusters).
+// Because an item's dependencies were all claimed before it, by CTAs that are running, the kernel needs no particular
+// number of resident CTAs: it completes next to other kernels, under MPS or with SM-limited contexts (the host still sizes
+// the grid to one CTA per SM, which is the fastest configuration).  The order in which tiles are reduced into an fp32
+// accumulator is fixed by the counters, not by which CTA runs a tile: results stay bit-reproducible.
 #pragma once
 #include "opd_dense.cuh"
 
@@ -26,6 +30,9 @@ struct BwdParams {
     const int* n_live;
     int* g_done;               // [S]
     int* c_done;               // [S]
+    int* ticket;               // [1] next unclaimed item of the tile list (zeroed by the host before the launch)
+    int dw_store_first;        // 1: the grad_W tiles of the first token super-tile store instead of reduce-add (grad_W is
+                               //    overwritten, not accumulated into: no memset and no read-modify-write for that pass)
     int type_mask;             // bit t set = run tiles of type t.  All types of the variant = the normal run; a tile waits
                                // on a counter only if every tile type that increments it is enabled (dense forward-only
                                // runs Q + G; other subsets are timing experiments and give wrong gradients)
@@ -82,6 +89,7 @@ struct BwdSched {
     }
     // decode `item` (monotonically increasing between calls); false when the list is exhausted
     __device__ __forceinline__ bool get(long item, BwdTile& t) {
+        if (S <= 0) return false;
         while (blk <= S + GOFF) {
             const int sz = block_size(blk);
             if (item < base + sz) break;
@@ -142,7 +150,6 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     if (*bp.n_live <= 0) return;                      // uniform over the grid
-    const long first_item = blockIdx.x / CG, item_step = gridDim.x / CG;
 
     if (warp == 0 && lane == 0) {
         prefetch_tmap(&m_xc_k); prefetch_tmap(&m_w_fwd); prefetch_tmap(&m_gs_k);
@@ -166,7 +173,10 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             BwdSched<CG, DENSE> sc; sc.init(bp);
             BwdTile t;
             int it = 0;
-            for (long item = first_item; sc.get(item, t); item += item_step) {
+            for (int n = 0;; ++n) {
+                // the leader's producer claims the pair's next item; the peer's producer reads it from the queue
+                const uint32_t item = rank == 0 ? ticket_claim<CG>(P, bp.ticket, n) : ticket_read<CG>(P, n);
+                if (!sc.get(item, t)) break;
                 if (!on(t.type)) continue;
                 TileOp op;
                 int pa_off = 0, pb_off = 0;
@@ -211,7 +221,8 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             BwdSched<CG, DENSE> sc; sc.init(bp);
             BwdTile t;
             int it = 0, lt = 0;
-            for (long item = first_item; sc.get(item, t); item += item_step) {
+            for (int n = 0;; ++n) {
+                if (!sc.get(ticket_read<CG>(P, n), t)) break;
                 if (!on(t.type)) continue;
                 int a_mn, b_mn, K;
                 if (t.type == T_G) { a_mn = 0; b_mn = (bp.wl == 0); K = bp.d; }
@@ -234,7 +245,11 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             if (lane == 0) { wait_counter(counter, expected); fence_proxy_async_all(); }
             __syncwarp();
         };
-        for (long item = first_item; sc.get(item, t); item += item_step) {
+        for (int n = 0;; ++n) {
+            uint32_t item = 0;
+            if (lane == 0) item = ticket_read<CG>(P, n);
+            item = __shfl_sync(0xffffffffu, item, 0);
+            if (!sc.get(item, t)) break;
             if (!on(t.type)) continue;
             const int m_blk = t.m_blk * CG + rank;    // this CTA's 128-row block inside the GEMM
             GemmParams gp{};                      // the fields the epilogues read
@@ -279,6 +294,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 int M_eff;
                 if (bp.wl == 0) { gp.N = t.Vb_eff; gp.row_off = 0; gp.col_off = t.vb0; M_eff = bp.d; }
                 else { gp.N = bp.d; gp.row_off = t.vb0; gp.col_off = 0; M_eff = t.Vb_eff; }
+                gp.first = bp.dw_store_first && t.tb0 == 0;          // first token super-tile: plain stores
                 const uint32_t taddr = epi_acquire<CG>(P, lt, quarter);
                 DwEpi::run(bp.dw, gp, NoState{}, taddr, m_blk, t.n_blk, row_in_tile, M_eff, P.epi_smem, epi_tid);
             }

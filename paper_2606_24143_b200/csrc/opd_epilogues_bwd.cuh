@@ -27,6 +27,7 @@ struct GEpi {
         const float* beta;       // [T][C] beta_tj / N in sorted-slot order
         int C;
         int V;
+        unsigned long long st_hint;   // L2 eviction policy of the G stores (0 = plain stores)
     };
     struct State { int cursor; int next_col; float lse2; float coef; };
     static __device__ __forceinline__ State prepare(const Params& p, const GemmParams& gp, int m_blk, int n_blk,
@@ -89,8 +90,13 @@ struct GEpi {
                     }
                 }
                 uint4* dst = reinterpret_cast<uint4*>(out + pl * p.plane_stride + c * 32);
+                if (p.st_hint) {
 #pragma unroll
-                for (int q = 0; q < 4; ++q) dst[q] = make_uint4(w[4 * q], w[4 * q + 1], w[4 * q + 2], w[4 * q + 3]);
+                    for (int q = 0; q < 4; ++q) st_global_v4_hint(dst + q, w[4 * q], w[4 * q + 1], w[4 * q + 2], w[4 * q + 3], p.st_hint);
+                } else {
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) dst[q] = make_uint4(w[4 * q], w[4 * q + 1], w[4 * q + 2], w[4 * q + 3]);
+                }
             }
         }
     }
@@ -130,7 +136,9 @@ struct DxEpi {
     struct Params {
         CUtensorMap m_acc;       // fp32 [Tb_pad][d], boxes of 32 x 32
         uint64_t hint;           // L2 eviction policy of the partial-sum stores / reductions
-        int dbg;                 // timing experiments: 1 = plain stores instead of reductions, 2 = no output
+#ifdef OPD_EXPERIMENTS
+        int dbg;                 // timing experiments (wrong gradients): 1 = plain stores instead of reductions, 2 = no output
+#endif
         float* acc;              // same buffer, for the last super-tile's read
         long ld_acc;
         void* out;               // grad_hidden
@@ -160,9 +168,14 @@ struct DxEpi {
             tmem_ld_wait();
             const int col0 = n_blk * BN + c * 32;
             if (col0 >= gp.N) break;                                  // d % 64 == 0: chunks are all-in or all-out (warp-uniform)
+#ifdef OPD_EXPERIMENTS
             if (p.dbg == 2) continue;
+            const bool reduce = !gp.first && p.dbg != 1;
+#else
+            const bool reduce = !gp.first;
+#endif
             if (!gp.last) {
-                stage_and_send(&p.m_acc, wbuf, c & 1, v, lane, col0, lrow - lane, !gp.first && p.dbg != 1, p.hint);
+                stage_and_send(&p.m_acc, wbuf, c & 1, v, lane, col0, lrow - lane, reduce, p.hint);
             } else if (live) {
                 if (!gp.first) {
                     const float4* a4 = reinterpret_cast<const float4*>(acc + c * 32);
@@ -190,14 +203,17 @@ struct DxEpi {
 };
 
 // ------------------------------------------------------------------------------------------ DwEpi
-// S8: grad_W tile += accumulator (TMA reduce-add; grad_W was zeroed or holds the caller's running sum).  Output element
+// S8: grad_W tile (+)= accumulator (TMA reduce-add; the tiles of the first token super-tile store instead unless the call
+// accumulates into the caller's running sum, so grad_W needs no memset).  Output element
 // (row, col) of this GEMM lives at row = row_off + tile row, col = col_off + tile col of the fp32 tensor the map
 // describes ((d,V) or (V,d)); TMA clips rows / columns outside the tensor.
 struct DwEpi {
     struct Params {
         CUtensorMap m_gw;        // fp32 [rows_total][cols_total] (row stride ld), boxes of 32 x 32
         uint64_t hint;           // L2 eviction policy of the grad_W reductions
-        int dbg;                 // timing experiments: 1 = plain stores instead of reductions, 2 = no output
+#ifdef OPD_EXPERIMENTS
+        int dbg;                 // timing experiments (wrong gradients): 1 = plain stores instead of reductions, 2 = no output
+#endif
     };
     using State = NoState;
     static __device__ __forceinline__ State prepare(const Params&, const GemmParams&, int, int, int, int) { return {}; }
@@ -214,7 +230,13 @@ struct DwEpi {
             tmem_ld_wait();
             const int lc0 = n_blk * BN + c * 32;
             if (lc0 >= gp.N) break;
-            if (warp_ok && p.dbg != 2) stage_and_send(&p.m_gw, wbuf, c & 1, v, lane, gp.col_off + lc0, gp.row_off + lrow0, p.dbg != 1, p.hint);
+#ifdef OPD_EXPERIMENTS
+            if (p.dbg == 2) continue;
+            const bool reduce = !gp.first && p.dbg != 1;
+#else
+            const bool reduce = !gp.first;      // first token super-tile of an overwriting call: plain store
+#endif
+            if (warp_ok) stage_and_send(&p.m_gw, wbuf, c & 1, v, lane, gp.col_off + lc0, gp.row_off + lrow0, reduce, p.hint);
         }
         drain_sends(lane);
     }

@@ -23,6 +23,7 @@ struct EstParams {
     float* lse2; float* coef; float* beta;               // compact-row order ([T], [T], [T][C])
     float* per_token_kl; float* lse_out; float* slp_out; // caller order; lse_out / slp_out may be null
     float* rho_out; long ld_rho; float* var1_out;        // optional diagnostics (opd_set_diagnostics), caller order
+    float* seq_l1; float* seq_var1;                      // optional [T] (opd_set_seq_diagnostics): first-draw estimate, Eq.(16) variance
     double* block_sums;                                  // [gridDim.x]
 };
 
@@ -101,6 +102,7 @@ __global__ void __launch_bounds__(128) k_estimator(const EstParams p) {
             const float invm = 1.f / static_cast<float>(Cr);
             float sum_term = 0.f, sum_w = 0.f;
             float sx = 0.f, sxx = 0.f;                      // one-sample estimates X_j = -rho_j A_theta,j (Eq.(16))
+            float x_first = 0.f;                            // X of the caller's slot 0 (the one-sample estimator L^MC_1)
             for (int s = 0; s < Cr; ++s) {
                 const float ell = zc[s] - lse;
                 const float o = old[pm[s]];
@@ -109,7 +111,7 @@ __global__ void __launch_bounds__(128) k_estimator(const EstParams p) {
                 const float A = (p.flags & FL_SUR_A_OLD) ? (lm - o) : (lm - ell);
                 float term = rho * A, w = rho * A;
                 if (p.rho_out) p.rho_out[static_cast<size_t>(tok) * p.ld_rho + pm[s]] = rho;
-                { const float x = -rho * (lm - ell); sx += x; sxx += x * x; }
+                { const float x = -rho * (lm - ell); sx += x; sxx += x * x; if (pm[s] == 0) x_first = x; }
                 if (p.flags & FL_SUR_CLIP) {
                     const float rbar = fminf(fmaxf(rho, 1.f - CLIP_EPS), 1.f + CLIP_EPS);
                     const float cl = rbar * A;
@@ -124,7 +126,9 @@ __global__ void __launch_bounds__(128) k_estimator(const EstParams p) {
             }
             L = -sum_term * invm;
             alpha = sum_w * invm;
-            if (p.var1_out) p.var1_out[tok] = Cr > 1 ? fmaxf(0.f, (sxx - sx * sx * invm) / static_cast<float>(Cr - 1)) : 0.f;
+            const float var1 = Cr > 1 ? fmaxf(0.f, (sxx - sx * sx * invm) / static_cast<float>(Cr - 1)) : 0.f;
+            if (p.var1_out) p.var1_out[tok] = var1;
+            if (p.seq_l1) { p.seq_l1[tok] = x_first; p.seq_var1[tok] = var1; }
         }
         for (int s = Cr; s < p.C; ++s) beta[s] = 0.f;
         p.lse2[i] = lse * LOG2E;
@@ -157,6 +161,36 @@ __global__ void __launch_bounds__(256) k_loss_final(const double* __restrict__ b
     if (threadIdx.x == 0) {
         const double norm = norm_override > 0.f ? static_cast<double>(norm_override) : static_cast<double>(*n_live);
         *loss = norm > 0.0 ? static_cast<float>(sh[0] / norm) : 0.f;
+    }
+}
+
+// Sequence-level diagnostics (opd_set_seq_diagnostics; Eq.(17)): per sequence the timestep averages of
+// the m-sample and of the one-sample estimator and the fixed-path variance of the former.  One block per sequence,
+// fp64 tree reduction in a fixed order.
+__global__ void __launch_bounds__(256) k_seq_diag(const int* __restrict__ cu, int n_seq, int T, const unsigned char* __restrict__ mask,
+                                                  int mode, int m, const float* __restrict__ per_token_kl, const float* __restrict__ l1,
+                                                  const float* __restrict__ var1, float* __restrict__ mean_m, float* __restrict__ mean_1,
+                                                  float* __restrict__ var_m) {
+    const int n = blockIdx.x;
+    const int b = max(0, min(T, cu[n])), e = max(b, min(T, cu[n + 1]));
+    double cnt = 0.0, sm = 0.0, s1 = 0.0, sv = 0.0;
+    for (int t = b + threadIdx.x; t < e; t += blockDim.x) {
+        const int mk = mask[t];
+        if (mk != 0 && (mode == MODE_MC || mk == 2)) { cnt += 1.0; sm += per_token_kl[t]; s1 += l1[t]; sv += var1[t]; }
+    }
+    __shared__ double sh[4][256];
+    sh[0][threadIdx.x] = cnt; sh[1][threadIdx.x] = sm; sh[2][threadIdx.x] = s1; sh[3][threadIdx.x] = sv;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (threadIdx.x < s)
+            for (int q = 0; q < 4; ++q) sh[q][threadIdx.x] += sh[q][threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const double Tn = sh[0][0];
+        mean_m[n] = Tn > 0 ? static_cast<float>(sh[1][0] / Tn) : 0.f;
+        mean_1[n] = Tn > 0 ? static_cast<float>(sh[2][0] / Tn) : 0.f;
+        var_m[n] = Tn > 0 ? static_cast<float>(sh[3][0] / (Tn * Tn * m)) : 0.f;
     }
 }
 

@@ -27,8 +27,9 @@ constexpr int EPI_SMEM_BYTES = 32768;                 // 4 epilogue warps x 2 st
 constexpr int TMEM_COLS = 512;                        // 2 accumulator stages x 256 columns
 constexpr int MAX_STAGES = 6;
 #ifndef OPD_PAIR_STAGES
-#define OPD_PAIR_STAGES 6                  // TMA ring depth of the CTA-pair configuration (32 KiB per stage)
-#endif
+#define OPD_PAIR_STAGES 4                  // TMA ring depth of the CTA-pair configuration (32 KiB per stage): 4 stages keep the
+#endif                                     // tensor pipe as busy as 6 and re-fetch far less of W from HBM (profiles/r02_*)
+constexpr int SCHED_Q = 4;                 // depth of the tile-ticket queue of the dynamically scheduled kernels
 
 template <int CG>
 struct Cfg {
@@ -84,6 +85,8 @@ struct Pipe {
     using C = Cfg<CG>;
     uint8_t* smem;
     uint64_t *full_bar, *empty_bar, *tfull_bar, *tempty_bar;
+    uint64_t *sfull_bar, *sempty_bar;     // tile-ticket queue (bwd_kernel): ticket q published / consumed by every reader
+    uint32_t* sticket;                    // [SCHED_Q] claimed tickets (a copy in each CTA of a pair)
     uint32_t* tmem_slot;
     uint8_t* epi_smem;
     uint32_t tmem_base;
@@ -96,11 +99,17 @@ struct Pipe {
         tfull_bar = empty_bar + MAX_STAGES;
         tempty_bar = tfull_bar + 2;
         tmem_slot = reinterpret_cast<uint32_t*>(tempty_bar + 2);
+        sfull_bar = reinterpret_cast<uint64_t*>(smem + C::RING_BYTES + 256);
+        sempty_bar = sfull_bar + SCHED_Q;
+        sticket = reinterpret_cast<uint32_t*>(sempty_bar + SCHED_Q);
         epi_smem = smem + C::RING_BYTES + 1024;
         rank = CG == 1 ? 0u : cluster_ctarank();
         if (warp == 0 && lane == 0) {
             for (int s = 0; s < C::STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
             for (int s = 0; s < 2; ++s) { mbar_init(&tfull_bar[s], 1); mbar_init(&tempty_bar[s], 4 * CG); }
+            // readers of a ticket: the MMA issuer and the 4 epilogue warps of the leader, the producer and the 4 epilogue
+            // warps of the peer CTA (the leader's producer is the claimer)
+            for (int s = 0; s < SCHED_Q; ++s) { mbar_init(&sfull_bar[s], 1); mbar_init(&sempty_bar[s], CG == 1 ? 5 : 10); }
             fence_mbar_init();
         }
         if (warp == 1) {
@@ -118,6 +127,34 @@ struct Pipe {
         if (warp == 1) tmem_dealloc<CG>(tmem_base, TMEM_COLS);
     }
 };
+
+// ------------------------------------------------------------------------------------------------ tile tickets
+// Dynamic tile scheduling for kernels whose tiles wait on tiles of other CTAs: ONE thread of a CTA (pair) claims the next
+// item of the tile list from a global counter and publishes it to every warp role of the CTA (pair) through a small queue
+// in shared memory.  Items are claimed in list order, so everything an item depends on has been claimed by a CTA that is
+// already running: the kernel makes progress with any number of resident CTAs (no co-residency requirement).
+template <int CG>
+__device__ __forceinline__ uint32_t ticket_claim(const Pipe<CG>& P, int* counter, int n) {
+    const int q = n % SCHED_Q;
+    mbar_wait_cluster(&P.sempty_bar[q], ((n / SCHED_Q) & 1) ^ 1);
+    const uint32_t t = static_cast<uint32_t>(atomicAdd(counter, 1));
+    P.sticket[q] = t;
+    if constexpr (CG == 2) {
+        st_shared_cluster_u32(mapa_rank(smem_u32(&P.sticket[q]), 1), t);
+        mbar_arrive_cluster(mapa_rank(smem_u32(&P.sfull_bar[q]), 1));
+    }
+    mbar_arrive(&P.sfull_bar[q]);
+    return t;
+}
+// called by one lane of a reader; every reader consumes every ticket exactly once, in order
+template <int CG>
+__device__ __forceinline__ uint32_t ticket_read(const Pipe<CG>& P, int n) {
+    const int q = n % SCHED_Q;
+    mbar_wait_cluster(&P.sfull_bar[q], (n / SCHED_Q) & 1);
+    const uint32_t t = *reinterpret_cast<volatile uint32_t*>(&P.sticket[q]);
+    mbar_arrive_cluster(mapa_rank(smem_u32(&P.sempty_bar[q]), 0));
+    return t;
+}
 
 // One tile's operand stream as the TMA producer of ONE CTA sees it.
 struct TileOp {

@@ -19,6 +19,8 @@ struct opd_handle_s {
     int num_sms = 0;
     int cg = 2;                    // tcgen05 cta_group of the GEMM core: 2 = CTA pairs (default), 1 = single CTAs (OPD_CTA_GROUP)
     bool arch_ok = false;
+    int l2_bytes = 0, l2_persist_max = 0, l2_window_max = 0;   // L2 size, largest persisting carve-out, largest access-policy window
+    size_t l2_persist = 0;         // persisting carve-out this handle asked for (cudaLimitPersistingL2CacheSize)
     void* ws = nullptr;            // workspace in use
     size_t ws_bytes = 0;
     bool ws_owned = false;
@@ -30,10 +32,14 @@ struct opd_handle_s {
     cudaEvent_t ev_in[2] = {}, ev_c[2] = {}, ev_out[2] = {};
     size_t slot_h2d[2] = {0, 0}, slot_d2h[2] = {0, 0};
     bool slot_busy[2] = {false, false};
+    int bwd_grid[3][2] = {{0, 0}, {0, 0}, {0, 0}};   // [cta group][dense]: grid of the persistent backward on THIS device (0 = not computed)
     // stats of the last call
     int n_kernels = 0, n_gemm = 0, super_rows = 0, super_cols = 0;
     cudaEvent_t* phase_events = nullptr;
     float* diag_rho = nullptr; long diag_ld_rho = 0; float* diag_var1 = nullptr;   // opd_set_diagnostics
+    int diag_rows = 0, diag_cols = 0;                                               // capacity of the diagnostics arrays
+    int seq_n = 0; const int* seq_cu = nullptr;                                     // opd_set_seq_diagnostics
+    float *seq_mean_m = nullptr, *seq_mean_1 = nullptr, *seq_var_m = nullptr;
 };
 
 namespace opd {
@@ -94,7 +100,8 @@ struct Plan {
     int Tb, Vb;           // backward super-tile (rows of tokens x vocabulary columns), multiples of 128 / 256
     int est_blocks;
     size_t off_nlive, off_badidx, off_live_rows, off_xc, off_wsplit, off_sorted, off_perm, off_zc, off_beta,
-           off_partials, off_lse2, off_coef, off_gs, off_dxacc, off_block_sums, off_counters, off_wt, off_gwt, total;
+           off_partials, off_lse2, off_coef, off_gs, off_dxacc, off_block_sums, off_counters, off_wt, off_gwt, off_gw32,
+           off_seq_l1, off_seq_var1, total;
     bool sparse_bwd;      // alpha == 0 on every row: gradients live on the cached columns only (no dense backward)
     int n_super;          // number of backward super-tiles (upper bound)
     int gs_bufs;          // ring depth of the G super-tile buffer
@@ -122,9 +129,21 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int 
     const int TM = BM * cta_group_setting();              // tile rows of the GEMM core (CTA or CTA pair)
     p.t_pad = ceil_div(T, TM) * TM;
     p.num_n = ceil_div(V, BN);
-    // Super-tile of the backward: 4608 (4736 for single-CTA tiles) token rows x 4096 vocabulary columns = 288 pair
-    // tiles (592 CTA tiles) per G re-formation; the bf16 G super-tile (36-37 MiB) is consumed out of L2.
-    const int tb = env_int("OPD_TB", TM == 256 ? 18 * 256 : 37 * BM), vb = env_int("OPD_VB", 4096);
+    // Super-tile of the backward: up to 4608 (4736 for single-CTA tiles) token rows x 4096 vocabulary columns = 288 pair
+    // tiles (592 CTA tiles) per G re-formation; the bf16 G super-tile (at most 36-37 MiB) is consumed out of L2.  Among
+    // the row counts between 3584 and the maximum the one that wastes the fewest padded rows in the last token
+    // super-tile is taken (T = 32768 or 65536: 4096 rows, i.e. equal super-tiles; measured 2% faster than 4608 at C4).
+    const int tb_max = TM == 256 ? 18 * 256 : 37 * BM;
+    int tb = env_int("OPD_TB", 0);
+    if (tb <= 0) {
+        tb = tb_max;
+        long best_waste = -1;
+        for (int cand = tb_max; cand >= 3584 && p.t_pad > tb_max; cand -= TM) {
+            const long waste = (long)ceil_div(p.t_pad, cand) * cand - p.t_pad;
+            if (best_waste < 0 || waste < best_waste) { best_waste = waste; tb = cand; }
+        }
+    }
+    const int vb = env_int("OPD_VB", 4096);
     p.Tb = std::min(p.t_pad, std::max(TM, tb / TM * TM));
     p.Vb = std::min(p.num_n * BN, std::max(BN, vb / BN * BN));
     p.est_blocks = ceil_div(T, 128);
@@ -144,14 +163,20 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int 
     p.off_lse2 = take(sizeof(float) * (size_t)p.t_pad);
     p.off_coef = take(sizeof(float) * (size_t)p.t_pad);
     const bool bwd = !(flags & OPD_F_FWD_ONLY);
-    p.sparse_bwd = (mode == OPD_RKL_TOPK || (mode == OPD_FKL_TOPK && (flags & OPD_F_RENORM_STUDENT))) && !env_int("OPD_DENSE_BWD", 0);
+    p.sparse_bwd = (mode == OPD_RKL_TOPK || (mode == OPD_FKL_TOPK && (flags & OPD_F_RENORM_STUDENT)));
+#ifdef OPD_EXPERIMENTS
+    if (env_int("OPD_DENSE_BWD", 0)) p.sparse_bwd = false;     // timing experiment: run the dense backward anyway
+#endif
     // sparse backward with [d,V] storage works on [V,d] transposes (contiguous d-vectors per cached column)
     p.off_wt = take(bwd && p.sparse_bwd ? (size_t)d * V * (fp32 ? 4 : 2) : 0);
     p.off_gwt = take(bwd && p.sparse_bwd ? (size_t)d * V * 4 : 0);
+    p.off_gw32 = take(bwd && (flags & OPD_F_GRADW_BF16) ? (size_t)d * V * 4 : 0);      // fp32 sums behind a bf16 grad_W
+    p.off_seq_l1 = take(sizeof(float) * (size_t)p.t_pad);                               // per-token terms of opd_set_seq_diagnostics
+    p.off_seq_var1 = take(sizeof(float) * (size_t)p.t_pad);
     p.gs_plane = (size_t)p.Tb * p.Vb;
     p.gs_bufs = std::min(3, std::max(2, env_int("OPD_G_BUFS", 2)));
     p.n_super = ceil_div(p.t_pad, p.Tb) * ceil_div(V, p.Vb);
-    p.off_counters = take(bwd ? sizeof(int) * 2 * (size_t)p.n_super : 0);
+    p.off_counters = take(bwd ? sizeof(int) * (2 * (size_t)p.n_super + 1) : 0);      // g_done, c_done, tile ticket
     // The per-tile LSE partials are dead once the estimators have run, the G ring and the grad_hidden partial
     // sums only live in the backward: they share one region.
     const size_t partial_bytes = align_up(sizeof(float2) * (size_t)p.num_n * p.t_pad, 1024);
@@ -168,21 +193,36 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int 
 
 // ---------------------------------------------------------------- GEMM launcher
 // Launch `kernel` on `grid` CTAs of GEMM_THREADS threads; CG = 2 launches clusters of two CTAs (a pair per tile).
+// `window` (optional): an L2 access-policy window for this launch only (persisting hits inside [base, base + bytes)).
+struct L2Window { void* base = nullptr; size_t bytes = 0; float hit_ratio = 1.f; };
 template <int CG, class... KArgs, class... Args>
-inline cudaError_t launch_cg(void (*kernel)(KArgs...), int grid, cudaStream_t st, Args&&... args) {
+inline cudaError_t launch_cg_w(void (*kernel)(KArgs...), int grid, cudaStream_t st, const L2Window& window, Args&&... args) {
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<CG>::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid); cfg.blockDim = dim3(GEMM_THREADS); cfg.dynamicSmemBytes = Cfg<CG>::SMEM_BYTES; cfg.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
+    if (window.base && window.bytes) {
+        attr[1].id = cudaLaunchAttributeAccessPolicyWindow;
+        attr[1].val.accessPolicyWindow.base_ptr = window.base;
+        attr[1].val.accessPolicyWindow.num_bytes = window.bytes;
+        attr[1].val.accessPolicyWindow.hitRatio = window.hit_ratio;
+        attr[1].val.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+        attr[1].val.accessPolicyWindow.missProp = cudaAccessPropertyNormal;
+        cfg.numAttrs = 2;
+    }
     return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
+template <int CG, class... KArgs, class... Args>
+inline cudaError_t launch_cg(void (*kernel)(KArgs...), int grid, cudaStream_t st, Args&&... args) {
+    return launch_cg_w<CG>(kernel, grid, st, L2Window{}, std::forward<Args>(args)...);
+}
 
-// Number of clusters (CG = 2) / CTAs (CG = 1) of `kernel` that can be resident at the same time on the device: the
-// persistent backward sizes its grid with it, because its tiles wait on tiles of other CTAs (all must be resident).
+// Number of clusters (CG = 2) / CTAs (CG = 1) of `kernel` that can be resident at the same time on the current device:
+// the persistent kernels size their grid with it (one wave; more CTAs would only queue behind the resident ones).
 template <int CG, class... KArgs>
 inline int max_resident_groups(void (*kernel)(KArgs...), int num_sms) {
     if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<CG>::SMEM_BYTES) != cudaSuccess) return 0;

@@ -18,6 +18,21 @@ using namespace opd;
         if (_e != cudaSuccess) OPD_FAIL(h, OPD_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(_e)); \
     } while (0)
 
+// Makes the handle's device current for the duration of an entry point and restores the caller's device afterwards
+// (a library call must not change the caller's / torch's current device in a multi-GPU process).
+struct DeviceGuard {
+    int prev = -1, dev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int device) : dev(device) {
+        ok = cudaGetDevice(&prev) == cudaSuccess;
+        if (ok && prev != dev) ok = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (prev >= 0 && prev != dev) cudaSetDevice(prev); }
+};
+#define OPD_ON_DEVICE(h)                                                                                       \
+    DeviceGuard _device_guard((h)->device);                                                                    \
+    if (!_device_guard.ok) OPD_FAIL(h, OPD_ERR_CUDA, "cannot make device %d current", (h)->device)
+
 extern "C" const char* opd_version(void) { return "opd-b200 0.1 (sm_100a, tcgen05/TMEM/TMA)"; }
 
 extern "C" opd_status_t opd_create(opd_handle_t* out, int device) {
@@ -30,6 +45,7 @@ extern "C" opd_status_t opd_create(opd_handle_t* out, int device) {
     if (e != cudaSuccess) { delete h; return OPD_ERR_CUDA; }
     h->num_sms = prop.multiProcessorCount;
     h->arch_ok = (prop.major == 10);
+    h->l2_bytes = prop.l2CacheSize; h->l2_persist_max = prop.persistingL2CacheMaxSize; h->l2_window_max = prop.accessPolicyMaxWindowSize;
     *out = h;
     return OPD_OK;
 }
@@ -78,9 +94,16 @@ extern "C" opd_status_t opd_set_workspace(opd_handle_t h, void* ws, size_t bytes
     return OPD_OK;
 }
 
-static opd_status_t ensure_workspace(opd_handle_s* h, size_t need) {
+// The handle-owned workspace only ever grows.  Growing it frees and reallocates device memory, which synchronises the
+// device: a call whose shapes need more scratch than any earlier call on the handle is NOT asynchronous (documented in
+// opd.h; opd_set_workspace avoids it).  Inside a stream capture that is impossible: OPD_ERR_WORKSPACE instead.
+static opd_status_t ensure_workspace(opd_handle_s* h, size_t need, cudaStream_t st) {
     if (h->ws && h->ws_bytes >= need) return OPD_OK;
     if (h->ws && !h->ws_owned) OPD_FAIL(h, OPD_ERR_WORKSPACE, "caller workspace has %zu bytes, %zu needed", h->ws_bytes, need);
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone)
+        OPD_FAIL(h, OPD_ERR_WORKSPACE, "the workspace must grow to %zu bytes, which cannot happen inside a stream capture: run the "
+                 "call once eagerly with these shapes, or provide memory with opd_set_workspace", need);
     if (h->ws) { cudaFree(h->ws); h->ws = nullptr; h->ws_bytes = 0; }
     cudaError_t e = cudaMalloc(&h->ws, need);
     if (e != cudaSuccess) { h->ws = nullptr; OPD_FAIL(h, OPD_ERR_WORKSPACE, "cudaMalloc(%zu) failed: %s", need, cudaGetErrorString(e)); }
@@ -103,10 +126,21 @@ extern "C" opd_status_t opd_set_phase_events(opd_handle_t h, void** events) {
     return OPD_OK;
 }
 
-extern "C" opd_status_t opd_set_diagnostics(opd_handle_t h, float* rho_out, long ld_rho, float* var1_out) {
+extern "C" opd_status_t opd_set_diagnostics(opd_handle_t h, int rows, int cols, float* rho_out, long ld_rho, float* var1_out) {
     if (!h) return OPD_ERR_BAD_ARG;
-    if (rho_out && ld_rho < 1) OPD_FAIL(h, OPD_ERR_BAD_ARG, "ld_rho must be >= the cache width");
+    if ((rho_out || var1_out) && rows < 1) OPD_FAIL(h, OPD_ERR_BAD_ARG, "rows must be the number of token rows the arrays hold");
+    if (rho_out && (cols < 1 || ld_rho < cols)) OPD_FAIL(h, OPD_ERR_BAD_ARG, "rho_out needs cols >= 1 and ld_rho >= cols");
     h->diag_rho = rho_out; h->diag_ld_rho = ld_rho; h->diag_var1 = var1_out;
+    h->diag_rows = (rho_out || var1_out) ? rows : 0; h->diag_cols = rho_out ? cols : 0;
+    return OPD_OK;
+}
+
+extern "C" opd_status_t opd_set_seq_diagnostics(opd_handle_t h, int n_seq, const int* cu_seqlens,
+                                                float* seq_mean_m, float* seq_mean_1, float* seq_var_m) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    if (n_seq < 0 || (n_seq > 0 && (!cu_seqlens || !seq_mean_m || !seq_mean_1 || !seq_var_m)))
+        OPD_FAIL(h, OPD_ERR_BAD_ARG, "n_seq > 0 needs cu_seqlens and the three output arrays");
+    h->seq_n = n_seq; h->seq_cu = cu_seqlens; h->seq_mean_m = seq_mean_m; h->seq_mean_1 = seq_mean_1; h->seq_var_m = seq_var_m;
     return OPD_OK;
 }
 

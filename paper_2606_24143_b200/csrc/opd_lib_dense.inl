@@ -24,7 +24,7 @@ static DensePlan make_dense_plan(int T, int d, int dT, int V, int fp32, unsigned
     p.off_lse2_t = take(sizeof(float) * (size_t)p.base.t_pad);
     p.off_acc_a = take(sizeof(float) * (size_t)p.base.t_pad);
     p.off_acc_b = take(sizeof(float) * (size_t)p.base.t_pad);
-    p.off_qdone = take(sizeof(int) * 3 * (size_t)p.base.n_super);      // q_done, g_done, c_done
+    p.off_qdone = take(sizeof(int) * (3 * (size_t)p.base.n_super + 1));      // q_done, g_done, c_done, tile ticket
     p.total = o;
     return p;
 }
@@ -69,12 +69,12 @@ extern "C" opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, 
     }
     if (!get_encode_fn()) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
 
-    OPD_CUDA(h, cudaSetDevice(h->device));
+    OPD_ON_DEVICE(h);
     h->cg = cta_group_setting();
     const uint32_t b_box = BN / h->cg;
     const DensePlan dp = make_dense_plan(T, d, dT, V, fp32, flags);
     const Plan& p = dp.base;
-    s = ensure_workspace(h, dp.total);
+    s = ensure_workspace(h, dp.total, st);
     if (s != OPD_OK) return s;
     h->n_kernels = h->n_gemm = 0;
     h->super_rows = p.Tb; h->super_cols = p.Vb;
@@ -102,10 +102,12 @@ extern "C" opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, 
     OPD_CUDA(h, cudaMemsetAsync(per_token_kl, 0, sizeof(float) * T, st));
     if (!fwd_only) {
         OPD_CUDA(h, cudaMemset2DAsync(grad_hidden, (size_t)ld_gh * esz, 0, (size_t)d * esz, T, st));
-        if (!(flags & OPD_F_GRADW_ACCUM))
-            OPD_CUDA(h, cudaMemset2DAsync(grad_W, (size_t)ldgw * 4, 0, (size_t)(wl == 0 ? V : d) * 4, wl == 0 ? d : V, st));
     }
     k_compact<<<1, 1024, 0, st>>>(mask, T, 0, live_rows, n_live);
+    if (!fwd_only && !(flags & OPD_F_GRADW_ACCUM)) {       // the first token super-tile stores grad_W; zeros only if no token is live
+        k_zero_matrix<<<h->num_sms * 4, 256, 0, st>>>(static_cast<float*>(grad_W), ldgw, wl == 0 ? d : V, wl == 0 ? V : d, n_live);
+        h->n_kernels++;
+    }
     k_gather_rows<<<p.t_pad, 256, 0, st>>>(hidden, ld_hidden, fp32 ? 1 : 0, d, p.t_pad, live_rows, n_live, xc, (long)p.xc_plane);
     k_gather_rows<<<p.t_pad, 256, 0, st>>>(teacher_hidden, ld_th, fp32 ? 1 : 0, dT, p.t_pad, live_rows, n_live, txc, (long)dp.txc_plane);
     h->n_kernels += 3;
@@ -171,10 +173,12 @@ extern "C" opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, 
     // ---- pass B: Q / G (/ grad_hidden / grad_W) tiles in one persistent launch
     int* q_done = reinterpret_cast<int*>(ws + dp.off_qdone);
     int* counters = q_done + p.n_super;
-    OPD_CUDA(h, cudaMemsetAsync(q_done, 0, sizeof(int) * 3 * (size_t)p.n_super, st));
+    OPD_CUDA(h, cudaMemsetAsync(q_done, 0, sizeof(int) * (3 * (size_t)p.n_super + 1), st));
     BwdParams bp{};
     bp.d = d; bp.V = V; bp.Tb = p.Tb; bp.Vb = p.Vb; bp.nvb = ceil_div(V, p.Vb); bp.wl = wl; bp.planes = p.planes; bp.gbufs = p.gs_bufs;
     bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super; bp.q_done = q_done;
+    bp.ticket = counters + 2 * p.n_super;
+    bp.dw_store_first = (flags & OPD_F_GRADW_ACCUM) ? 0 : 1;
     bp.dx = dxp; bp.dw = dwp;
     bp.hint_x = bp.hint_w = bp.hint_g = L2_EVICT_NORMAL;
     bp.dT = dT; bp.wl_t = wlt; bp.qbytes = fp32 ? 4 : 2; bp.q_buf_bytes = dp.q_buf_bytes;

@@ -18,7 +18,7 @@ extern "C" opd_status_t opd_debug_gemm(opd_handle_t h, void* cuda_stream, int M,
     if (!h->arch_ok) OPD_FAIL(h, OPD_ERR_ARCH, "device %d is not compute capability 10.x", h->device);
     if (M < 1 || N < 1 || K < 1 || M % 8 || N % 8 || K % 8) OPD_FAIL(h, OPD_ERR_BAD_SHAPE, "M, N, K must be positive multiples of 8");
     if (!get_encode_fn()) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled not available");
-    OPD_CUDA(h, cudaSetDevice(h->device));
+    OPD_ON_DEVICE(h);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     CUtensorMap tA, tB;
     bool ok = true;
@@ -36,6 +36,28 @@ extern "C" opd_status_t opd_debug_gemm(opd_handle_t h, void* cuda_stream, int M,
     StoreEpi::Params ep{D, (long)N};
     h->n_kernels = h->n_gemm = 0;
     OPD_CUDA(h, launch_gemm<StoreEpi>(h, st, tA, tB, gp, ep));
+    return OPD_OK;
+}
+
+// Test aid: n_ctas CTAs that each fill an SM's shared memory (one CTA per SM) and spin for `milliseconds`.  Used to check
+// that the persistent backward completes while another kernel holds SMs (tests/test_robustness_gpu.py).
+__global__ void __launch_bounds__(32) k_occupy(unsigned long long ns) {
+    unsigned long long t0, t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    do {
+        __nanosleep(2000);
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    } while (t - t0 < ns);
+}
+extern "C" opd_status_t opd_debug_occupy(opd_handle_t h, void* cuda_stream, int n_ctas, float milliseconds) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    if (n_ctas < 1 || n_ctas > 1024 || !(milliseconds > 0.f) || milliseconds > 10000.f)
+        OPD_FAIL(h, OPD_ERR_BAD_ARG, "n_ctas in [1,1024], milliseconds in (0, 10000]");
+    OPD_ON_DEVICE(h);
+    const int smem = 200 * 1024;
+    OPD_CUDA(h, cudaFuncSetAttribute(k_occupy, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    k_occupy<<<n_ctas, 32, smem, static_cast<cudaStream_t>(cuda_stream)>>>(static_cast<unsigned long long>(milliseconds * 1e6));
+    OPD_CUDA(h, cudaGetLastError());
     return OPD_OK;
 }
 
@@ -63,20 +85,24 @@ extern "C" opd_status_t opd_loss_fwd_bwd_host_submit(opd_handle_t h, int slot, i
     if (slot < 0 || slot > 1) OPD_FAIL(h, OPD_ERR_BAD_ARG, "slot must be 0 or 1");
     if (h->slot_busy[slot]) OPD_FAIL(h, OPD_ERR_BAD_ARG, "slot %d is in flight: call opd_loss_fwd_bwd_host_wait first", slot);
     if (!hidden_h || !W_h || !idx_h || !lam_h || !mask_h) OPD_FAIL(h, OPD_ERR_BAD_ARG, "null host input");
+    if (flags & OPD_F_GRADW_ACCUM)
+        OPD_FAIL(h, OPD_ERR_BAD_ARG, "OPD_F_GRADW_ACCUM is not available through the host entry points (grad_W is staged on the device "
+                 "per call; accumulate on the host, or use opd_loss_fwd_bwd with a device grad_W)");
     int kf, Km;
     const int C = cache_width(mode, k_or_K, &kf, &Km);
     opd_status_t s = check_shape(h, T, d, V, C);
     if (s != OPD_OK) return s;
-    OPD_CUDA(h, cudaSetDevice(h->device));
+    OPD_ON_DEVICE(h);
     s = host_streams(h);
     if (s != OPD_OK) return s;
     const size_t esz = dtype == OPD_FP32 ? 4 : 2;
     const bool bwd = !(flags & OPD_F_FWD_ONLY);
+    const size_t gwsz = (flags & OPD_F_GRADW_BF16) ? 2 : 4;
     size_t o = 0;
     auto take = [&](size_t b) { size_t r = o; o = align_up(o + b, 256); return r; };
     const size_t o_hid = take((size_t)T * d * esz), o_w = take((size_t)d * V * esz), o_idx = take((size_t)T * C * 4),
                  o_lam = take((size_t)T * C * 4), o_old = take((size_t)T * C * 4), o_mask = take(T), o_loss = take(4),
-                 o_ptk = take((size_t)T * 4), o_gh = take(bwd ? (size_t)T * d * esz : 0), o_gw = take(bwd ? (size_t)d * V * 4 : 0);
+                 o_ptk = take((size_t)T * 4), o_gh = take(bwd ? (size_t)T * d * esz : 0), o_gw = take(bwd ? (size_t)d * V * gwsz : 0);
     if (h->stage_bytes[slot] < o) {
         if (h->stage[slot]) cudaFree(h->stage[slot]);
         h->stage[slot] = nullptr; h->stage_bytes[slot] = 0;
@@ -98,7 +124,7 @@ extern "C" opd_status_t opd_loss_fwd_bwd_host_submit(opd_handle_t h, int slot, i
     OPD_CUDA(h, cudaStreamWaitEvent(sc, h->ev_in[slot], 0));
     s = opd_loss_fwd_bwd(h, sc, T, d, V, dtype, sb + o_hid, d, sb + o_w, V, 1, reinterpret_cast<int*>(sb + o_idx), C,
                          reinterpret_cast<float*>(sb + o_lam), old_h ? reinterpret_cast<float*>(sb + o_old) : nullptr, sb + o_mask,
-                         mode, k_or_K, flags & ~OPD_F_GRADW_ACCUM, norm_override, reinterpret_cast<float*>(sb + o_loss),
+                         mode, k_or_K, flags, norm_override, reinterpret_cast<float*>(sb + o_loss),
                          reinterpret_cast<float*>(sb + o_ptk), nullptr, nullptr, bwd ? sb + o_gh : nullptr, d,
                          bwd ? sb + o_gw : nullptr, V, 1);
     if (s != OPD_OK) return s;
@@ -108,7 +134,7 @@ extern "C" opd_status_t opd_loss_fwd_bwd_host_submit(opd_handle_t h, int slot, i
     if (loss_h) OPD_CUDA(h, d2h(loss_h, o_loss, 4));
     if (ptk_h) OPD_CUDA(h, d2h(ptk_h, o_ptk, (size_t)T * 4));
     if (bwd && gh_h) OPD_CUDA(h, d2h(gh_h, o_gh, (size_t)T * d * esz));
-    if (bwd && gw_h) OPD_CUDA(h, d2h(gw_h, o_gw, (size_t)d * V * 4));
+    if (bwd && gw_h) OPD_CUDA(h, d2h(gw_h, o_gw, (size_t)d * V * gwsz));
     OPD_CUDA(h, cudaEventRecord(h->ev_out[slot], sout));
     // the next copy-in into THIS slot must not start before these kernels have consumed it: the caller waits on the slot
     h->slot_h2d[slot] = up; h->slot_d2h[slot] = down; h->slot_busy[slot] = true;

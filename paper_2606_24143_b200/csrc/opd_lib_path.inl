@@ -16,20 +16,24 @@ struct PathIO {
     float* dbg_logits; float* dbg_gathered; bool stop_after_fwd; bool all_live;
 };
 
-// Launch the persistent backward kernel on as many CTAs (pairs) as can be resident at once: its tiles wait on tiles of
-// other CTAs through counters in global memory, so every CTA of the grid must be running.
+// Launch the persistent backward kernel on as many CTAs (pairs) as can be resident at once on the handle's device (one
+// wave).  Tiles are claimed dynamically in dependency order (opd_bwd_kernel.cuh), so the kernel also completes when fewer
+// CTAs than that get to run (another kernel holding SMs, MPS, SM-limited contexts): residency is a speed matter only.
 template <bool DENSE>
 static opd_status_t launch_bwd(opd_handle_s* h, cudaStream_t st, const CUtensorMap& m_xc_k, const CUtensorMap& m_w_fwd,
                                const CUtensorMap& m_gs_k, const CUtensorMap& m_w_dx, const CUtensorMap& m_xc_mn,
-                               const CUtensorMap& m_gs_mn, const CUtensorMap& m_tx_k, const CUtensorMap& m_wt_fwd, const BwdParams& bp) {
-    static int resident[3] = {0, -1, -1};
-    if (resident[h->cg] < 0)
-        resident[h->cg] = h->cg == 2 ? max_resident_groups<2>(bwd_kernel<2, DENSE>, h->num_sms)
-                                     : max_resident_groups<1>(bwd_kernel<1, DENSE>, h->num_sms);
-    if (resident[h->cg] < 1) OPD_FAIL(h, OPD_ERR_CUDA, "the backward kernel cannot be made resident on device %d", h->device);
-    const int grid = resident[h->cg] * h->cg;
-    if (h->cg == 2) OPD_CUDA(h, launch_cg<2>(bwd_kernel<2, DENSE>, grid, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
-    else OPD_CUDA(h, launch_cg<1>(bwd_kernel<1, DENSE>, grid, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
+                               const CUtensorMap& m_gs_mn, const CUtensorMap& m_tx_k, const CUtensorMap& m_wt_fwd, const BwdParams& bp,
+                               const L2Window& win = L2Window{}) {
+    int& cached = h->bwd_grid[h->cg][DENSE ? 1 : 0];      // per handle = per device; a failed query is not cached
+    if (cached < 1) {
+        const int r = h->cg == 2 ? max_resident_groups<2>(bwd_kernel<2, DENSE>, h->num_sms)
+                                 : max_resident_groups<1>(bwd_kernel<1, DENSE>, h->num_sms);
+        if (r < 1) OPD_FAIL(h, OPD_ERR_CUDA, "the backward kernel cannot be made resident on device %d", h->device);
+        cached = r * h->cg;
+    }
+    const int grid = cached;
+    if (h->cg == 2) OPD_CUDA(h, launch_cg_w<2>(bwd_kernel<2, DENSE>, grid, st, win, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
+    else OPD_CUDA(h, launch_cg_w<1>(bwd_kernel<1, DENSE>, grid, st, win, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
     return OPD_OK;
 }
 
@@ -47,7 +51,7 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     opd_status_t s = check_shape(h, T, d, V, C);
     if (s != OPD_OK) return s;
     if (a.mode == OPD_MIXED && (kf < 1 || Km < 1)) OPD_FAIL(h, OPD_ERR_BAD_SHAPE, "OPD_MIXED needs k>=1 and K>=1 (k_or_K = k | K<<16)");
-    const unsigned known = OPD_F_NO_RENORM_TEACHER | OPD_F_RENORM_STUDENT | OPD_F_GRADW_ACCUM | OPD_F_VALIDATE_IDX |
+    const unsigned known = OPD_F_NO_RENORM_TEACHER | OPD_F_RENORM_STUDENT | OPD_F_GRADW_ACCUM | OPD_F_GRADW_BF16 | OPD_F_VALIDATE_IDX |
                            OPD_F_FWD_ONLY | OPD_F_SUR_CLIP | OPD_F_SUR_A_OLD;
     if (a.flags & ~known) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unknown flag bits 0x%x", a.flags & ~known);
     const bool fwd_only = (a.flags & OPD_F_FWD_ONLY) || a.stop_after_fwd;
@@ -67,23 +71,24 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         a.ld_hidden < d)
         OPD_FAIL(h, OPD_ERR_BAD_ARG, "hidden / W must be 16-byte aligned with row strides that are multiples of %d elements", al);
     if (a.ld_cache < C) OPD_FAIL(h, OPD_ERR_BAD_ARG, "ld_cache %ld < C %d", a.ld_cache, C);
-    long ldgw = 0;
+    long ldgw = 0;                                 // row stride of the caller's grad_W (elements of ITS dtype)
+    const bool gw_bf16 = !fwd_only && (a.flags & OPD_F_GRADW_BF16);
     if (!fwd_only) {
         const int gwl = (a.ldgw_v == 1) ? 0 : ((a.ldgw_k == 1) ? 1 : -1);
         if (gwl != wl && !(wl == 0 && a.ldgw_v == 1) ) OPD_FAIL(h, OPD_ERR_BAD_ARG, "grad_W must use the same unit stride as W");
         ldgw = wl == 0 ? a.ldgw_k : a.ldgw_v;
-        if (ldgw < (wl == 0 ? V : d) || ldgw % 4 || (reinterpret_cast<uintptr_t>(a.grad_W) & 15))
-            OPD_FAIL(h, OPD_ERR_BAD_ARG, "grad_W must be 16-byte aligned, row stride a multiple of 4 and >= the inner extent");
+        if (ldgw < (wl == 0 ? V : d) || ldgw % (gw_bf16 ? 8 : 4) || (reinterpret_cast<uintptr_t>(a.grad_W) & 15))
+            OPD_FAIL(h, OPD_ERR_BAD_ARG, "grad_W must be 16-byte aligned, row stride a multiple of %d and >= the inner extent", gw_bf16 ? 8 : 4);
         if (a.ld_gh < d || a.ld_gh % al || (reinterpret_cast<uintptr_t>(a.grad_hidden) & 15))
             OPD_FAIL(h, OPD_ERR_BAD_ARG, "grad_hidden must be 16-byte aligned with a row stride that is a multiple of %d", al);
     }
     if (!get_encode_fn()) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
 
-    OPD_CUDA(h, cudaSetDevice(h->device));
+    OPD_ON_DEVICE(h);
     h->cg = cta_group_setting();
     const uint32_t b_box = BN / h->cg;                    // rows of a K-major B box: each CTA of a pair loads half of N
     const Plan p = make_plan(T, d, V, C, fp32, a.flags | (a.stop_after_fwd ? OPD_F_FWD_ONLY : 0), (int)a.mode);
-    s = ensure_workspace(h, p.total);
+    s = ensure_workspace(h, p.total, st);
     if (s != OPD_OK) return s;
     h->n_kernels = h->n_gemm = 0;
     h->super_rows = p.Tb; h->super_cols = p.Vb;
@@ -103,6 +108,12 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     __nv_bfloat16* gs = reinterpret_cast<__nv_bfloat16*>(ws + p.off_gs);
     float* dxacc = reinterpret_cast<float*>(ws + p.off_dxacc);
     double* block_sums = reinterpret_cast<double*>(ws + p.off_block_sums);
+    // fp32 array the backward accumulates grad_W in: the caller's, or (OPD_F_GRADW_BF16) a dense scratch copy that is
+    // rounded into the caller's bf16 array at the end (k_emit_bf16)
+    const int gw_rows = wl == 0 ? d : V, gw_cols = wl == 0 ? V : d;
+    float* gw32 = gw_bf16 ? reinterpret_cast<float*>(ws + p.off_gw32) : static_cast<float*>(a.grad_W);
+    const long ldgw32 = gw_bf16 ? gw_cols : ldgw;
+    const bool gw_accum = (a.flags & OPD_F_GRADW_ACCUM) && !gw_bf16;     // accumulate INTO gw32 (bf16: the scratch starts fresh)
 
     // ------------------------------------------------------------------ S0 pre-pass
     phase_mark(h, st, OPD_PHASE_PREP, 0);
@@ -111,10 +122,14 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     if (a.per_token_kl) OPD_CUDA(h, cudaMemsetAsync(a.per_token_kl, 0, sizeof(float) * T, st));
     if (!fwd_only) {
         OPD_CUDA(h, cudaMemset2DAsync(a.grad_hidden, (size_t)a.ld_gh * esz, 0, (size_t)d * esz, T, st));
-        if (!(a.flags & OPD_F_GRADW_ACCUM))
-            OPD_CUDA(h, cudaMemset2DAsync(a.grad_W, (size_t)ldgw * 4, 0, (size_t)(wl == 0 ? V : d) * 4, wl == 0 ? d : V, st));
     }
     k_compact<<<1, 1024, 0, st>>>(a.mask, T, a.all_live ? 1 : 0, live_rows, n_live);
+    if (!fwd_only && !gw_accum) {
+        // An overwriting call needs no memset of grad_W: the grad_W tiles of the first token super-tile store (dense
+        // backward).  Only the sparse backward (scatter-adds) and a call without any live token start from zeros.
+        k_zero_matrix<<<h->num_sms * 4, 256, 0, st>>>(gw32, ldgw32, gw_rows, gw_cols, p.sparse_bwd ? nullptr : n_live);
+        h->n_kernels++;
+    }
     k_gather_rows<<<p.t_pad, 256, 0, st>>>(a.hidden, a.ld_hidden, fp32 ? 1 : 0, d, p.t_pad, live_rows, n_live, xc, (long)p.xc_plane);
     k_sort_cache<<<ceil_div(T, 8), 256, 0, st>>>(a.cache_idx, a.ld_cache, a.mask, (int)a.mode, kf, Km, C, V, live_rows, n_live,
                                                  sorted_idx, perm, bad_idx);
@@ -154,12 +169,14 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     DwEpi::Params dwp{};
     if (!fwd_only) {
         ok &= make_map_f32(&dxp.m_acc, dxacc, d, p.Tb, (uint64_t)d * 4);
-        ok &= make_map_f32(&dwp.m_gw, a.grad_W, wl == 0 ? V : d, wl == 0 ? d : V, (uint64_t)ldgw * 4);
+        ok &= make_map_f32(&dwp.m_gw, gw32, gw_cols, gw_rows, (uint64_t)ldgw32 * 4);
         dxp.acc = dxacc; dxp.ld_acc = d; dxp.out = a.grad_hidden; dxp.ld_out = a.ld_gh; dxp.out_fp32 = fp32 ? 1 : 0;
         dxp.live_rows = live_rows;
         dxp.hint = hint_policy(env_int("OPD_HINT_DX", 0));
         dwp.hint = hint_policy(env_int("OPD_HINT_GW", 0));
+#ifdef OPD_EXPERIMENTS
         dxp.dbg = dwp.dbg = env_int("OPD_DBG_ACC", 0);
+#endif
     }
     if (!ok) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled failed");
 
@@ -195,9 +212,19 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         e.mode = (int)a.mode; e.k_fkl = kf; e.K_mc = Km; e.C = C; e.flags = a.flags; e.norm_override = a.norm_override;
         e.lse2 = lse2; e.coef = coef; e.beta = beta; e.per_token_kl = a.per_token_kl; e.lse_out = a.lse_out; e.slp_out = a.slp_out;
         e.block_sums = block_sums;
+        if ((h->diag_rho || h->diag_var1) && (T > h->diag_rows || (h->diag_rho && C > h->diag_cols)))
+            OPD_FAIL(h, OPD_ERR_BAD_ARG, "the diagnostics arrays set with opd_set_diagnostics hold %d x %d entries, this call needs %d x %d",
+                     h->diag_rows, h->diag_cols, T, C);
         e.rho_out = h->diag_rho; e.ld_rho = h->diag_ld_rho; e.var1_out = h->diag_var1;
         if (h->diag_var1) OPD_CUDA(h, cudaMemsetAsync(h->diag_var1, 0, sizeof(float) * T, st));
+        const bool seq_diag = h->seq_n > 0 && (a.mode == OPD_RKL_MC || a.mode == OPD_MIXED);
+        if (seq_diag) { e.seq_l1 = reinterpret_cast<float*>(ws + p.off_seq_l1); e.seq_var1 = reinterpret_cast<float*>(ws + p.off_seq_var1); }
         k_estimator<<<p.est_blocks, 128, 0, st>>>(e);
+        if (seq_diag) {
+            k_seq_diag<<<h->seq_n, 256, 0, st>>>(h->seq_cu, h->seq_n, T, a.mask, (int)a.mode, Km, a.per_token_kl, e.seq_l1, e.seq_var1,
+                                                  h->seq_mean_m, h->seq_mean_1, h->seq_var_m);
+            h->n_kernels++;
+        }
         k_loss_final<<<1, 256, 0, st>>>(block_sums, p.est_blocks, n_live, a.norm_override, a.loss);
         h->n_kernels += 2;
         OPD_CUDA(h, cudaGetLastError());
@@ -210,8 +237,8 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     const bool sparse_bwd = p.sparse_bwd;
     if (!fwd_only && sparse_bwd) {
         const void* Wv = a.W;                                   // [V,d] view of W / grad_W: contiguous d-vectors per column
-        float* gwv = static_cast<float*>(a.grad_W);
-        long ldwv = ldw, ldgv = ldgw;
+        float* gwv = gw32;
+        long ldwv = ldw, ldgv = ldgw32;
         if (wl == 0) {
             void* wt = ws + p.off_wt;
             gwv = reinterpret_cast<float*>(ws + p.off_gwt);
@@ -230,7 +257,7 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         h->n_kernels++;
         if (wl == 0) {                                          // grad_W[d,V] += gWt^T
             const dim3 tg(ceil_div(d, 32), ceil_div(V, 32));
-            k_transpose<float><<<tg, dim3(32, 8), 0, st>>>(gwv, (long)d, V, d, static_cast<float*>(a.grad_W), ldgw, 1);
+            k_transpose<float><<<tg, dim3(32, 8), 0, st>>>(gwv, (long)d, V, d, gw32, ldgw32, 1);
             h->n_kernels++;
         }
         OPD_CUDA(h, cudaGetLastError());
@@ -239,20 +266,51 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         // one persistent kernel walks every super-tile: G re-formation, grad_hidden and grad_W tiles interleaved,
         // ordered by dependency counters in global memory (opd_bwd_kernel.cuh)
         int* counters = reinterpret_cast<int*>(ws + p.off_counters);
-        OPD_CUDA(h, cudaMemsetAsync(counters, 0, sizeof(int) * 2 * (size_t)p.n_super, st));
+        OPD_CUDA(h, cudaMemsetAsync(counters, 0, sizeof(int) * (2 * (size_t)p.n_super + 1), st));
         BwdParams bp{};
         bp.d = d; bp.V = V; bp.Tb = p.Tb; bp.Vb = p.Vb; bp.nvb = ceil_div(V, p.Vb); bp.wl = wl; bp.planes = p.planes; bp.gbufs = p.gs_bufs;
-        bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super;
-        bp.g = GEpi::Params{gs, p.Tb, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V};
+        bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super; bp.ticket = counters + 2 * p.n_super;
+        bp.dw_store_first = gw_accum ? 0 : 1;
+        bp.g = GEpi::Params{gs, p.Tb, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V, 0ull};
+        { const int gh_ = env_int("OPD_HINT_GST", 0); bp.g.st_hint = gh_ ? hint_policy(gh_) : 0ull; }
         bp.dx = dxp;
         bp.dw = dwp;
         bp.hint_x = hint_policy(env_int("OPD_HINT_X", 0)); bp.hint_w = hint_policy(env_int("OPD_HINT_W", 0));
         bp.hint_g = hint_policy(env_int("OPD_HINT_G", 0));
-        bp.type_mask = env_int("OPD_BWD_TYPES", 7) & 7;
-        // every CTA (pair) must be resident at once: items wait on earlier items of other CTAs
-        opd_status_t ls = launch_bwd<false>(h, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_xc_k, m_w_fwd, bp);
+        bp.type_mask = 7;
+#ifdef OPD_EXPERIMENTS
+        bp.type_mask = env_int("OPD_BWD_TYPES", 7) & 7;       // timing experiment: subsets give wrong gradients
+#endif
+        // L2 residency experiments: persisting carve-out (device limit) + access-policy window over the G ring / partial sums
+        L2Window win{};
+        {
+            const int pm = env_int("OPD_L2_PERSIST_MB", -1);
+            if (pm >= 0) {
+                const size_t want = std::min<size_t>((size_t)pm << 20, (size_t)h->l2_persist_max);
+                if (want != h->l2_persist) { OPD_CUDA(h, cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want)); h->l2_persist = want; }
+            }
+            const int wm = env_int("OPD_L2_WINDOW", 0);
+            const size_t gs_b = 2 * p.gs_plane * p.planes * p.gs_bufs, dx_b = sizeof(float) * (size_t)p.Tb * d;
+            if (wm == 1) { win.base = gs; win.bytes = gs_b + dx_b; }
+            else if (wm == 2) { win.base = gs; win.bytes = gs_b; }
+            else if (wm == 3) { win.base = dxacc; win.bytes = dx_b; }
+            if (win.bytes) {
+                win.bytes = std::min<size_t>(win.bytes, (size_t)h->l2_window_max);
+                win.hit_ratio = h->l2_persist ? std::min(1.f, (float)h->l2_persist / (float)win.bytes) : 1.f;
+                if (env_int("OPD_L2_VERBOSE", 0))
+                    std::fprintf(stderr, "[opd] L2 %d B, persist max %d, window max %d, carve-out %zu, window %zu B hit %.2f\n",
+                                 h->l2_bytes, h->l2_persist_max, h->l2_window_max, h->l2_persist, win.bytes, win.hit_ratio);
+            }
+        }
+        opd_status_t ls = launch_bwd<false>(h, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_xc_k, m_w_fwd, bp, win);
         if (ls != OPD_OK) return ls;
         h->n_kernels++; h->n_gemm++;
+        OPD_CUDA(h, cudaGetLastError());
+    }
+    if (gw_bf16) {       // round the fp32 sums into the caller's bf16 grad_W (added to its old contents with OPD_F_GRADW_ACCUM)
+        k_emit_bf16<<<h->num_sms * 8, 256, 0, st>>>(gw32, ldgw32, gw_rows, gw_cols, static_cast<__nv_bfloat16*>(a.grad_W), ldgw,
+                                                     (a.flags & OPD_F_GRADW_ACCUM) ? 1 : 0);
+        h->n_kernels++;
         OPD_CUDA(h, cudaGetLastError());
     }
     phase_mark(h, st, OPD_PHASE_BWD, 1);

@@ -69,11 +69,11 @@ static opd_status_t run_producer(opd_handle_s* h, cudaStream_t st, int which, in
     if (ld_idx < n || ld_logp < n || (which == 1 && ld_u < n)) OPD_FAIL(h, OPD_ERR_BAD_ARG, "output / uniform row stride smaller than %d", n);
     if (!get_encode_fn()) OPD_FAIL(h, OPD_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
 
-    OPD_CUDA(h, cudaSetDevice(h->device));
+    OPD_ON_DEVICE(h);
     h->cg = cta_group_setting();
     const uint32_t b_box = BN / h->cg;
     const ProducerPlan p = make_producer_plan(T, d, V, fp32, which == 0 ? n : 0, which == 1 ? n : 0);
-    s = ensure_workspace(h, p.total);
+    s = ensure_workspace(h, p.total, st);
     if (s != OPD_OK) return s;
     h->n_kernels = h->n_gemm = 0;
     uint8_t* ws = static_cast<uint8_t*>(h->ws);

@@ -85,6 +85,42 @@ __global__ void __launch_bounds__(256) k_split_matrix(const float* __restrict__ 
     }
 }
 
+// Zero an fp32 matrix (rows x cols, row stride ld).  With `only_if_empty` set, only when *only_if_empty == 0: the dense
+// backward overwrites grad_W itself (its first token super-tile stores) unless the call has no live token at all.
+__global__ void __launch_bounds__(256) k_zero_matrix(float* __restrict__ m, long ld, int rows, int cols, const int* __restrict__ only_if_empty) {
+    if (only_if_empty != nullptr && *only_if_empty != 0) return;
+    const size_t n4 = static_cast<size_t>(rows) * (cols / 4);
+    for (size_t e = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; e < n4; e += static_cast<size_t>(gridDim.x) * blockDim.x) {
+        const size_t r = e / (cols / 4), c = e - r * (cols / 4);
+        reinterpret_cast<float4*>(m + r * ld)[c] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
+// out (bf16, row stride ldo) = round(acc) or round(out + acc): the final emit of OPD_F_GRADW_BF16 (sums are kept in fp32)
+__global__ void __launch_bounds__(256) k_emit_bf16(const float* __restrict__ acc, long lda, int rows, int cols,
+                                                   __nv_bfloat16* __restrict__ out, long ldo, int accumulate) {
+    const size_t n8 = static_cast<size_t>(rows) * (cols / 8);
+    for (size_t e = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; e < n8; e += static_cast<size_t>(gridDim.x) * blockDim.x) {
+        const size_t r = e / (cols / 8), c = (e - r * (cols / 8)) * 8;
+        const float4 a0 = *reinterpret_cast<const float4*>(acc + r * lda + c), a1 = *reinterpret_cast<const float4*>(acc + r * lda + c + 4);
+        float v[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+        uint4* o = reinterpret_cast<uint4*>(out + r * ldo + c);
+        if (accumulate) {
+            const uint4 old = *o;
+            const uint32_t w[4] = {old.x, old.y, old.z, old.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const __nv_bfloat162 h2 = *reinterpret_cast<const __nv_bfloat162*>(&w[i]);
+                v[2 * i] += __low2float(h2); v[2 * i + 1] += __high2float(h2);
+            }
+        }
+        uint32_t w[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { __nv_bfloat162 t = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]); w[i] = *reinterpret_cast<uint32_t*>(&t); }
+        *o = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+}
+
 // ------------------------------------------------------------------------------------------ S0c
 // Per live row: ascending (stable) sort of the first C_row cache indices by rank counting; keeps the
 // permutation so outputs go back in caller slot order.  One warp per compact row.

@@ -18,14 +18,14 @@ OPD_OK = 0
 ERR_BAD_ARG, ERR_BAD_SHAPE, ERR_BAD_INDEX, ERR_WORKSPACE, ERR_ARCH, ERR_CUDA = -1, -2, -3, -4, -5, -6
 FKL_TOPK, RKL_MC, MIXED, RKL_TOPK = 0, 1, 2, 3
 BF16, FP32 = 0, 1
-F_NO_RENORM_TEACHER, F_RENORM_STUDENT, F_GRADW_ACCUM, F_VALIDATE_IDX, F_FWD_ONLY = 1, 2, 4, 16, 32
-F_SUR_CLIP, F_SUR_A_OLD = 64, 128
+F_NO_RENORM_TEACHER, F_RENORM_STUDENT, F_GRADW_ACCUM, F_GRADW_BF16, F_VALIDATE_IDX, F_FWD_ONLY = 1, 2, 4, 8, 16, 32
+F_SUR_CLIP, F_SUR_A_OLD, F_DENSE_REVERSE = 64, 128, 256
 N_PHASES = 4
 PHASE_NAMES = ("prep", "fwd", "est", "bwd")
 
 EXPORTS = ("opd_create", "opd_destroy", "opd_last_error", "opd_version", "opd_workspace_bytes", "opd_set_workspace",
            "opd_loss_fwd_bwd", "opd_loss_fwd_bwd_host", "opd_loss_fwd_bwd_host_submit", "opd_loss_fwd_bwd_host_wait", "opd_debug_logits", "opd_debug_gemm", "opd_last_launch_stats",
-           "opd_set_phase_events", "opd_set_diagnostics", "opd_cache_workspace_bytes", "opd_cache_topk", "opd_cache_sample",
+           "opd_set_phase_events", "opd_set_diagnostics", "opd_set_seq_diagnostics", "opd_debug_occupy", "opd_cache_workspace_bytes", "opd_cache_topk", "opd_cache_sample",
            "opd_dense_kl_workspace_bytes", "opd_dense_kl_fwd_bwd")
 
 _lib = None
@@ -91,8 +91,12 @@ def load_library():
                                          c_void_p, c_long, c_void_p, c_long, c_long, c_void_p, c_uint, c_float,
                                          c_void_p, c_void_p, c_void_p, c_long, c_void_p, c_long, c_long]
     lib.opd_dense_kl_fwd_bwd.restype = c_int
-    lib.opd_set_diagnostics.argtypes = [c_void_p, c_void_p, c_long, c_void_p]
+    lib.opd_set_diagnostics.argtypes = [c_void_p, c_int, c_int, c_void_p, c_long, c_void_p]
     lib.opd_set_diagnostics.restype = c_int
+    lib.opd_set_seq_diagnostics.argtypes = [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.opd_set_seq_diagnostics.restype = c_int
+    lib.opd_debug_occupy.argtypes = [c_void_p, c_void_p, c_int, c_float]
+    lib.opd_debug_occupy.restype = c_int
     lib.opd_set_phase_events.argtypes = [c_void_p, c_void_p]
     lib.opd_set_phase_events.restype = c_int
     _lib = lib
@@ -113,9 +117,59 @@ def _dtype_code(t: torch.Tensor) -> int:
 
 def _w_strides(W: torch.Tensor, d: int):
     """W is either [d,V] (v contiguous) or a [V,d] weight passed as W.t() view / with layout='vd'."""
-    if W.shape[0] != d:
+    if W.dim() != 2 or W.shape[0] != d:
         raise OpdError(ERR_BAD_SHAPE, f"W must be logical [d,V]; got {tuple(W.shape)} with d={d} (pass weight.t() for a [V,d] weight)")
+    if W.stride(0) != 1 and W.stride(1) != 1:
+        raise OpdError(ERR_BAD_ARG, f"W must be stored [d,V] or [V,d] row-major (one unit stride); strides are {tuple(W.stride())}")
     return W.stride(0), W.stride(1)
+
+
+def _marshal(hidden, W, cache_idx, lam, old, mask, host: bool = False):
+    """Checks what the C ABI cannot see from raw pointers (dtype, device, strides) and normalises the cheap cases:
+    int64 indices -> int32, bool mask -> uint8, non-unit inner strides / unequal cache row strides -> contiguous copies.
+    Everything else raises instead of being reinterpreted silently. Returns the tensors to pass on (keep them alive)."""
+    if hidden.dim() != 2:
+        raise OpdError(ERR_BAD_SHAPE, f"hidden must be [T,d]; got {tuple(hidden.shape)}")
+    T = hidden.shape[0]
+    dev = hidden.device
+    if (dev.type == "cuda") == host:
+        raise OpdError(ERR_BAD_ARG, f"hidden is on {dev}; this entry point takes {'host' if host else 'CUDA'} tensors")
+    for name, t in (("W", W), ("cache_idx", cache_idx), ("cache_teacher_logp", lam), ("cache_old_logp", old), ("mask", mask)):
+        if t is not None and t.device != dev:
+            raise OpdError(ERR_BAD_ARG, f"{name} is on {t.device}, hidden on {dev}")
+    if hidden.stride(1) != 1:
+        hidden = hidden.contiguous()
+    if cache_idx.dim() != 2 or cache_idx.shape[0] != T:
+        raise OpdError(ERR_BAD_SHAPE, f"cache_idx must be [T,C]; got {tuple(cache_idx.shape)}")
+    if cache_idx.dtype == torch.int64:
+        cache_idx = cache_idx.to(torch.int32)
+    elif cache_idx.dtype != torch.int32:
+        raise OpdError(ERR_BAD_ARG, f"cache_idx must be int32 (or int64, converted); got {cache_idx.dtype}")
+    for name, t in (("cache_teacher_logp", lam), ("cache_old_logp", old)):
+        if t is None:
+            continue
+        if t.dtype != torch.float32:
+            raise OpdError(ERR_BAD_ARG, f"{name} must be float32; got {t.dtype}")
+        if tuple(t.shape) != tuple(cache_idx.shape):
+            raise OpdError(ERR_BAD_SHAPE, f"{name} has shape {tuple(t.shape)}, cache_idx {tuple(cache_idx.shape)}")
+    caches = [t for t in (cache_idx, lam, old) if t is not None]
+    if any(t.stride(1) != 1 or t.stride(0) != cache_idx.stride(0) for t in caches) or (host and cache_idx.stride(0) != cache_idx.shape[1]):
+        cache_idx = cache_idx.contiguous()            # the ABI takes ONE row stride for the three cache arrays
+        lam = None if lam is None else lam.contiguous()
+        old = None if old is None else old.contiguous()
+    if mask is not None:
+        if mask.dtype == torch.bool:
+            mask = mask.view(torch.uint8)
+        elif mask.dtype != torch.uint8:
+            raise OpdError(ERR_BAD_ARG, f"mask must be uint8 (or bool); got {mask.dtype}")
+        if mask.dim() != 1 or mask.shape[0] != T:
+            raise OpdError(ERR_BAD_SHAPE, f"mask must be [T]; got {tuple(mask.shape)}")
+        if mask.stride(0) != 1:
+            mask = mask.contiguous()
+    if host:                                           # the host entry points take dense arrays, W as [d,V] row-major
+        hidden = hidden.contiguous()
+        W = W.contiguous()
+    return hidden, W, cache_idx, lam, old, mask
 
 
 class Handle:
@@ -157,9 +211,38 @@ class Handle:
 
     def set_diagnostics(self, rho_out=None, var1_out=None):
         """opd_set_diagnostics: rho_out [T,C] / var1_out [T] float32 device tensors written by the following calls."""
+        for t in (rho_out, var1_out):
+            if t is not None and (t.dtype != torch.float32 or not t.is_cuda or t.stride(-1) != 1):
+                raise OpdError(ERR_BAD_ARG, "diagnostics outputs must be float32 CUDA tensors with a unit inner stride")
         self._diag = (rho_out, var1_out)          # keep the tensors alive
-        self._check(self.lib.opd_set_diagnostics(self._h, _ptr(rho_out), rho_out.stride(0) if rho_out is not None else 0,
-                                                 _ptr(var1_out)))
+        rows = rho_out.shape[0] if rho_out is not None else (var1_out.shape[0] if var1_out is not None else 0)
+        if rho_out is not None and var1_out is not None:
+            rows = min(rows, var1_out.shape[0])
+        self._check(self.lib.opd_set_diagnostics(self._h, rows, rho_out.shape[1] if rho_out is not None else 0, _ptr(rho_out),
+                                                 rho_out.stride(0) if rho_out is not None else 0, _ptr(var1_out)))
+
+    def set_seq_diagnostics(self, cu_seqlens=None):
+        """opd_set_seq_diagnostics: cu_seqlens [n_seq+1] int32 CUDA tensor of sequence boundaries (token offsets). Returns the
+        dict of float32 [n_seq] tensors (seq_mean_m, seq_mean_1, seq_var_m) the following RKL_MC / MIXED calls fill; None
+        switches the hook off."""
+        if cu_seqlens is None:
+            self._seq = None
+            self._check(self.lib.opd_set_seq_diagnostics(self._h, 0, None, None, None, None))
+            return None
+        if cu_seqlens.dtype != torch.int32 or not cu_seqlens.is_cuda or cu_seqlens.dim() != 1 or cu_seqlens.numel() < 2:
+            raise OpdError(ERR_BAD_ARG, "cu_seqlens must be a 1-D int32 CUDA tensor with n_seq + 1 entries")
+        cu = cu_seqlens.contiguous()
+        n = cu.numel() - 1
+        out = {k: torch.zeros(n, dtype=torch.float32, device=cu.device) for k in ("seq_mean_m", "seq_mean_1", "seq_var_m")}
+        self._seq = (cu, out)
+        self._check(self.lib.opd_set_seq_diagnostics(self._h, n, _ptr(cu), _ptr(out["seq_mean_m"]), _ptr(out["seq_mean_1"]),
+                                                     _ptr(out["seq_var_m"])))
+        return out
+
+    def debug_occupy(self, n_ctas: int, milliseconds: float, stream=None):
+        """opd_debug_occupy: keep n_ctas SMs busy for about `milliseconds` on `stream` (a test aid: one CTA per SM)."""
+        s = torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream
+        self._check(self.lib.opd_debug_occupy(self._h, c_void_p(s), n_ctas, float(milliseconds)))
 
     # ------------------------------------------------------------------ phase timing
     def enable_phase_timing(self, on: bool = True):
@@ -174,9 +257,22 @@ class Handle:
             self._events = None
             self.lib.opd_set_phase_events(self._h, None)
 
-    def phase_times_ms(self) -> dict:
+    def phase_times_ms(self, events=None) -> dict:
         torch.cuda.synchronize()
-        return {PHASE_NAMES[i]: self._events[2 * i].elapsed_time(self._events[2 * i + 1]) for i in range(N_PHASES)}
+        ev = self._events if events is None else events[0]
+        return {PHASE_NAMES[i]: ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(N_PHASES)}
+
+    def new_phase_events(self):
+        """A set of 2*N_PHASES timing events (and the C array of their handles) for use_phase_events."""
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * N_PHASES)]
+        for e in ev:                         # force creation of the underlying cudaEvent_t
+            e.record()
+        return ev, (c_void_p * (2 * N_PHASES))(*[c_void_p(e.cuda_event) for e in ev])
+
+    def use_phase_events(self, events):
+        """Record the following calls' phases into `events` (from new_phase_events); None switches the hook off."""
+        self._phase_set = events             # keep alive while the library holds the pointer
+        self.lib.opd_set_phase_events(self._h, None if events is None else ctypes.cast(events[1], c_void_p))
 
     # ------------------------------------------------------------------ the hot path
     def loss_fwd_bwd(self, hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K, flags=0,
@@ -184,14 +280,17 @@ class Handle:
         """opd_loss_fwd_bwd(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K)
         -> dict(loss, per_token_kl, grad_hidden, grad_W[, lse, student_logp]).  All tensors live on the GPU.
         W is the logical [d,V] matrix (any of the two layouts through its strides)."""
+        hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask = _marshal(hidden, W, cache_idx, cache_teacher_logp,
+                                                                                  cache_old_logp, mask)
         T, d = hidden.shape
-        V = W.shape[1]
         dt = _dtype_code(hidden)
         if W.dtype != hidden.dtype:
             raise OpdError(ERR_BAD_ARG, "hidden and W must have the same dtype")
         ldk, ldv = _w_strides(W, d)
+        V = W.shape[1]
         dev = hidden.device
         fwd_only = bool(flags & F_FWD_ONLY)
+        gw_dtype = torch.bfloat16 if flags & F_GRADW_BF16 else torch.float32
         loss = torch.empty(1, dtype=torch.float32, device=dev)
         ptk = torch.empty(T, dtype=torch.float32, device=dev)
         lse = torch.empty(T, dtype=torch.float32, device=dev) if want_lse else None
@@ -201,8 +300,14 @@ class Handle:
         if not fwd_only:
             if grad_hidden is None:
                 grad_hidden = torch.empty_like(hidden)
+            elif grad_hidden.dtype != hidden.dtype or tuple(grad_hidden.shape) != (T, d) or grad_hidden.stride(1) != 1 or grad_hidden.device != dev:
+                raise OpdError(ERR_BAD_ARG, "grad_hidden must be a [T,d] tensor of hidden's dtype and device with a unit inner stride")
             if grad_W is None:
-                grad_W = torch.empty_strided(tuple(W.shape), (ldk, ldv), dtype=torch.float32, device=dev)
+                if flags & F_GRADW_ACCUM:
+                    raise OpdError(ERR_BAD_ARG, "OPD_F_GRADW_ACCUM accumulates into the caller's grad_W: pass it")
+                grad_W = torch.empty_strided(tuple(W.shape), (ldk, ldv), dtype=gw_dtype, device=dev)
+            elif grad_W.dtype != gw_dtype or tuple(grad_W.shape) != (d, V) or grad_W.device != dev:
+                raise OpdError(ERR_BAD_ARG, f"grad_W must be a logical [d,V] {gw_dtype} tensor on {dev}")
         s = torch.cuda.current_stream(dev).cuda_stream if stream is None else stream
         gk, gv = (grad_W.stride(0), grad_W.stride(1)) if grad_W is not None else (0, 0)
         st = self.lib.opd_loss_fwd_bwd(
@@ -219,6 +324,8 @@ class Handle:
                           norm_override=0.0, out=None):
         """Same call with HOST tensors (pinned or pageable, dense); copies in, runs, copies out, synchronises.
         `out`: optional dict of preallocated host tensors (loss, per_token_kl, grad_hidden, grad_W)."""
+        hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask = _marshal(hidden, W, cache_idx, cache_teacher_logp,
+                                                                                  cache_old_logp, mask, host=True)
         T, d = hidden.shape
         V = W.shape[1]
         dt = _dtype_code(hidden)
@@ -226,7 +333,7 @@ class Handle:
         if out is None:
             out = dict(loss=torch.empty(1, dtype=torch.float32), per_token_kl=torch.empty(T, dtype=torch.float32),
                        grad_hidden=None if fwd_only else torch.empty_like(hidden),
-                       grad_W=None if fwd_only else torch.empty(d, V, dtype=torch.float32))
+                       grad_W=None if fwd_only else torch.empty(d, V, dtype=torch.bfloat16 if flags & F_GRADW_BF16 else torch.float32))
         up, down = c_size_t(), c_size_t()
         st = self.lib.opd_loss_fwd_bwd_host(
             self._h, T, d, V, dt, _ptr(hidden), _ptr(W), _ptr(cache_idx), _ptr(cache_teacher_logp), _ptr(cache_old_logp),
@@ -240,6 +347,8 @@ class Handle:
                     norm_override=0.0):
         """opd_loss_fwd_bwd_host_submit: enqueue one step on staging slot 0/1 (host tensors; `out` = dict of host tensors
         loss, per_token_kl, grad_hidden, grad_W that receive the results once host_wait(slot) has returned)."""
+        hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask = _marshal(hidden, W, cache_idx, cache_teacher_logp,
+                                                                                  cache_old_logp, mask, host=True)
         T, d = hidden.shape
         V = W.shape[1]
         self._pending = getattr(self, "_pending", {})

@@ -38,6 +38,7 @@ def test_enum_values_match_header():
     for name, val in [("OPD_FKL_TOPK", opd.FKL_TOPK), ("OPD_RKL_MC", opd.RKL_MC), ("OPD_MIXED", opd.MIXED), ("OPD_BF16", opd.BF16),
                       ("OPD_FP32", opd.FP32), ("OPD_F_NO_RENORM_TEACHER", opd.F_NO_RENORM_TEACHER),
                       ("OPD_F_RENORM_STUDENT", opd.F_RENORM_STUDENT), ("OPD_F_GRADW_ACCUM", opd.F_GRADW_ACCUM),
+                      ("OPD_F_GRADW_BF16", opd.F_GRADW_BF16),
                       ("OPD_F_VALIDATE_IDX", opd.F_VALIDATE_IDX), ("OPD_F_FWD_ONLY", opd.F_FWD_ONLY),
                       ("OPD_F_SUR_CLIP", opd.F_SUR_CLIP), ("OPD_F_SUR_A_OLD", opd.F_SUR_A_OLD),
                       ("OPD_ERR_BAD_INDEX", opd.ERR_BAD_INDEX), ("OPD_ERR_ARCH", opd.ERR_ARCH)]:
@@ -69,6 +70,38 @@ def test_no_cpu_fallback():
         opd.Handle(0)
     src = open(os.path.join(ROOT, "paper_2606_24143_b200", "opd.py")).read()
     assert "oracle" not in src.replace("no CPU fallback", "")
+
+
+def test_wrong_gradient_switches_are_not_in_the_product_library(lib):
+    """OPD_BWD_TYPES / OPD_DBG_ACC / OPD_DENSE_BWD (timing experiments that return wrong gradients) are compiled in only with
+    -DOPD_EXPERIMENTS: the default build never reads them, so a stray environment variable in a training job is inert."""
+    from paper_2606_24143_b200 import opd
+    blob = open(opd.LIB_PATH, "rb").read()
+    for name in (b"OPD_BWD_TYPES", b"OPD_DBG_ACC", b"OPD_DENSE_BWD"):
+        assert name not in blob, name
+    assert b"OPD_TB" in blob          # result-neutral tuning knobs are still read
+
+
+def test_binding_rejects_what_raw_pointers_cannot_express():
+    """Host-side argument marshalling (no GPU needed): dtypes, shapes and strides are checked before any pointer is passed."""
+    import torch
+    from paper_2606_24143_b200 import opd
+    T, d, V, C = 8, 64, 256, 4
+    X = torch.zeros(T, d, dtype=torch.bfloat16); W = torch.zeros(d, V, dtype=torch.bfloat16)
+    idx = torch.zeros(T, C, dtype=torch.int64); lam = torch.zeros(T, C); m = torch.ones(T, dtype=torch.bool)
+    out = opd._marshal(X, W, idx, lam, None, m, host=True)
+    assert out[2].dtype == torch.int32 and out[5].dtype == torch.uint8 and out[4] is None
+    wide = torch.zeros(T, C + 2)
+    out = opd._marshal(X, W, idx.int(), wide[:, :C], None, m, host=True)
+    assert out[3].stride(0) == C and out[2].stride(0) == C
+    for bad in (dict(lam=lam.double()), dict(idx=idx.to(torch.int16)), dict(m=m.to(torch.int32)), dict(lam=lam[:, :-1]), dict(m=m[:-1])):
+        a = dict(idx=idx, lam=lam, m=m); a.update(bad)
+        with pytest.raises(opd.OpdError):
+            opd._marshal(X, W, a["idx"], a["lam"], None, a["m"], host=True)
+    with pytest.raises(opd.OpdError):
+        opd._marshal(X, W, idx, lam, None, m, host=False)            # CPU tensors to the device entry point
+    with pytest.raises(opd.OpdError):
+        opd._w_strides(torch.zeros(d, 2 * V)[:, ::2], d)
 
 
 def test_null_handle_is_an_error(lib):

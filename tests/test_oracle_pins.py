@@ -333,6 +333,102 @@ def test_surrogate_variants_reduce_to_reference():
         assert cl[0] >= nc[0] - 1e-15
 
 
+def _clip_case(seed=71, T=4, d=6, V=12, C=6):
+    """Inputs on which old != ell, A_old != A_theta, and the PPO clip bites in BOTH directions: every row holds slots with
+    rho > 1+eps and rho < 1-eps, each with advantages of both signs (checked by the caller)."""
+    t = tiny(seed, T=T, d=d, V=V, C=C, dup=True, mask=[1, 0, 1, 1])
+    rng = np.random.default_rng(seed)
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    ell = np.take_along_axis(logp, t["idx"], 1)
+    # rollout-time log-probs placed so that rho = exp(ell - old) lands on both sides of the clip range, away from its edges
+    shift = np.array([0.9, -0.9, 0.45, -0.45, 0.05, -0.07])[:C]
+    t["old"] = ell - np.stack([rng.permutation(shift) for _ in range(T)])
+    # teacher scores around both log-probs so that A_theta and A_old take both signs and differ
+    t["lam"] = 0.5 * (ell + t["old"]) + rng.normal(size=ell.shape) * 0.8
+    return t, ell
+
+
+def _ppo_surrogate_from_scratch(X, W, t, A_frozen, clip, eps=0.2):
+    """Eq.(4) / Eq.(6),(7) written out with the expectation over a ~ p_old replaced by the mean over
+    the m cached draws (Eq.(15)):  L = (1/N) sum_t -(1/m) sum_j min(rho_j A_j, clip(rho_j, 1-eps, 1+eps) A_j),
+    rho_j = p_theta(a_j) / p_old(a_j); without clipping the clipped term is dropped.  A is a constant here
+    (stop-gradient): the caller passes A_old = log q - log p_old or A_theta frozen at the base point."""
+    tot, N = 0.0, 0
+    for ti in range(X.shape[0]):
+        if t["mask"][ti] == 0:
+            continue
+        N += 1
+        z = X[ti] @ W
+        lse = math.log(sum(math.exp(v) for v in z))
+        acc = 0.0
+        m = t["idx"].shape[1]
+        for j in range(m):
+            rho = math.exp(z[t["idx"][ti, j]] - lse - t["old"][ti, j])
+            a = A_frozen[ti, j]
+            if clip:
+                acc += min(rho * a, min(max(rho, 1.0 - eps), 1.0 + eps) * a)
+            else:
+                acc += rho * a
+        tot += -acc / m
+    return tot / N
+
+
+@pytest.mark.parametrize("sur", [O.SUR_THETA_NOCLIP, O.SUR_THETA_CLIP, O.SUR_OLD_NOCLIP, O.SUR_OLD_CLIP])
+def test_surrogates_against_eq4_eq6_eq7_written_out(sur):
+    """NEXT-1 pins: value of each of the four surrogates against Eq.(6)/(7) written from scratch (1e-13) and its gradients
+    against central differences of that frozen-A surrogate, on inputs where p_old != p_theta and the clip is active in both
+    directions.  An oracle that ignored the A_old flag, or that let gradient through clipped slots, fails here."""
+    t, ell = _clip_case()
+    live = t["mask"] != 0
+    rho = np.exp(ell - t["old"])
+    A_th, A_old = t["lam"] - ell, t["lam"] - t["old"]
+    for A in (A_th, A_old):                          # the case really exercises all four corners of the clip
+        assert ((rho > 1.2) & (A > 0))[live].any() and ((rho > 1.2) & (A < 0))[live].any()
+        assert ((rho < 0.8) & (A > 0))[live].any() and ((rho < 0.8) & (A < 0))[live].any()
+    assert np.abs(np.abs(rho - 1.0) - 0.2).min() > 1e-3       # no slot sits on a clip edge (finite differences are valid)
+    use_old = sur in (O.SUR_OLD_NOCLIP, O.SUR_OLD_CLIP)
+    clip = sur in (O.SUR_THETA_CLIP, O.SUR_OLD_CLIP)
+    A0 = A_old if use_old else A_th
+    r = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], O.RKL_MC, t["idx"].shape[1], surrogate=sur)
+    f = lambda X, W: _ppo_surrogate_from_scratch(X, W, t, A0, clip)
+    assert abs(r["loss"] - f(t["X"], t["W"])) < 1e-13
+    # discriminating power of the value pin: the other advantage / the other clipping give a different number
+    assert abs(f(t["X"], t["W"]) - _ppo_surrogate_from_scratch(t["X"], t["W"], t, A_th if use_old else A_old, clip)) > 1e-2
+    assert abs(f(t["X"], t["W"]) - _ppo_surrogate_from_scratch(t["X"], t["W"], t, A0, not clip)) > 1e-2
+    h = 1e-6
+    rng = np.random.default_rng(5)
+    probes = [(int(rng.integers(4)), int(rng.integers(6)), int(rng.integers(12))) for _ in range(10)]
+    probes += [(ti, 3, int(t["idx"][ti, j])) for ti in (0, 2, 3) for j in range(t["idx"].shape[1])]
+    worst_noclip_gap = 0.0
+    rn = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], t["old"], t["mask"], O.RKL_MC, t["idx"].shape[1],
+                      surrogate=O.SUR_OLD_NOCLIP if use_old else O.SUR_THETA_NOCLIP)
+    for ti, ki, vi in probes:
+        Xp, Xm = t["X"].copy(), t["X"].copy(); Xp[ti, ki] += h; Xm[ti, ki] -= h
+        fd = (f(Xp, t["W"]) - f(Xm, t["W"])) / (2 * h)
+        assert abs(fd - r["grad_hidden"][ti, ki]) < 2e-8
+        Wp, Wm = t["W"].copy(), t["W"].copy(); Wp[ki, vi] += h; Wm[ki, vi] -= h
+        fd = (f(t["X"], Wp) - f(t["X"], Wm)) / (2 * h)
+        assert abs(fd - r["grad_W"][ki, vi]) < 2e-8
+        worst_noclip_gap = max(worst_noclip_gap, abs(fd - rn["grad_W"][ki, vi]))
+    if clip:        # dropping the clip's "active" mask from the gradient would give the unclipped gradient: visibly different
+        assert worst_noclip_gap > 1e-3
+    assert np.all(r["grad_hidden"][1] == 0)
+
+
+def test_clipped_surrogate_slot_by_slot():
+    """Eq.(4) PAPER.md:72 slot by slot through token_terms (K = 1): in the two clipped corners (rho > 1+eps with A > 0,
+    rho < 1-eps with A < 0) the term is the constant clip(rho) A and carries no gradient; in the other two the unclipped
+    term rho A is the minimum and the gradient is that of rho A (beta = -rho A, alpha = rho A)."""
+    for rho, A in [(1.5, 0.7), (0.6, -0.4), (1.5, -0.7), (0.6, 0.4), (1.1, 0.3), (0.9, -0.3)]:
+        ell, old = -2.0, -2.0 - math.log(rho)
+        for sur, lam in ((O.SUR_THETA_CLIP, ell + A), (O.SUR_OLD_CLIP, old + A)):
+            L, alpha, beta = O.token_terms(O.RKL_MC, [lam], [old], [ell], 0, sur)
+            clipped = (rho > 1.2 and A > 0) or (rho < 0.8 and A < 0)
+            want = -(min(max(rho, 0.8), 1.2) * A) if clipped else -(rho * A)
+            assert abs(L - want) < 1e-15
+            assert abs(alpha - (0.0 if clipped else rho * A)) < 1e-15 and abs(beta[0] + alpha) < 1e-15
+
+
 def test_sparse_reverse_kl_definition_and_gradient():
     """Eq.(9),(10) PAPER.md:293-301: S = V gives dense D_R; gradient by finite differences; D >= 0."""
     t = tiny(17, T=2, d=5, V=8)
@@ -408,6 +504,40 @@ def test_mc_diagnostics():
         assert np.abs(r["rho"][ti] - np.exp(ell - t["old"][ti])).max() < 1e-14
     r1 = O.opd_oracle(t["X"], t["W"], t["idx"][:, :1], t["lam"][:, :1], t["old"][:, :1], t["mask"], O.RKL_MC, 1)
     assert np.all(r1["var1"] == 0)
+
+
+def test_seq_diagnostics_by_enumeration():
+    """Eq.(17) PAPER.md:388-390 on a 2-token toy sequence: enumerating every pair of m-tuples of local draws (prefix path
+    fixed) gives the exact variance of the sequence mean of L^MC_m; the oracle's var_m is an unbiased
+    estimate of it (its expectation over all draws equals it), its mean_m / mean_1 average to the mean dense reverse KL
+    (Eq.(5)), and the ratio of the fixed-path variances is 1/m."""
+    import itertools
+    t = tiny(81, T=2, d=4, V=4)
+    V, m = 4, 2
+    logp, _ = O.log_softmax_rows(t["X"] @ t["W"])
+    po = np.exp(t["logpo"])
+    DR = O.dense_reverse_kl(t["logq"], logp)
+    tuples = list(itertools.product(range(V), repeat=m))
+    E_mean_m = E_mean_1 = E_sq = E_sq1 = E_var = 0.0
+    for a0 in tuples:
+        for a1 in tuples:
+            idx = np.array([a0, a1])
+            pr = float(np.prod(po[0, list(a0)]) * np.prod(po[1, list(a1)]))
+            lam = np.take_along_axis(t["logq"], idx, 1)
+            old = np.take_along_axis(t["logpo"], idx, 1)
+            r = O.opd_oracle(t["X"], t["W"], idx, lam, old, np.ones(2), O.RKL_MC, m, want_grads=False)
+            mm, m1, vm = O.seq_diagnostics(r["per_token_kl"], r["first_draw"], r["var1"], np.ones(2), [0, 2], m)
+            # the pieces, written out: L_m per token is the mean of the per-draw terms, L_1 the first of them
+            x = [[-math.exp(logp[ti, a] - t["logpo"][ti, a]) * (t["logq"][ti, a] - logp[ti, a]) for a in idx[ti]] for ti in range(2)]
+            assert abs(mm[0] - 0.5 * (np.mean(x[0]) + np.mean(x[1]))) < 1e-14 and abs(m1[0] - 0.5 * (x[0][0] + x[1][0])) < 1e-14
+            E_mean_m += pr * mm[0]; E_mean_1 += pr * m1[0]; E_sq += pr * mm[0] ** 2; E_sq1 += pr * m1[0] ** 2; E_var += pr * vm[0]
+    assert abs(E_mean_m - DR.mean()) < 1e-12 and abs(E_mean_1 - DR.mean()) < 1e-12          # Eq.(5), averaged over the sequence
+    var_m, var_1 = E_sq - E_mean_m ** 2, E_sq1 - E_mean_1 ** 2
+    assert abs(E_var - var_m) < 1e-12                                                        # unbiased estimate of Var(mean_m)
+    assert abs(var_m / var_1 - 1.0 / m) < 1e-10                                              # fixed path, iid draws: exactly 1/m
+    # rows outside the sequence, masked rows and (MIXED) non-MC rows do not take part; empty sequences give zeros
+    mm, m1, vm = O.seq_diagnostics([1.0, 2.0, 4.0, 8.0], [1.0, 1.0, 1.0, 1.0], [0.5, 0.5, 0.5, 0.5], [2, 1, 0, 2], [0, 3, 3, 4], 4, mc_code=2)
+    assert np.allclose(mm, [1.0, 0.0, 8.0]) and np.allclose(vm, [0.5 / 4, 0.0, 0.5 / 4])
 
 
 def test_cache_topk_against_library_topk_and_ties():

@@ -5,7 +5,10 @@ one — lse, per-token loss, student log-probs and whole grad_hidden rows of sam
 directly, and (ii) grad_W is checked through properties that hold at any size:
    sum_v grad_W[k,v] = 0                       (softmax shift invariance, pin P10)
    sum_v W[k,v] grad_W[k,v] = sum_t x[t,k] grad_hidden[t,k]   for every k   (both equal <z, G> split by k)
-plus (iii) a few-live-token variant of the 1.7B-class shape where the oracle computes grad_W in full."""
+plus (iii) a few-live-token variant of the 1.7B-class shape where the oracle computes grad_W in full, and (iv) grad_W element by
+element on >= 256 vocabulary columns at the full T / d / V of C3, C4 and C5 (oracle.grad_W_columns: every live token contributes to
+every column, so the oracle runs one fp64 forward over all live tokens; C3 keeps its own variable-length mask, C4 and C5 use a
+scattered subset of live tokens that still spans several token super-tiles so that the check finishes in about a minute)."""
 import numpy as np
 import pytest
 import torch
@@ -126,3 +129,59 @@ def test_producers_at_C3_shape_sampled_rows(handle):
     lo = np.where(si > 0, np.take_along_axis(cdf, np.maximum(si - 1, 0), 1), 0.0)
     assert np.all(u64 <= hi + 2e-5) and np.all(u64 >= lo - 2e-5)
     assert np.abs(f64(slp[sel]) - np.take_along_axis(logp, si, 1)).max() <= LOGP_ATOL
+
+
+def _columns_for(idx, live, V, rng, n_tok=16, n_rand=96):
+    """>= 256 vocabulary columns: every cached column of n_tok random live tokens (where the sparse beta terms land), random
+    columns, and the last, partial vocabulary tile (V = 151936 = 593 * 256 + 128)."""
+    toks = rng.choice(live, n_tok, replace=False)
+    cached = np.unique(f64(idx[torch.as_tensor(toks, device=idx.device)]).astype(np.int64).ravel())
+    cached = cached[(cached >= 0) & (cached < V)][:160]
+    tail = np.arange(V - V % 256 if V % 256 else V - 256, V)
+    return np.unique(np.concatenate([cached, rng.choice(V, n_rand, replace=False), tail, [0, 255, 256, 4095, 4096]]))
+
+
+def grad_W_column_check(handle, cfg, c, mode, n_live_target=None, layout="dv", flags=0):
+    inp = synth.make_inputs(cfg, c=c, device=DEV)
+    T, V = cfg["T"], cfg["V"]
+    if n_live_target is not None:        # scattered subset of the live tokens (the mode codes of OPD_MIXED are kept)
+        live0 = torch.nonzero(inp["mask"] != 0).flatten()
+        keep = live0[torch.randperm(live0.numel(), generator=torch.Generator().manual_seed(c))[:n_live_target].to(DEV)]
+        m = torch.zeros_like(inp["mask"])
+        m[keep] = inp["mask"][keep]
+        inp["mask"] = m
+    idx, lam, old, kk = pick(inp, cfg, mode)
+    W = inp["W"] if layout == "dv" else inp["W"].t().contiguous().t()
+    r = handle.loss_fwd_bwd(inp["hidden"], W, idx, lam, old, inp["mask"], mode, kk, flags=flags)
+    torch.cuda.synchronize()
+    st = handle.launch_stats()
+    mask = f64(inp["mask"])
+    live = np.flatnonzero(mask)
+    assert live.size > st["super_rows"], "the check must span more than one token super-tile"
+    cols = _columns_for(idx, live, V, np.random.default_rng(100 + c))
+    assert cols.size >= 256
+    ref = O.grad_W_columns(f64(inp["hidden"]), f64(inp["W"]), f64(idx), f64(lam), f64(old) if old is not None else None, mask,
+                           mode, kk, cols)
+    got = f64(r["grad_W"][:, torch.as_tensor(cols, device=DEV)])
+    # the bar is relative to the largest entry of the compared columns (they hold the cached columns, where grad_W peaks)
+    check_grad(got, ref, "bf16", f"grad_W[:, {cols.size} columns] at {cfg['name']}")
+    # per-column: no single column may hide behind the global maximum by more than 4x its own scale
+    col_scale = np.maximum(np.abs(ref).max(axis=0), 1e-3 * np.abs(ref).max())
+    assert (np.abs(got - ref).max(axis=0) <= 4 * GRAD_TOL["bf16"] * col_scale).all()
+    return r, inp
+
+
+def test_C3_grad_W_columns_full_mask(handle):
+    """C3 (T=16384, d=2048, V=151936, variable-length mask, ~9.2k live tokens): grad_W columns element by element, both modes."""
+    grad_W_column_check(handle, synth.CONFIGS[3], 3, O.RKL_MC)
+    grad_W_column_check(handle, synth.CONFIGS[3], 3, O.FKL_TOPK, layout="vd")
+
+
+def test_C4_grad_W_columns(handle):
+    """C4 (T=32768, d=4096, V=151936): 6144 scattered live tokens (two token super-tiles, all 38 vocabulary super-tiles)."""
+    grad_W_column_check(handle, synth.CONFIGS[4], 4, O.RKL_MC, n_live_target=6144)
+
+
+def test_C5_grad_W_columns_mixed(handle):
+    """C5 (T=65536, d=2560, V=151936, mixed FKL k=64 / MC K=8 rows): 8192 scattered live tokens."""
+    grad_W_column_check(handle, synth.CONFIGS[5], 5, O.MIXED, n_live_target=8192)

@@ -234,6 +234,84 @@ def test_mc_diagnostics_outputs(handle, opd):
     assert np.all(v[f64(m) != 2] == 0)
 
 
+def test_seq_diagnostics_outputs(handle, opd):
+    """opd_set_seq_diagnostics (Eq.(17)): per-sequence timestep averages of the m-sample and one-sample
+    estimators and the fixed-path variance, against the oracle; MIXED batch (only the RKL_MC rows take part), ragged
+    sequence boundaries, an empty sequence and one that holds no MC row."""
+    cfg = dict(RAGGED, K=6)
+    inp = synth.make_inputs(cfg, c=19, device=DEV)
+    T = cfg["T"]
+    m = inp["mask"].clone()
+    m[(torch.arange(T, device=DEV) % 2 == 0) & (m != 0)] = 2
+    m[100:140][m[100:140] == 2] = 1                       # a sequence without any MC row
+    inp["mask"] = m
+    idx, lam, old, kk = synth.mixed_cache(inp)
+    cu = torch.tensor([0, 37, 100, 140, 140, 512, T], dtype=torch.int32, device=DEV)
+    out = handle.set_seq_diagnostics(cu)
+    try:
+        handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, m, O.MIXED, kk)
+        torch.cuda.synchronize()
+    finally:
+        handle.set_seq_diagnostics(None)
+    ref = oracle_for(inp, idx, lam, old, O.MIXED, kk)
+    K = kk >> 16
+    mm, m1, vm = O.seq_diagnostics(ref["per_token_kl"], ref["first_draw"], ref["var1"], f64(m), cu.cpu().numpy(), K, mc_code=2)
+    for got, want in ((out["seq_mean_m"], mm), (out["seq_mean_1"], m1), (out["seq_var_m"], vm)):
+        g = f64(got)
+        assert np.abs(g - want).max() <= 2e-3 * max(1e-30, np.abs(want).max())
+        assert g[2] == 0 and g[3] == 0                    # no MC row / empty sequence
+    # plain RKL_MC: every live row takes part
+    idx, lam, old, kk = pick(inp, cfg, O.RKL_MC)
+    out = handle.set_seq_diagnostics(cu)
+    try:
+        handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, m, O.RKL_MC, kk)
+        torch.cuda.synchronize()
+    finally:
+        handle.set_seq_diagnostics(None)
+    ref = oracle_for(inp, idx, lam, old, O.RKL_MC, kk)
+    mm, m1, vm = O.seq_diagnostics(ref["per_token_kl"], ref["first_draw"], ref["var1"], f64(m), cu.cpu().numpy(), kk)
+    assert np.abs(f64(out["seq_mean_m"]) - mm).max() <= 2e-3 * np.abs(mm).max()
+    assert np.abs(f64(out["seq_mean_1"]) - m1).max() <= 2e-3 * np.abs(m1).max()
+    assert np.abs(f64(out["seq_var_m"]) - vm).max() <= 2e-3 * np.abs(vm).max()
+
+
+@pytest.mark.parametrize("case", ["C1", "C2", "ragged_vd", "ragged_sparse"])
+def test_grad_W_bf16_output(handle, opd, case):
+    """OPD_F_GRADW_BF16 (SURVEY 8(b), reading Q15): grad_W as a bf16 array, summed in fp32 and rounded once at the end;
+    with OPD_F_GRADW_ACCUM the rounded sum of the old contents and this call; the host entry copies half the bytes back."""
+    cfg = {"C1": synth.CONFIGS[1], "C2": synth.CONFIGS[2]}.get(case, RAGGED)
+    c = {"C1": 1, "C2": 2}.get(case, 21)
+    mode = O.RKL_TOPK if case == "ragged_sparse" else O.RKL_MC
+    inp = synth.make_inputs(cfg, c=c, device=DEV)
+    idx, lam, old, kk = pick(inp, cfg, mode)
+    W = inp["W"].t().contiguous().t() if case == "ragged_vd" else inp["W"]
+    ref = oracle_for(inp, idx, lam, old, mode, kk)
+    r = handle.loss_fwd_bwd(inp["hidden"], W, idx, lam, old, inp["mask"], mode, kk, flags=opd.F_GRADW_BF16)
+    torch.cuda.synchronize()
+    assert r["grad_W"].dtype == torch.bfloat16 and r["grad_W"].stride() == W.stride()
+    check_loss(r["loss"].item(), ref)
+    check_grad(f64(r["grad_W"]), ref["grad_W"], "bf16", "bf16 grad_W")
+    check_grad(f64(r["grad_hidden"]), ref["grad_hidden"], cfg["dtype"], "grad_hidden")
+    # the bf16 array is the rounding of the fp32 result of the default call (same sums, one rounding)
+    r32 = handle.loss_fwd_bwd(inp["hidden"], W, idx, lam, old, inp["mask"], mode, kk)
+    torch.cuda.synchronize()
+    assert (r["grad_W"].float() - r32["grad_W"]).abs().max().item() <= 2.0 ** -8 * r32["grad_W"].abs().max().item()
+    # accumulate: twice the gradient, rounded after the fp32 add
+    gw = r["grad_W"].clone()
+    handle.loss_fwd_bwd(inp["hidden"], W, idx, lam, old, inp["mask"], mode, kk, flags=opd.F_GRADW_BF16 | opd.F_GRADW_ACCUM, grad_W=gw)
+    torch.cuda.synchronize()
+    check_grad(f64(gw), 2.0 * ref["grad_W"], "bf16", "accumulated bf16 grad_W")
+    if case == "ragged_vd":
+        return
+    hr = handle.loss_fwd_bwd_host(inp["hidden"].cpu(), inp["W"].cpu(), idx.cpu(), lam.cpu(), None if old is None else old.cpu(),
+                                  inp["mask"].cpu(), mode, kk, flags=opd.F_GRADW_BF16)
+    assert hr["grad_W"].dtype == torch.bfloat16
+    check_grad(f64(hr["grad_W"]), ref["grad_W"], "bf16", "host bf16 grad_W")
+    h32 = handle.loss_fwd_bwd_host(inp["hidden"].cpu(), inp["W"].cpu(), idx.cpu(), lam.cpu(), None if old is None else old.cpu(),
+                                   inp["mask"].cpu(), mode, kk)
+    assert h32["d2h_bytes"] - hr["d2h_bytes"] == 2 * cfg["d"] * cfg["V"]
+
+
 def test_pipelined_host_entry(handle, opd):
     """opd_loss_fwd_bwd_host_submit / _wait: two steps in flight on the two staging slots give the results of the
     synchronous call; a busy slot refuses a second submit; waiting on an idle slot is an error."""
