@@ -62,7 +62,8 @@ enum {
     OPD_F_FWD_ONLY = 32,         /* loss / per-token outputs only; grad pointers may be NULL                     */
     /* reverse-KL surrogate of the 2x2 ablation, Eq.(6),(7) PAPER.md:132-141 (default: A_theta, no clip = Eq.(15)) */
     OPD_F_SUR_CLIP = 64,         /* PPO clip of rho to [1-eps, 1+eps], eps = 0.2                  */
-    OPD_F_SUR_A_OLD = 128        /* frozen rollout-time advantage A_old = log q - log p_old instead of A_theta   */
+    OPD_F_SUR_A_OLD = 128,       /* frozen rollout-time advantage A_old = log q - log p_old instead of A_theta   */
+    OPD_F_DENSE_REVERSE = 256    /* opd_dense_kl_fwd_bwd only: reverse direction KL(p || q), Eq.(2)  */
 };
 
 /* lifetime ------------------------------------------------------------------------------------- */
@@ -183,7 +184,11 @@ opd_status_t opd_cache_sample(opd_handle_t h, void* cuda_stream, int T, int d, i
  * Both heads are streamed tile by tile; neither set of logits is stored (bounded L2-resident rings of q and of the
  * gradient tiles only). teacher_hidden [T,dT] (row stride ld_th) and W_T (logical [dT,V], strides ldt_k / ldt_v, either
  * storage order) have the dtype of hidden / W; dT % 64 == 0. mask [T]: 0 = masked. flags: OPD_F_GRADW_ACCUM,
- * OPD_F_FWD_ONLY. With bf16 inputs q is rounded to bf16 before use (in the loss AND the gradient, consistently).
+ * OPD_F_FWD_ONLY, OPD_F_DENSE_REVERSE. With bf16 inputs q is rounded to bf16 before use (in the loss AND the gradient,
+ * consistently).
+ * OPD_F_DENSE_REVERSE: the student-weighted direction (Eq.(2); gradient Eq.(3)):
+ *     per_token_kl[t] = sum_v p_tv (log p_tv - log q_tv),   dL_t/dz_tv = p_tv (log p_tv - log q_tv - per_token_kl[t]);
+ * log q is kept in fp32 tiles and the per-token value is formed by one more streamed pass before the gradient tiles.
  * Other arguments and outputs as for opd_loss_fwd_bwd. */
 size_t opd_dense_kl_workspace_bytes(int T, int d, int dT, int V, opd_dtype_t dtype, unsigned flags);
 opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, int T, int d, int dT, int V, opd_dtype_t dtype,

@@ -443,10 +443,13 @@ def cache_sample(hidden, W, uniforms):
 # ------------------------------------------------------------------------------------------------
 # Dense two-head forward KL: the teacher's distribution recomputed from transmitted teacher
 # hidden states (the direction PAPER.md:240 names as future work), objective Eq.(1), gradient PAPER.md:59.
-def dense_kl_oracle(hidden, W, teacher_hidden, W_T, mask, norm_override: float = 0.0, chunk: int = 512):
+def dense_kl_oracle(hidden, W, teacher_hidden, W_T, mask, norm_override: float = 0.0, chunk: int = 512, reverse: bool = False):
     """q_t = softmax(h^T_t . W_T), p_t = softmax(x_t . W);  L_t = sum_v q_tv (log q_tv - log p_tv)  (Eq.(1));
     loss = (1/N) sum_t m_t L_t;  dL_t/dz_tv = (sum_v q_tv) p_tv - q_tv  (= p - q, PAPER.md:59);
     grad_hidden / grad_W by the chain rule (O8, O9).
+    reverse=True: the student-weighted direction, Eq.(2):  L_t = sum_v p_tv (log p_tv - log q_tv), whose exact
+    gradient in the student logits is  dL_t/dz_tv = p_tv (log p_tv - log q_tv - L_t)  (Eq.(3): the "+1" term
+    drops out because sum_v p_v d(log p_v) = 0).
     Returns dict(loss, N, per_token_kl[T], grad_hidden[T,d], grad_W[d,V])."""
     X = np.asarray(hidden, dtype=np.float64)
     Wd = np.asarray(W, dtype=np.float64)
@@ -467,8 +470,14 @@ def dense_kl_oracle(hidden, W, teacher_hidden, W_T, mask, norm_override: float =
         logp, _ = log_softmax_rows(X[tt] @ Wd)
         logq, _ = log_softmax_rows(XT[tt] @ WT)
         q = np.exp(logq)
-        per_token[tt] = np.sum(q * (logq - logp), axis=1)
-        G = (np.sum(q, axis=1, keepdims=True) * np.exp(logp) - q) * scale
+        if reverse:
+            pr = np.exp(logp)
+            Lt = np.sum(pr * (logp - logq), axis=1)
+            per_token[tt] = Lt
+            G = pr * (logp - logq - Lt[:, None]) * scale
+        else:
+            per_token[tt] = np.sum(q * (logq - logp), axis=1)
+            G = (np.sum(q, axis=1, keepdims=True) * np.exp(logp) - q) * scale
         gh[tt] = G @ Wd.T
         gW += X[tt].T @ G
     return dict(loss=float(np.sum(per_token)) * scale, N=N, per_token_kl=per_token, grad_hidden=gh, grad_W=gW)

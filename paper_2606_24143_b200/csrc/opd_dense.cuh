@@ -9,6 +9,12 @@
 // followed by the unchanged grad_hidden / grad_W tiles.  L_t = A_t - B_t uses the SAME rounded q^ in both sums, so the
 // bf16 rounding of q only perturbs the weights of the KL terms (relative 2^-9 per term), not the large entropy and
 // cross-entropy sums separately.  With fp32 inputs the Q ring is fp32 and q^ = q.
+//
+// Reverse direction (OPD_F_DENSE_REVERSE; Eq.(2)):  L_t = D_R = sum_v p_tv (log p_tv - log q_tv),
+//     dL_t/dz_tv = p_tv (log p_tv - log q_tv - L_t)       (the "+1" of Eq.(3) cancels against the softmax Jacobian)
+// The Q tiles then store log q = z^T - lse_T (always fp32: a bf16 log-prob of magnitude ~10 would carry an absolute error of
+// 0.03 into every term), a first launch of Q + G tiles accumulates L_t = sum_v p (log p - log q) without storing G, and the
+// backward launch re-forms Q, then G = (1/N) p (log p - log q - L_t), followed by the unchanged grad_hidden / grad_W tiles.
 #pragma once
 #include "opd_epilogues_bwd.cuh"
 
@@ -35,8 +41,9 @@ struct QEpi {
         void* qs;                // Q ring buffer of this tile: [rows][ldq] bf16 (or fp32)
         int rows; long ldq; int q_fp32;
         const float* lse2_t;     // [T] teacher lse * log2(e), compact rows
-        float* acc_a;            // [T] A_t
+        float* acc_a;            // [T] A_t (forward direction)
         int V;
+        int logq;                // reverse direction: store log q (fp32 ring) instead of q, no A_t
     };
     struct State { float lse2; };
     static __device__ __forceinline__ State prepare(const Params& p, const GemmParams& gp, int m_blk, int, int row_in_tile, int M_eff) {
@@ -58,6 +65,12 @@ struct QEpi {
 #pragma unroll
             for (int i = 0; i < 32; i += 2) {
                 float q0 = 0.f, q1 = 0.f;
+                if (p.logq) {                                     // log q_tv = z^T_tv - lse_T
+                    if (live && col0 + i < p.V) q0 = v[i] - st.lse2 * (1.f / LOG2E);
+                    if (live && col0 + i + 1 < p.V) q1 = v[i + 1] - st.lse2 * (1.f / LOG2E);
+                    v[i] = q0; v[i + 1] = q1;
+                    continue;
+                }
                 if (live && col0 + i < p.V) q0 = exp2f(fmaf(v[i], LOG2E, -st.lse2));
                 if (live && col0 + i + 1 < p.V) q1 = exp2f(fmaf(v[i + 1], LOG2E, -st.lse2));
                 if (!p.q_fp32) {                                  // the rounded value is the one every later use sees
@@ -80,7 +93,7 @@ struct QEpi {
                 for (int q = 0; q < 4; ++q) dst[q] = make_uint4(w[4 * q], w[4 * q + 1], w[4 * q + 2], w[4 * q + 3]);
             }
         }
-        if (live) atomicAdd(p.acc_a + gp.tok_off + lrow, a);
+        if (live && !p.logq) atomicAdd(p.acc_a + gp.tok_off + lrow, a);
     }
 };
 
@@ -93,14 +106,19 @@ struct GDenseEpi {
         long ldq; int q_fp32;
         const float* lse2_p;     // [T] student lse * log2(e)
         const float* coef;       // [T] 1/N (0 on dead rows)
-        float* acc_b;            // [T] B_t
+        float* acc_b;            // [T] B_t (forward) / L_t (reverse, first launch); null: not accumulated
         int V;
+        int reverse;             // the Q ring holds log q; G = coef * p * (log p - log q - L_t)
+        const float* lt;         // [T] L_t of the reverse direction (second launch), compact rows
     };
-    struct State { float lse2; float coef; };
+    struct State { float lse2; float coef; float lt; };
     static __device__ __forceinline__ State prepare(const Params& p, const GemmParams& gp, int m_blk, int, int row_in_tile, int M_eff) {
         const int lrow = m_blk * BM + row_in_tile;
-        State st{0.f, 0.f};
-        if (lrow < M_eff) { st.lse2 = p.lse2_p[gp.tok_off + lrow]; st.coef = p.coef[gp.tok_off + lrow]; }
+        State st{0.f, 0.f, 0.f};
+        if (lrow < M_eff) {
+            st.lse2 = p.lse2_p[gp.tok_off + lrow]; st.coef = p.coef[gp.tok_off + lrow];
+            if (p.reverse && p.lt) st.lt = p.lt[gp.tok_off + lrow];
+        }
         return st;
     }
     static __device__ __forceinline__ void run(const Params& p, const GemmParams& gp, State st, uint32_t taddr,
@@ -139,8 +157,15 @@ struct GDenseEpi {
 #pragma unroll
             for (int i = 0; i < 32; ++i) {
                 if (live && col0 + i < p.V) {
-                    b = fmaf(q[i], v[i] - st.lse2 * (1.f / LOG2E), b);
-                    v[i] = st.coef * (exp2f(fmaf(v[i], LOG2E, -st.lse2)) - q[i]);
+                    if (p.reverse) {
+                        const float pr = exp2f(fmaf(v[i], LOG2E, -st.lse2));
+                        const float tdiff = (v[i] - st.lse2 * (1.f / LOG2E)) - q[i];      // log p - log q
+                        b = fmaf(pr, tdiff, b);
+                        v[i] = st.coef * pr * (tdiff - st.lt);
+                    } else {
+                        b = fmaf(q[i], v[i] - st.lse2 * (1.f / LOG2E), b);
+                        v[i] = st.coef * (exp2f(fmaf(v[i], LOG2E, -st.lse2)) - q[i]);
+                    }
                 } else {
                     v[i] = 0.f;
                 }
@@ -162,20 +187,22 @@ struct GDenseEpi {
                 for (int qq = 0; qq < 4; ++qq) dst[qq] = make_uint4(w[4 * qq], w[4 * qq + 1], w[4 * qq + 2], w[4 * qq + 3]);
             }
         }
-        if (live) atomicAdd(p.acc_b + gp.tok_off + lrow, b);
+        if (live && p.acc_b) atomicAdd(p.acc_b + gp.tok_off + lrow, b);
     }
 };
 
-// L_t = A_t - B_t (caller order), block sums for the deterministic loss reduction (k_loss_final finishes it)
-__global__ void __launch_bounds__(128) k_dense_loss(const float* __restrict__ acc_a, const float* __restrict__ acc_b,
+// L_t = A_t - B_t (forward; reverse: L_t = B_t) in caller order, block sums for the deterministic loss reduction
+// (k_loss_final finishes it); lt (optional, compact rows) keeps L_t for the reverse direction's gradient tiles
+__global__ void __launch_bounds__(128) k_dense_loss(const float* __restrict__ acc_a, const float* __restrict__ acc_b, int reverse,
                                                     const int* __restrict__ live_rows, const int* __restrict__ n_live,
-                                                    float* __restrict__ per_token_kl, double* __restrict__ block_sums) {
+                                                    float* __restrict__ per_token_kl, float* __restrict__ lt, double* __restrict__ block_sums) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     float L = 0.f;
     if (i < *n_live) {
-        L = acc_a[i] - acc_b[i];
+        L = reverse ? acc_b[i] : acc_a[i] - acc_b[i];
         per_token_kl[live_rows[i]] = L;
     }
+    if (lt != nullptr && i < gridDim.x * blockDim.x) lt[i] = L;
     __shared__ double sh[128];
     sh[threadIdx.x] = static_cast<double>(L);
     __syncthreads();

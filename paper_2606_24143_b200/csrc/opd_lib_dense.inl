@@ -3,7 +3,7 @@
 
 struct DensePlan {
     Plan base;                 // the learner path's plan (student operands, G ring, partial sums, counters ...)
-    size_t off_txc, off_wtsplit, off_qring, off_lse_p, off_lse_t, off_lse2_t, off_acc_a, off_acc_b, off_qdone, total;
+    size_t off_txc, off_wtsplit, off_qring, off_lse_p, off_lse_t, off_lse2_t, off_acc_a, off_acc_b, off_lt, off_qdone, total;
     size_t txc_plane, wt_plane, q_buf_bytes;
 };
 
@@ -17,13 +17,15 @@ static DensePlan make_dense_plan(int T, int d, int dT, int V, int fp32, unsigned
     p.off_txc = take(2 * p.txc_plane * planes);
     p.wt_plane = (size_t)dT * V;
     p.off_wtsplit = take(fp32 ? 2 * p.wt_plane * 3 : 0);
-    p.q_buf_bytes = align_up((size_t)p.base.Tb * p.base.Vb * (fp32 ? 4 : 2), 1024);
+    const bool q32 = fp32 || (flags & OPD_F_DENSE_REVERSE);      // the reverse direction keeps log q, always in fp32
+    p.q_buf_bytes = align_up((size_t)p.base.Tb * p.base.Vb * (q32 ? 4 : 2), 1024);
     p.off_qring = take(2 * p.q_buf_bytes);
     p.off_lse_p = take(sizeof(float) * (size_t)p.base.t_pad);
     p.off_lse_t = take(sizeof(float) * (size_t)p.base.t_pad);
     p.off_lse2_t = take(sizeof(float) * (size_t)p.base.t_pad);
     p.off_acc_a = take(sizeof(float) * (size_t)p.base.t_pad);
     p.off_acc_b = take(sizeof(float) * (size_t)p.base.t_pad);
+    p.off_lt = take(sizeof(float) * (size_t)p.base.t_pad);
     p.off_qdone = take(sizeof(int) * (3 * (size_t)p.base.n_super + 1));      // q_done, g_done, c_done, tile ticket
     p.total = o;
     return p;
@@ -43,7 +45,9 @@ extern "C" opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, 
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     if (!h->arch_ok) OPD_FAIL(h, OPD_ERR_ARCH, "device %d is not compute capability 10.x (sm_100a required, no fallback)", h->device);
     if (dtype != OPD_BF16 && dtype != OPD_FP32) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unknown dtype %d", (int)dtype);
-    if (flags & ~(unsigned)(OPD_F_GRADW_ACCUM | OPD_F_FWD_ONLY)) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unsupported flag bits 0x%x", flags);
+    if (flags & ~(unsigned)(OPD_F_GRADW_ACCUM | OPD_F_FWD_ONLY | OPD_F_DENSE_REVERSE)) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unsupported flag bits 0x%x", flags);
+    const bool reverse = (flags & OPD_F_DENSE_REVERSE) != 0;
+    const bool q32 = dtype == OPD_FP32 || reverse;
     opd_status_t s = check_shape(h, T, d, V, 1);
     if (s != OPD_OK) return s;
     if (dT < 64 || dT > 16384 || dT % 64) OPD_FAIL(h, OPD_ERR_BAD_SHAPE, "teacher width dT=%d must be a multiple of 64 in [64,16384]", dT);
@@ -93,6 +97,7 @@ extern "C" opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, 
     float* lse2_t = reinterpret_cast<float*>(ws + dp.off_lse2_t);
     float* acc_a = reinterpret_cast<float*>(ws + dp.off_acc_a);
     float* acc_b = reinterpret_cast<float*>(ws + dp.off_acc_b);
+    float* lt = reinterpret_cast<float*>(ws + dp.off_lt);
     __nv_bfloat16* gs = reinterpret_cast<__nv_bfloat16*>(ws + p.off_gs);
     float* dxacc = reinterpret_cast<float*>(ws + p.off_dxacc);
     double* block_sums = reinterpret_cast<double*>(ws + p.off_block_sums);
@@ -170,10 +175,9 @@ extern "C" opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, 
     k_dense_rows<<<ceil_div(p.t_pad, 256), 256, 0, st>>>(lse_p, lse_t, n_live, norm_override, p.t_pad, lse2_p, lse2_t, coef, acc_a, acc_b);
     h->n_kernels += 3;
 
-    // ---- pass B: Q / G (/ grad_hidden / grad_W) tiles in one persistent launch
+    // ---- pass B: Q / G (/ grad_hidden / grad_W) tiles in one persistent launch (two launches for the reverse direction)
     int* q_done = reinterpret_cast<int*>(ws + dp.off_qdone);
     int* counters = q_done + p.n_super;
-    OPD_CUDA(h, cudaMemsetAsync(q_done, 0, sizeof(int) * (3 * (size_t)p.n_super + 1), st));
     BwdParams bp{};
     bp.d = d; bp.V = V; bp.Tb = p.Tb; bp.Vb = p.Vb; bp.nvb = ceil_div(V, p.Vb); bp.wl = wl; bp.planes = p.planes; bp.gbufs = p.gs_bufs;
     bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super; bp.q_done = q_done;
@@ -181,18 +185,37 @@ extern "C" opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, 
     bp.dw_store_first = (flags & OPD_F_GRADW_ACCUM) ? 0 : 1;
     bp.dx = dxp; bp.dw = dwp;
     bp.hint_x = bp.hint_w = bp.hint_g = L2_EVICT_NORMAL;
-    bp.dT = dT; bp.wl_t = wlt; bp.qbytes = fp32 ? 4 : 2; bp.q_buf_bytes = dp.q_buf_bytes;
-    bp.q = QEpi::Params{qring, p.Tb, (long)p.Vb, fp32 ? 1 : 0, lse2_t, acc_a, V};
-    bp.gd = GDenseEpi::Params{gs, p.Tb, (long)p.Vb, (long)p.gs_plane, p.planes, qring, (long)p.Vb, fp32 ? 1 : 0, lse2_p, coef, acc_b, V};
-    bp.type_mask = fwd_only ? ((1 << T_Q) | (1 << T_G)) : 15;
-    s = launch_bwd<true>(h, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp);
-    if (s != OPD_OK) return s;
-    h->n_kernels++; h->n_gemm++;
-
-    // ---- loss: L_t = A_t - B_t, token mean
-    k_dense_loss<<<p.est_blocks, 128, 0, st>>>(acc_a, acc_b, live_rows, n_live, per_token_kl, block_sums);
-    k_loss_final<<<1, 256, 0, st>>>(block_sums, p.est_blocks, n_live, norm_override, loss);
-    h->n_kernels += 2;
+    bp.dT = dT; bp.wl_t = wlt; bp.qbytes = q32 ? 4 : 2; bp.q_buf_bytes = dp.q_buf_bytes;
+    bp.q = QEpi::Params{qring, p.Tb, (long)p.Vb, q32 ? 1 : 0, lse2_t, acc_a, V, reverse ? 1 : 0};
+    bp.gd = GDenseEpi::Params{gs, p.Tb, (long)p.Vb, (long)p.gs_plane, p.planes, qring, (long)p.Vb, q32 ? 1 : 0, lse2_p, coef, acc_b, V,
+                              reverse ? 1 : 0, nullptr};
+    const int fwd_types = (1 << T_Q) | (1 << T_G);
+    auto launch = [&](int type_mask) -> opd_status_t {
+        OPD_CUDA(h, cudaMemsetAsync(q_done, 0, sizeof(int) * (3 * (size_t)p.n_super + 1), st));
+        bp.type_mask = type_mask;
+        opd_status_t ls = launch_bwd<true>(h, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp);
+        if (ls == OPD_OK) { h->n_kernels++; h->n_gemm++; }
+        return ls;
+    };
+    auto loss_kernels = [&]() {
+        k_dense_loss<<<p.est_blocks, 128, 0, st>>>(acc_a, acc_b, reverse ? 1 : 0, live_rows, n_live, per_token_kl, reverse ? lt : nullptr, block_sums);
+        k_loss_final<<<1, 256, 0, st>>>(block_sums, p.est_blocks, n_live, norm_override, loss);
+        h->n_kernels += 2;
+    };
+    if (!reverse) {
+        s = launch(fwd_only ? fwd_types : 15);
+        if (s != OPD_OK) return s;
+        loss_kernels();                                   // L_t = A_t - B_t, token mean
+    } else {
+        s = launch(fwd_types);                            // L_t = sum_v p (log p - log q): the gradient tiles need it
+        if (s != OPD_OK) return s;
+        loss_kernels();
+        if (!fwd_only) {
+            bp.gd.acc_b = nullptr; bp.gd.lt = lt;
+            s = launch(15);
+            if (s != OPD_OK) return s;
+        }
+    }
     OPD_CUDA(h, cudaGetLastError());
     return OPD_OK;
 }

@@ -31,10 +31,10 @@ def make(dtype, T, d, dT, V, seed, masked=True):
     return X, W, XT, WT, mask
 
 
-def compare(r, X, W, XT, WT, mask, dtype):
-    """Every output against Eq.(1) as written (the oracle knows nothing about how the kernel rounds q)."""
+def compare(r, X, W, XT, WT, mask, dtype, reverse=False):
+    """Every output against Eq.(1) / Eq.(2) as written (the oracle knows nothing about how the kernel rounds q)."""
     live = f64(mask) != 0
-    exact = O.dense_kl_oracle(f64(X), f64(W), f64(XT), f64(WT), f64(mask))
+    exact = O.dense_kl_oracle(f64(X), f64(W), f64(XT), f64(WT), f64(mask), reverse=reverse)
     ptk = f64(r["per_token_kl"])
     bar = LOSS_RTOL * np.abs(exact["per_token_kl"]).max()
     assert np.abs(ptk - exact["per_token_kl"]).max() <= bar and np.all(ptk[~live] == 0)
@@ -56,6 +56,33 @@ def test_dense_kl_parity(handle, dtype, T, d, dT, V, layouts):
     r = handle.dense_kl_fwd_bwd(X, Wl, XT, WTl, mask)
     torch.cuda.synchronize()
     compare(r, X, W, XT, WT, mask, dtype)
+
+
+@pytest.mark.parametrize("dtype,T,d,dT,V,layouts,tiles", [
+    ("fp32", 256, 256, 128, 4096, ("dv", "dv"), None), ("bf16", 700, 320, 448, 2056, ("dv", "vd"), None),
+    ("bf16", 700, 320, 448, 2056, ("vd", "dv"), (256, 512)), ("bf16", 1024, 512, 1024, 32768, ("dv", "dv"), None)])
+def test_dense_reverse_kl_parity(handle, dtype, T, d, dT, V, layouts, tiles, monkeypatch):
+    """OPD_F_DENSE_REVERSE: KL(p || q) of Eq.(2) and its gradient Eq.(3), fp32 and bf16, both storage orders of
+    both heads, several super-tiles (ring reuse across the two launches), forward-only, N = 0."""
+    from paper_2606_24143_b200 import opd
+    if tiles:
+        monkeypatch.setenv("OPD_TB", str(tiles[0])); monkeypatch.setenv("OPD_VB", str(tiles[1]))
+    X, W, XT, WT, mask = make(dtype, T, d, dT, V, 4)
+    Wl = W if layouts[0] == "dv" else W.t().contiguous().t()
+    WTl = WT if layouts[1] == "dv" else WT.t().contiguous().t()
+    r = handle.dense_kl_fwd_bwd(X, Wl, XT, WTl, mask, flags=opd.F_DENSE_REVERSE)
+    torch.cuda.synchronize()
+    compare(r, X, W, XT, WT, mask, dtype, reverse=True)
+    f = handle.dense_kl_fwd_bwd(X, Wl, XT, WTl, mask, flags=opd.F_DENSE_REVERSE | opd.F_FWD_ONLY)
+    torch.cuda.synchronize()
+    assert f["grad_W"] is None and abs(f["loss"].item() - r["loss"].item()) <= 1e-5 * abs(r["loss"].item())
+    none = handle.dense_kl_fwd_bwd(X, Wl, XT, WTl, torch.zeros_like(mask), flags=opd.F_DENSE_REVERSE)
+    torch.cuda.synchronize()
+    assert none["loss"].item() == 0 and not none["grad_W"].any() and not none["grad_hidden"].any()
+    z = handle.dense_kl_fwd_bwd(X, Wl, X, Wl, mask, flags=opd.F_DENSE_REVERSE) if d == dT else None
+    if z is not None:
+        torch.cuda.synchronize()
+        assert abs(z["loss"].item()) <= 1e-5 and z["grad_W"].abs().max().item() <= 1e-3 * r["grad_W"].abs().max().item()
 
 
 def test_dense_kl_super_tiles_fwd_only_and_zero_case(handle, monkeypatch):

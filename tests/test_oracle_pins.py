@@ -645,3 +645,41 @@ def test_dense_two_head_kl_pins():
         assert abs((f(Xp, t["W"]) - f(Xm, t["W"])) / (2 * h) - r["grad_hidden"][ti, ki]) < 2e-8
         Wp, Wm = t["W"].copy(), t["W"].copy(); Wp[ki, vi] += h; Wm[ki, vi] -= h
         assert abs((f(t["X"], Wp) - f(t["X"], Wm)) / (2 * h) - r["grad_W"][ki, vi]) < 2e-8
+
+
+def test_dense_two_head_reverse_kl_pins():
+    """dense_kl_oracle(reverse=True) (Eq.(2); gradient Eq.(3)): equals torch's kl_div with the
+    roles swapped (library) and its autograd gradients; equals the MC estimator with K = V and a uniform proposal (pin P3's
+    relation) and the sparse reverse KL on S = V, through opd_oracle; zero when the heads coincide; >= 0; central finite
+    differences; masked rows contribute nothing."""
+    t = tiny(62, T=5, d=6, V=13, mask=[1, 0, 1, 1, 1])
+    rng = np.random.default_rng(6)
+    XT = rng.normal(size=(5, 8)); WT = rng.normal(size=(8, 13)) / math.sqrt(8)
+    r = O.dense_kl_oracle(t["X"], t["W"], XT, WT, t["mask"], reverse=True)
+    X = torch.tensor(t["X"], requires_grad=True); W = torch.tensor(t["W"], requires_grad=True)
+    logp = torch.log_softmax(X @ W, dim=1)
+    logq = torch.log_softmax(torch.tensor(XT) @ torch.tensor(WT), dim=1)
+    m = torch.tensor(t["mask"] != 0)
+    per = torch.nn.functional.kl_div(logq, logp, reduction="none", log_target=True).sum(1)      # sum_v p (log p - log q)
+    loss = per[m].sum() / m.sum()
+    loss.backward()
+    assert abs(r["loss"] - loss.item()) < 1e-14 and np.abs(r["per_token_kl"][m.numpy()] - per[m].detach().numpy()).max() < 1e-14
+    assert np.abs(r["grad_hidden"] - X.grad.numpy()).max() < 1e-14 and np.abs(r["grad_W"] - W.grad.numpy()).max() < 1e-14
+    assert np.all(r["grad_hidden"][1] == 0) and r["per_token_kl"][1] == 0 and np.all(r["per_token_kl"] >= 0)
+    full = np.tile(np.arange(13), (5, 1))
+    lq = logq.numpy()
+    mc = O.opd_oracle(t["X"], t["W"], full, lq, np.full((5, 13), -math.log(13)), t["mask"], O.RKL_MC, 13)
+    assert abs(mc["loss"] - r["loss"]) < 1e-13 and np.abs(mc["grad_W"] - r["grad_W"]).max() < 1e-13
+    sp = O.opd_oracle(t["X"], t["W"], full, lq, None, t["mask"], O.RKL_TOPK, 13)
+    assert abs(sp["loss"] - r["loss"]) < 1e-13 and np.abs(sp["grad_hidden"] - r["grad_hidden"]).max() < 1e-13
+    z = O.dense_kl_oracle(t["X"], t["W"], t["X"], t["W"], t["mask"], reverse=True)
+    assert abs(z["loss"]) < 1e-15 and np.abs(z["grad_W"]).max() < 1e-15
+    f = lambda Xa, Wa: O.dense_kl_oracle(Xa, Wa, XT, WT, t["mask"], reverse=True)["loss"]
+    h = 1e-6
+    for ti, ki, vi in [(0, 1, 2), (3, 5, 12), (4, 0, 7)]:
+        Xp, Xm = t["X"].copy(), t["X"].copy(); Xp[ti, ki] += h; Xm[ti, ki] -= h
+        assert abs((f(Xp, t["W"]) - f(Xm, t["W"])) / (2 * h) - r["grad_hidden"][ti, ki]) < 2e-8
+        Wp, Wm = t["W"].copy(), t["W"].copy(); Wp[ki, vi] += h; Wm[ki, vi] -= h
+        assert abs((f(t["X"], Wp) - f(t["X"], Wm)) / (2 * h) - r["grad_W"][ki, vi]) < 2e-8
+    # the two directions differ (a swapped-roles mistake would show)
+    assert abs(O.dense_kl_oracle(t["X"], t["W"], XT, WT, t["mask"])["loss"] - r["loss"]) > 1e-3
