@@ -50,7 +50,7 @@ def peaks():
 
 
 def workload(cfg_id: int, args):
-    from paper_2606_24143_b200 import synth
+    from gen import synth
     cfg = dict(synth.CONFIGS[cfg_id])
     if args.tokens:
         cfg["T"] = args.tokens
@@ -60,7 +60,8 @@ def workload(cfg_id: int, args):
 
 
 def pick_cache(inp, cfg, mode_name):
-    from paper_2606_24143_b200 import opd, synth
+    from gen import synth
+    from paper_2606_24143_b200 import opd
     if mode_name == "fkl":
         return opd.FKL_TOPK, inp["topk_idx"], inp["topk_logq"], None, cfg["k"]
     if mode_name == "rtopk":
@@ -160,7 +161,7 @@ def run_reference(args, rank, world):
     cfg = workload(args.config, args)
     gen = dict(cfg)
     gen["T"] = min(cfg["T"], 2048)                 # the oracle only sees a bounded sample of the workload's rows
-    from paper_2606_24143_b200 import synth
+    from gen import synth
     inp = synth.make_inputs(gen, c=args.config, device=dev, sigma=args.sigma)
     mode, idx, lam, old, kk = pick_cache(inp, gen, args.mode)
     prep = oracle_prepare(inp, idx, lam, old, 2048)
@@ -285,7 +286,8 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
 
-    from paper_2606_24143_b200 import opd, synth
+    from gen import synth
+    from paper_2606_24143_b200 import opd
     cfg = workload(args.config, args)
     inp = synth.make_inputs(cfg, c=args.config + 10 * rank, device=dev, sigma=args.sigma)
     mode, idx, lam, old, kk = pick_cache(inp, cfg, args.mode)

@@ -1,6 +1,7 @@
 """Build libopd.so (csrc/opd_lib.cu) for sm_100a with nvcc, in-tree.
 
     python -m paper_2606_24143_b200.build [--force] [--verbose]
+    python -m paper_2606_24143_b200.build --sass-histogram      # tcgen05 / TMEM / TMA opcodes per kernel of the built library
 """
 from __future__ import annotations
 
@@ -54,5 +55,36 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def sass_histogram() -> str:
+    """Per kernel of the built libopd.so: how many tensor-core (UTC*MMA = tcgen05.mma), TMEM (LDTM / STTM = tcgen05.ld / st),
+    TMA (UTMALDG / UTMASTG / UTMAREDG = cp.async.bulk.tensor loads, stores, reductions) and tcgen05 barrier / allocation
+    (UTCBAR, UTCATOMSWS) instructions its SASS holds; HMMA (mma.sync) would show a legacy tensor-core path."""
+    import collections
+    import re
+    sass = subprocess.run(["cuobjdump", "-sass", build()], capture_output=True, text=True, check=True).stdout
+    pat = re.compile(r"\b(UTC\w*MMA[.\w]*|UTMA\w+[.\w]*|LDTM[.\w]*|STTM[.\w]*|UTCBAR[.\w]*|UTCCP[.\w]*|UTCATOM\w*[.\w]*|HMMA[.\w]*|UBLKCP[.\w]*)")
+    per_fn, fn = collections.OrderedDict(), None
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            fn = m.group(1)
+            per_fn.setdefault(fn, collections.Counter())
+        elif fn is not None:
+            m = pat.search(line)
+            if m:
+                per_fn[fn][m.group(1)] += 1
+    out = []
+    for fn, cnt in per_fn.items():
+        if not cnt:
+            continue
+        name = subprocess.run(["c++filt", fn], capture_output=True, text=True).stdout.strip() or fn
+        out.append(re.sub(r"\(CUtensorMap_st.*", "(...)", name))
+        out += [f"    {v:6d}  {k}" for k, v in sorted(cnt.items())]
+    return "\n".join(out) + "\n"
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--sass-histogram" in sys.argv:
+        sys.stdout.write(sass_histogram())
+    else:
+        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

@@ -31,6 +31,7 @@ struct BwdParams {
     int* g_done;               // [S]
     int* c_done;               // [S]
     int* ticket;               // [1] next unclaimed item of the tile list (zeroed by the host before the launch)
+    int order;                 // BwdSched::order
     int dw_store_first;        // 1: the grad_W tiles of the first token super-tile store instead of reduce-add (grad_W is
                                //    overwritten, not accumulated into: no memset and no read-modify-write for that pass)
     int type_mask;             // bit t set = run tiles of type t.  All types of the variant = the normal run; a tile waits
@@ -59,13 +60,15 @@ struct BwdTile {
 template <int CG, bool DENSE>
 struct BwdSched {
     static constexpr int GOFF = DENSE ? 1 : 0;
-    static constexpr int TM = Cfg<CG>::TILE_M;
+    static constexpr int TM = BM * CG;
     int S, nvb, Tb, Vb, V, d, wl, n_live;
+    int order;      // tile order knobs (result-neutral): bit 0 grad_W tiles before grad_hidden tiles inside a block,
+                    // bits 1-3: n-fastest raster of the G / grad_hidden / grad_W tiles (default m fastest)
     int blk;        // current block
     long base;      // items before the current block
     __device__ __forceinline__ void init(const BwdParams& p) {
         n_live = *p.n_live;
-        nvb = p.nvb; Tb = p.Tb; Vb = p.Vb; V = p.V; d = p.d; wl = p.wl;
+        nvb = p.nvb; Tb = p.Tb; Vb = p.Vb; V = p.V; d = p.d; wl = p.wl; order = p.order;
         S = ((n_live + Tb - 1) / Tb) * nvb;
         blk = 0; base = 0;
     }
@@ -110,8 +113,13 @@ struct BwdSched {
         }
         if (t.type < 0) {
             t.s = g - 1;
-            const int ndx = nDX(t.s);
-            if (r < ndx) t.type = T_DX; else { t.type = T_DW; r -= ndx; }
+            if (order & 1) {
+                const int ndw = nDW(t.s);
+                if (r < ndw) t.type = T_DW; else { t.type = T_DX; r -= ndw; }
+            } else {
+                const int ndx = nDX(t.s);
+                if (r < ndx) t.type = T_DX; else { t.type = T_DW; r -= ndx; }
+            }
         }
         int mt, nt;
         dims(t.s, mt, nt, t.Tb_eff, t.Vb_eff);
@@ -120,7 +128,16 @@ struct BwdSched {
         t.tb0 = ti * Tb; t.vb0 = t.vi * Vb;
         if (t.type == T_DW) rows = wl == 0 ? (d + TM - 1) / TM : (t.Vb_eff + TM - 1) / TM;
         else rows = mt;
-        t.m_blk = r % rows; t.n_blk = r / rows;     // m fastest: concurrently running CTAs share the B panel
+        const int tbit = t.type == T_DX ? 4 : (t.type == T_DW ? 8 : 2);
+        if (order & tbit) {                          // n fastest: concurrently running CTAs share the A panel
+            int cols;
+            if (t.type == T_DX) cols = (d + BN - 1) / BN;
+            else if (t.type == T_DW) cols = wl == 0 ? nt : (d + BN - 1) / BN;
+            else cols = nt;
+            t.n_blk = r % cols; t.m_blk = r / cols;
+        } else {
+            t.m_blk = r % rows; t.n_blk = r / rows;  // m fastest: concurrently running CTAs share the B panel
+        }
         return true;
     }
 };
@@ -145,7 +162,8 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
            const __grid_constant__ CUtensorMap m_xc_mn, const __grid_constant__ CUtensorMap m_gs_mn,
            const __grid_constant__ CUtensorMap m_tx_k, const __grid_constant__ CUtensorMap m_wt_fwd,
            const __grid_constant__ BwdParams bp) {
-    using C = Cfg<CG>;
+    constexpr int ST = bwd_stages<CG>();
+    using C = Cfg<CG, ST>;
     extern __shared__ uint8_t smem_raw[];
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -156,7 +174,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
         prefetch_tmap(&m_w_dx); prefetch_tmap(&m_xc_mn); prefetch_tmap(&m_gs_mn);
         if constexpr (DENSE) { prefetch_tmap(&m_tx_k); prefetch_tmap(&m_wt_fwd); }
     }
-    Pipe<CG> P;
+    Pipe<CG, ST> P;
     P.setup(smem_raw, warp, lane);
     const int rank = static_cast<int>(P.rank);
     const int mask = bp.type_mask;
@@ -174,8 +192,8 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             BwdTile t;
             int it = 0;
             for (int n = 0;; ++n) {
-                // the leader's producer claims the pair's next item; the peer's producer reads it from the queue
-                const uint32_t item = rank == 0 ? ticket_claim<CG>(P, bp.ticket, n) : ticket_read<CG>(P, n);
+                // CG = 1: the producer claims the next item itself; CG = 2: both producers read what the peer's warp 1 claimed
+                const uint32_t item = CG == 1 ? ticket_claim<CG, ST>(P, bp.ticket, n) : ticket_read<CG, ST>(P, n);
                 if (!sc.get(item, t)) break;
                 if (!on(t.type)) continue;
                 TileOp op;
@@ -212,24 +230,31 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                     wait_counter(bp.g_done + t.s, CG * sc.nG(t.s));
                     fence_proxy_async_all();
                 }
-                produce_tile<CG>(P, op, it);
+                produce_tile<CG, ST>(P, op, it);
             }
         }
     } else if (warp == 1) {
+        // =========================== tile claimer (peer CTA of a pair; this warp has no other work there) =========
+        if (CG == 2 && rank == 1 && elect_one()) {
+            BwdSched<CG, DENSE> sc; sc.init(bp);
+            BwdTile t;
+            for (int n = 0;; ++n)
+                if (!sc.get(ticket_claim<CG, ST>(P, bp.ticket, n), t)) break;
+        }
         // =========================== MMA issuer ===========================
         if (rank == 0 && elect_one()) {
             BwdSched<CG, DENSE> sc; sc.init(bp);
             BwdTile t;
             int it = 0, lt = 0;
             for (int n = 0;; ++n) {
-                if (!sc.get(ticket_read<CG>(P, n), t)) break;
+                if (!sc.get(ticket_read<CG, ST>(P, n), t)) break;
                 if (!on(t.type)) continue;
                 int a_mn, b_mn, K;
                 if (t.type == T_G) { a_mn = 0; b_mn = (bp.wl == 0); K = bp.d; }
                 else if (DENSE && t.type == T_Q) { a_mn = 0; b_mn = (bp.wl_t == 0); K = bp.dT; }
                 else if (t.type == T_DX) { a_mn = 0; b_mn = (bp.wl == 1); K = t.Vb_eff; }
                 else { a_mn = 1; b_mn = 1; K = t.Tb_eff; }
-                mma_tile<CG>(P, a_mn, b_mn, ((K + BK - 1) / BK) * nseg, lt, it);
+                mma_tile<CG, ST>(P, a_mn, b_mn, ((K + BK - 1) / BK) * nseg, lt, it);
                 ++lt;
             }
         }
@@ -247,7 +272,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
         };
         for (int n = 0;; ++n) {
             uint32_t item = 0;
-            if (lane == 0) item = ticket_read<CG>(P, n);
+            if (lane == 0) item = ticket_read<CG, ST>(P, n);
             item = __shfl_sync(0xffffffffu, item, 0);
             if (!sc.get(item, t)) break;
             if (!on(t.type)) continue;
@@ -267,7 +292,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 QEpi::Params ep = bp.q;
                 ep.qs = static_cast<uint8_t*>(ep.qs) + static_cast<size_t>(t.s & 1) * bp.q_buf_bytes;
                 QEpi::State st = QEpi::prepare(ep, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
-                const uint32_t taddr = epi_acquire<CG>(P, lt, quarter);
+                const uint32_t taddr = epi_acquire<CG, ST>(P, lt, quarter);
                 QEpi::run(ep, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, nullptr, epi_tid);
             } else if (DENSE && t.type == T_G) {
                 gp.b_off = t.vb0; gp.N = t.Vb_eff;
@@ -276,29 +301,29 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 ep.qs = static_cast<const uint8_t*>(ep.qs) + static_cast<size_t>(t.s & 1) * bp.q_buf_bytes;
                 if (!on(T_DX)) ep.rows = 0;                     // forward-only: nothing consumes G
                 GDenseEpi::State st = GDenseEpi::prepare(ep, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
-                const uint32_t taddr = epi_acquire<CG>(P, lt, quarter);
+                const uint32_t taddr = epi_acquire<CG, ST>(P, lt, quarter);
                 GDenseEpi::run(ep, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, nullptr, epi_tid);
             } else if (t.type == T_G) {
                 gp.b_off = t.vb0; gp.N = t.Vb_eff;
                 GEpi::Params ep = bp.g;
                 ep.gs += static_cast<size_t>(t.s % bp.gbufs) * bp.planes * ep.plane_stride;
                 GEpi::State st = GEpi::prepare(ep, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
-                const uint32_t taddr = epi_acquire<CG>(P, lt, quarter);
+                const uint32_t taddr = epi_acquire<CG, ST>(P, lt, quarter);
                 GEpi::run(ep, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, nullptr, epi_tid);
             } else if (t.type == T_DX) {
                 gp.N = bp.d; gp.first = (t.vi == 0); gp.last = (t.vi == bp.nvb - 1);
                 DxEpi::State st = DxEpi::prepare(bp.dx, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
-                const uint32_t taddr = epi_acquire<CG>(P, lt, quarter);
+                const uint32_t taddr = epi_acquire<CG, ST>(P, lt, quarter);
                 DxEpi::run(bp.dx, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, P.epi_smem, epi_tid);
             } else {
                 int M_eff;
                 if (bp.wl == 0) { gp.N = t.Vb_eff; gp.row_off = 0; gp.col_off = t.vb0; M_eff = bp.d; }
                 else { gp.N = bp.d; gp.row_off = t.vb0; gp.col_off = 0; M_eff = t.Vb_eff; }
                 gp.first = bp.dw_store_first && t.tb0 == 0;          // first token super-tile: plain stores
-                const uint32_t taddr = epi_acquire<CG>(P, lt, quarter);
+                const uint32_t taddr = epi_acquire<CG, ST>(P, lt, quarter);
                 DwEpi::run(bp.dw, gp, NoState{}, taddr, m_blk, t.n_blk, row_in_tile, M_eff, P.epi_smem, epi_tid);
             }
-            epi_release<CG>(P, lt, lane);                       // TMEM stage free for the MMA warp
+            epi_release<CG, ST>(P, lt, lane);                       // TMEM stage free for the MMA warp
             ++lt;
             // publish: all 128 epilogue threads' global stores, then one release increment
             __threadfence();

@@ -204,64 +204,4 @@ __global__ void k_unsort_gather(const float* __restrict__ zc, const unsigned cha
     }
 }
 
-// ------------------------------------------------------------------------------------------ sparse backward
-// S7/S8 when alpha_t == 0 for every row (OPD_RKL_TOPK; OPD_FKL_TOPK with OPD_F_RENORM_STUDENT): the full-vocabulary
-// lse cancels, dL/dz has support on the cached columns only, and the dense re-formation of softmax tiles is skipped:
-//   grad_hidden[t,:]  = sum_j beta_tj W(:, a_tj)            grad_W(:, a_tj) += beta_tj x_t   (fp32 atomics: columns
-// of different tokens collide; the summation order of grad_W is then not reproducible run to run).
-// Works on [V,d] storage (contiguous d-vectors per cached column): the caller's arrays when W is stored [V,d], else
-// transposed scratch copies (k_transpose).  One block per compact row.
-template <typename T>
-__device__ __forceinline__ float ld_as_float(const void* base, size_t i) {
-    if constexpr (sizeof(T) == 2) return __bfloat162float(static_cast<const __nv_bfloat16*>(base)[i]);
-    else return static_cast<const float*>(base)[i];
-}
-template <typename T>
-__global__ void __launch_bounds__(256) k_sparse_bwd(const void* __restrict__ hidden, long ld_hidden, const void* __restrict__ Wt, long ldwt,
-                                                    int d, int C, const int* __restrict__ sorted_idx,
-                                                    const float* __restrict__ beta, const int* __restrict__ live_rows,
-                                                    const int* __restrict__ n_live, void* __restrict__ grad_hidden, long ld_gh,
-                                                    float* __restrict__ gWt, long ldgwt) {
-    const int i = blockIdx.x;
-    if (i >= *n_live) return;
-    const int tok = live_rows[i];
-    const int* idx = sorted_idx + static_cast<size_t>(i) * C;
-    const float* b = beta + static_cast<size_t>(i) * C;
-    for (int k = threadIdx.x; k < d; k += blockDim.x) {
-        const float x = ld_as_float<T>(hidden, static_cast<size_t>(tok) * ld_hidden + k);
-        float g = 0.f;
-        for (int s = 0; s < C; ++s) {
-            const int col = idx[s];
-            if (col >= IDX_SENTINEL - 1) break;             // unused slots (and invalid indices) sort to the end
-            const float bs = b[s];
-            g = fmaf(bs, ld_as_float<T>(Wt, static_cast<size_t>(col) * ldwt + k), g);
-            atomicAdd(gWt + static_cast<size_t>(col) * ldgwt + k, bs * x);
-        }
-        if constexpr (sizeof(T) == 2) static_cast<__nv_bfloat16*>(grad_hidden)[static_cast<size_t>(tok) * ld_gh + k] = __float2bfloat16_rn(g);
-        else static_cast<float*>(grad_hidden)[static_cast<size_t>(tok) * ld_gh + k] = g;
-    }
-}
-
-// dst[c][r] (=|+=) src[r][c] for an R x Cn matrix (row strides lds / ldd), 32 x 32 tiles through shared memory.
-// Launch: grid (ceil(Cn/32), ceil(R/32)), block (32, 8).
-template <typename T>
-__global__ void __launch_bounds__(256) k_transpose(const T* __restrict__ src, long lds, int R, int Cn, T* __restrict__ dst, long ldd,
-                                                   int accumulate) {
-    __shared__ T tile[32][33];
-    const int c0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
-    for (int y = threadIdx.y; y < 32; y += 8) {
-        const int r = r0 + y, c = c0 + threadIdx.x;
-        if (r < R && c < Cn) tile[y][threadIdx.x] = src[static_cast<size_t>(r) * lds + c];
-    }
-    __syncthreads();
-    for (int y = threadIdx.y; y < 32; y += 8) {
-        const int c = c0 + y, r = r0 + threadIdx.x;
-        if (r < R && c < Cn) {
-            T* o = dst + static_cast<size_t>(c) * ldd + r;
-            if constexpr (sizeof(T) == 4) { if (accumulate) *o += tile[threadIdx.x][y]; else *o = tile[threadIdx.x][y]; }
-            else *o = tile[threadIdx.x][y];
-        }
-    }
-}
-
 }  // namespace opd

@@ -26,19 +26,30 @@ constexpr int GEMM_THREADS = 192;                     // warp0 TMA, warp1 MMA(+T
 constexpr int EPI_SMEM_BYTES = 32768;                 // 4 epilogue warps x 2 staging buffers x (32 rows x 128 B)
 constexpr int TMEM_COLS = 512;                        // 2 accumulator stages x 256 columns
 constexpr int MAX_STAGES = 6;
-#ifndef OPD_PAIR_STAGES
-#define OPD_PAIR_STAGES 4                  // TMA ring depth of the CTA-pair configuration (32 KiB per stage): 4 stages keep the
-#endif                                     // tensor pipe as busy as 6 and re-fetch far less of W from HBM (profiles/r02_*)
+// TMA ring depth of the CTA-pair configuration (32 KiB per stage), per kernel (profiles/r02_ring_depth.md):
+//   one-GEMM kernels (forward logits, producers): 4 stages keep the tensor pipe 98% busy and read W from HBM about once per
+//     token panel (10.6 GB per C4 launch; 6 stages let the pairs sharing a panel drift apart and re-fetch 46 GB);
+//   persistent backward: its operands miss L2 more often (G ring, partial sums, two W panels), 6 stages hide that latency
+//     better (tensor pipe 87% against 78% busy).
+#ifndef OPD_FWD_STAGES
+#define OPD_FWD_STAGES 4
+#endif
+#ifndef OPD_BWD_STAGES
+#define OPD_BWD_STAGES 6
+#endif
 constexpr int SCHED_Q = 4;                 // depth of the tile-ticket queue of the dynamically scheduled kernels
 
-template <int CG>
+template <int CG> __host__ __device__ constexpr int fwd_stages() { return CG == 1 ? 4 : OPD_FWD_STAGES; }
+template <int CG> __host__ __device__ constexpr int bwd_stages() { return CG == 1 ? 4 : OPD_BWD_STAGES; }
+
+template <int CG, int ST>
 struct Cfg {
     static constexpr int TILE_M = BM * CG;                // rows of one tile (of the CTA or of the pair)
     static constexpr int B_ROWS = BN / CG;                // B rows (n) each CTA loads
     static constexpr int A_STAGE_BYTES = BM * BK * 2;     // 16 KiB
     static constexpr int B_STAGE_BYTES = B_ROWS * BK * 2; // 32 / 16 KiB
     static constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
-    static constexpr int STAGES = CG == 1 ? 4 : OPD_PAIR_STAGES;
+    static constexpr int STAGES = ST;
     static constexpr int RING_BYTES = STAGES * STAGE_BYTES;
     static constexpr int SMEM_BYTES = RING_BYTES + 1024 /*barriers*/ + EPI_SMEM_BYTES + 1024 /*align slack*/;
 };
@@ -80,9 +91,9 @@ __device__ __forceinline__ void tile_coords(int tile, int num_m, int num_n, int 
 //   empty[s]   the MMAs that read stage s have completed (commit, multicast to both CTAs for CG = 2)
 //   tfull[a]   accumulator stage a is complete (commit, multicast)
 //   tempty[a]  (leader's copy) all 4*CG epilogue warps have drained accumulator stage a
-template <int CG>
+template <int CG, int ST>
 struct Pipe {
-    using C = Cfg<CG>;
+    using C = Cfg<CG, ST>;
     uint8_t* smem;
     uint64_t *full_bar, *empty_bar, *tfull_bar, *tempty_bar;
     uint64_t *sfull_bar, *sempty_bar;     // tile-ticket queue (bwd_kernel): ticket q published / consumed by every reader
@@ -107,9 +118,10 @@ struct Pipe {
         if (warp == 0 && lane == 0) {
             for (int s = 0; s < C::STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
             for (int s = 0; s < 2; ++s) { mbar_init(&tfull_bar[s], 1); mbar_init(&tempty_bar[s], 4 * CG); }
-            // readers of a ticket: the MMA issuer and the 4 epilogue warps of the leader, the producer and the 4 epilogue
-            // warps of the peer CTA (the leader's producer is the claimer)
-            for (int s = 0; s < SCHED_Q; ++s) { mbar_init(&sfull_bar[s], 1); mbar_init(&sempty_bar[s], CG == 1 ? 5 : 10); }
+            // readers of a ticket.  CG = 1: the MMA issuer and the 4 epilogue warps (the producer claims).  CG = 2: both
+            // producers, the MMA issuer and the 8 epilogue warps of the pair (the peer CTA's otherwise idle warp 1 claims,
+            // so that the round trip of the claim never sits between two tiles of the producer)
+            for (int s = 0; s < SCHED_Q; ++s) { mbar_init(&sfull_bar[s], 1); mbar_init(&sempty_bar[s], CG == 1 ? 5 : 11); }
             fence_mbar_init();
         }
         if (warp == 1) {
@@ -133,26 +145,28 @@ struct Pipe {
 // item of the tile list from a global counter and publishes it to every warp role of the CTA (pair) through a small queue
 // in shared memory.  Items are claimed in list order, so everything an item depends on has been claimed by a CTA that is
 // already running: the kernel makes progress with any number of resident CTAs (no co-residency requirement).
-template <int CG>
-__device__ __forceinline__ uint32_t ticket_claim(const Pipe<CG>& P, int* counter, int n) {
+// The claimer runs in CTA rank CG - 1 (its copy of the `sempty` barriers is the live one); it runs up to SCHED_Q tickets
+// ahead of the slowest reader.
+template <int CG, int ST>
+__device__ __forceinline__ uint32_t ticket_claim(const Pipe<CG, ST>& P, int* counter, int n) {
     const int q = n % SCHED_Q;
     mbar_wait_cluster(&P.sempty_bar[q], ((n / SCHED_Q) & 1) ^ 1);
     const uint32_t t = static_cast<uint32_t>(atomicAdd(counter, 1));
     P.sticket[q] = t;
     if constexpr (CG == 2) {
-        st_shared_cluster_u32(mapa_rank(smem_u32(&P.sticket[q]), 1), t);
-        mbar_arrive_cluster(mapa_rank(smem_u32(&P.sfull_bar[q]), 1));
+        st_shared_cluster_u32(mapa_rank(smem_u32(&P.sticket[q]), 0), t);
+        mbar_arrive_cluster(mapa_rank(smem_u32(&P.sfull_bar[q]), 0));
     }
     mbar_arrive(&P.sfull_bar[q]);
     return t;
 }
 // called by one lane of a reader; every reader consumes every ticket exactly once, in order
-template <int CG>
-__device__ __forceinline__ uint32_t ticket_read(const Pipe<CG>& P, int n) {
+template <int CG, int ST>
+__device__ __forceinline__ uint32_t ticket_read(const Pipe<CG, ST>& P, int n) {
     const int q = n % SCHED_Q;
     mbar_wait_cluster(&P.sfull_bar[q], (n / SCHED_Q) & 1);
     const uint32_t t = *reinterpret_cast<volatile uint32_t*>(&P.sticket[q]);
-    mbar_arrive_cluster(mapa_rank(smem_u32(&P.sempty_bar[q]), 0));
+    mbar_arrive_cluster(mapa_rank(smem_u32(&P.sempty_bar[q]), CG - 1));
     return t;
 }
 
@@ -170,9 +184,9 @@ struct TileOp {
 };
 
 // TMA producer (one elected lane): stream all k-blocks of all segments of `t` through the ring.
-template <int CG>
-__device__ __forceinline__ void produce_tile(const Pipe<CG>& P, const TileOp& t, int& it) {
-    using C = Cfg<CG>;
+template <int CG, int ST>
+__device__ __forceinline__ void produce_tile(const Pipe<CG, ST>& P, const TileOp& t, int& it) {
+    using C = Cfg<CG, ST>;
     const int kblocks = (t.K + BK - 1) / BK;
     for (int seg = 0; seg < t.nseg; ++seg) {
         for (int kb_i = 0; kb_i < kblocks; ++kb_i, ++it) {
@@ -217,9 +231,9 @@ __device__ __forceinline__ void produce_tile(const Pipe<CG>& P, const TileOp& t,
 }
 
 // MMA issuer (one elected lane of the CTA / of the pair leader): all MMAs of one tile into accumulator stage lt & 1.
-template <int CG>
-__device__ __forceinline__ void mma_tile(const Pipe<CG>& P, int a_mn, int b_mn, int kiters, int lt, int& it) {
-    using C = Cfg<CG>;
+template <int CG, int ST>
+__device__ __forceinline__ void mma_tile(const Pipe<CG, ST>& P, int a_mn, int b_mn, int kiters, int lt, int& it) {
+    using C = Cfg<CG, ST>;
     const uint32_t idesc = make_idesc_bf16(C::TILE_M, BN, a_mn, b_mn);
     const uint32_t a_kstep = a_mn ? (UMMA_K * MN_BOX * 2) : (UMMA_K * 2);   // bytes per UMMA_K step
     const uint32_t b_kstep = b_mn ? (UMMA_K * MN_BOX * 2) : (UMMA_K * 2);
@@ -249,15 +263,15 @@ __device__ __forceinline__ void mma_tile(const Pipe<CG>& P, int a_mn, int b_mn, 
 }
 
 // Epilogue side: wait for accumulator stage lt & 1; returns this warp's TMEM address (lane quarter in bits 16+).
-template <int CG>
-__device__ __forceinline__ uint32_t epi_acquire(const Pipe<CG>& P, int lt, int quarter) {
+template <int CG, int ST>
+__device__ __forceinline__ uint32_t epi_acquire(const Pipe<CG, ST>& P, int lt, int quarter) {
     const int as = lt & 1;
     mbar_wait(&P.tfull_bar[as], (lt >> 1) & 1);
     tc_fence_after();
     return P.tmem_base + as * BN + (static_cast<uint32_t>(quarter * 32) << 16);
 }
-template <int CG>
-__device__ __forceinline__ void epi_release(const Pipe<CG>& P, int lt, int lane) {
+template <int CG, int ST>
+__device__ __forceinline__ void epi_release(const Pipe<CG, ST>& P, int lt, int lane) {
     tc_fence_before();
     __syncwarp();
     if (lane == 0) {
@@ -275,7 +289,8 @@ template <class Epi, int CG>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
             const GemmParams gp, const __grid_constant__ typename Epi::Params ep) {
-    using C = Cfg<CG>;
+    constexpr int ST = fwd_stages<CG>();
+    using C = Cfg<CG, ST>;
     extern __shared__ uint8_t smem_raw[];
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -295,7 +310,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     const int first_tile = blockIdx.x / CG, tile_step = gridDim.x / CG;
 
     if (warp == 0 && lane == 0) { prefetch_tmap(&tmA); prefetch_tmap(&tmB); }
-    Pipe<CG> P;
+    Pipe<CG, ST> P;
     P.setup(smem_raw, warp, lane);
 
     if (warp == 0) {
@@ -312,7 +327,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                 tile_coords(tile, num_m, num_n, gp.group_m, m2, n_blk);
                 t.a_c = gp.a_off + (m2 * CG + static_cast<int>(P.rank)) * BM;
                 t.b_c = gp.b_off + n_blk * BN + static_cast<int>(P.rank) * C::B_ROWS;
-                produce_tile<CG>(P, t, it);
+                produce_tile<CG, ST>(P, t, it);
             }
         }
     } else if (warp == 1) {
@@ -320,7 +335,7 @@ gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         if (P.rank == 0 && elect_one()) {
             int it = 0, lt = 0;
             for (int tile = first_tile; tile < total_tiles; tile += tile_step, ++lt)
-                mma_tile<CG>(P, gp.a_mn, gp.b_mn, kblocks * gp.nseg, lt, it);
+                mma_tile<CG, ST>(P, gp.a_mn, gp.b_mn, kblocks * gp.nseg, lt, it);
         }
     } else {
         // =========================== epilogue warps (TMEM -> registers -> global) ===========================
@@ -334,9 +349,9 @@ gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             const int m_blk = m2 * CG + static_cast<int>(P.rank);
             // per-row state (scalars, cache cursor) is fetched while the MMAs of this tile are still running
             typename Epi::State st = Epi::prepare(ep, gp, m_blk, n_blk, row_in_tile, M);
-            const uint32_t taddr = epi_acquire<CG>(P, lt, quarter);
+            const uint32_t taddr = epi_acquire<CG, ST>(P, lt, quarter);
             Epi::run(ep, gp, st, taddr, m_blk, n_blk, row_in_tile, M, P.epi_smem, epi_tid);
-            epi_release<CG>(P, lt, lane);
+            epi_release<CG, ST>(P, lt, lane);
         }
     }
     P.teardown(warp);

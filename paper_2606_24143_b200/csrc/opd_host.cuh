@@ -12,6 +12,7 @@
 #include "../../include/opd.h"
 #include "opd_bwd_kernel.cuh"
 #include "opd_estimators.cuh"
+#include "opd_sparse_bwd.cuh"
 #include "opd_producer.cuh"
 
 struct opd_handle_s {
@@ -100,12 +101,13 @@ struct Plan {
     int Tb, Vb;           // backward super-tile (rows of tokens x vocabulary columns), multiples of 128 / 256
     int est_blocks;
     size_t off_nlive, off_badidx, off_live_rows, off_xc, off_wsplit, off_sorted, off_perm, off_zc, off_beta,
-           off_partials, off_lse2, off_coef, off_gs, off_dxacc, off_block_sums, off_counters, off_wt, off_gwt, off_gw32,
+           off_partials, off_lse2, off_coef, off_gs, off_dxacc, off_block_sums, off_counters, off_wt, off_skeys, off_shist, off_gw32,
            off_seq_l1, off_seq_var1, total;
     bool sparse_bwd;      // alpha == 0 on every row: gradients live on the cached columns only (no dense backward)
     int n_super;          // number of backward super-tiles (upper bound)
     int gs_bufs;          // ring depth of the G super-tile buffer
     size_t xc_plane, w_plane, gs_plane;   // elements per plane
+    size_t sort_n; int sort_blocks;       // sparse backward: entries to sort, blocks of the radix sort
 };
 
 inline int env_int(const char* name, int dflt) {
@@ -167,9 +169,13 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int 
 #ifdef OPD_EXPERIMENTS
     if (env_int("OPD_DENSE_BWD", 0)) p.sparse_bwd = false;     // timing experiment: run the dense backward anyway
 #endif
-    // sparse backward with [d,V] storage works on [V,d] transposes (contiguous d-vectors per cached column)
+    // sparse backward: with [d,V] storage W is read through a [V,d] transposed copy (contiguous d-vectors per cached
+    // column; callers that store W as [V,d] like lm_head.weight need none); sort buffers of the T*C (column, entry) pairs
     p.off_wt = take(bwd && p.sparse_bwd ? (size_t)d * V * (fp32 ? 4 : 2) : 0);
-    p.off_gwt = take(bwd && p.sparse_bwd ? (size_t)d * V * 4 : 0);
+    p.sort_n = (size_t)p.t_pad * C;
+    p.sort_blocks = (int)((p.sort_n + RS_TILE - 1) / RS_TILE);
+    p.off_skeys = take(bwd && p.sparse_bwd ? 4 * sizeof(uint32_t) * p.sort_n : 0);          // keys / values, ping-pong
+    p.off_shist = take(bwd && p.sparse_bwd ? sizeof(uint32_t) * 256 * (size_t)p.sort_blocks : 0);
     p.off_gw32 = take(bwd && (flags & OPD_F_GRADW_BF16) ? (size_t)d * V * 4 : 0);      // fp32 sums behind a bf16 grad_W
     p.off_seq_l1 = take(sizeof(float) * (size_t)p.t_pad);                               // per-token terms of opd_set_seq_diagnostics
     p.off_seq_var1 = take(sizeof(float) * (size_t)p.t_pad);
@@ -195,12 +201,12 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int 
 // Launch `kernel` on `grid` CTAs of GEMM_THREADS threads; CG = 2 launches clusters of two CTAs (a pair per tile).
 // `window` (optional): an L2 access-policy window for this launch only (persisting hits inside [base, base + bytes)).
 struct L2Window { void* base = nullptr; size_t bytes = 0; float hit_ratio = 1.f; };
-template <int CG, class... KArgs, class... Args>
+template <int CG, int ST, class... KArgs, class... Args>
 inline cudaError_t launch_cg_w(void (*kernel)(KArgs...), int grid, cudaStream_t st, const L2Window& window, Args&&... args) {
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<CG>::SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<CG, ST>::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(GEMM_THREADS); cfg.dynamicSmemBytes = Cfg<CG>::SMEM_BYTES; cfg.stream = st;
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(GEMM_THREADS); cfg.dynamicSmemBytes = Cfg<CG, ST>::SMEM_BYTES; cfg.stream = st;
     cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
@@ -216,18 +222,18 @@ inline cudaError_t launch_cg_w(void (*kernel)(KArgs...), int grid, cudaStream_t 
     }
     return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
-template <int CG, class... KArgs, class... Args>
+template <int CG, int ST, class... KArgs, class... Args>
 inline cudaError_t launch_cg(void (*kernel)(KArgs...), int grid, cudaStream_t st, Args&&... args) {
-    return launch_cg_w<CG>(kernel, grid, st, L2Window{}, std::forward<Args>(args)...);
+    return launch_cg_w<CG, ST>(kernel, grid, st, L2Window{}, std::forward<Args>(args)...);
 }
 
 // Number of clusters (CG = 2) / CTAs (CG = 1) of `kernel` that can be resident at the same time on the current device:
 // the persistent kernels size their grid with it (one wave; more CTAs would only queue behind the resident ones).
-template <int CG, class... KArgs>
+template <int CG, int ST, class... KArgs>
 inline int max_resident_groups(void (*kernel)(KArgs...), int num_sms) {
-    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<CG>::SMEM_BYTES) != cudaSuccess) return 0;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<CG, ST>::SMEM_BYTES) != cudaSuccess) return 0;
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(num_sms / CG * CG); cfg.blockDim = dim3(GEMM_THREADS); cfg.dynamicSmemBytes = Cfg<CG>::SMEM_BYTES;
+    cfg.gridDim = dim3(num_sms / CG * CG); cfg.blockDim = dim3(GEMM_THREADS); cfg.dynamicSmemBytes = Cfg<CG, ST>::SMEM_BYTES;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
@@ -240,10 +246,10 @@ inline int max_resident_groups(void (*kernel)(KArgs...), int num_sms) {
 template <class Epi, int CG>
 inline cudaError_t launch_gemm_cg(opd_handle_s* h, cudaStream_t st, const CUtensorMap& tA, const CUtensorMap& tB,
                                   const GemmParams& gp, const typename Epi::Params& ep) {
-    const long tiles = (long)ceil_div(gp.M, Cfg<CG>::TILE_M) * gp.num_n;
+    const long tiles = (long)ceil_div(gp.M, BM * CG) * gp.num_n;
     const int grid = CG * (int)std::min<long>(tiles, h->num_sms / CG);
     if (grid <= 0) return cudaSuccess;
-    cudaError_t e = launch_cg<CG>(gemm_kernel<Epi, CG>, grid, st, tA, tB, gp, ep);
+    cudaError_t e = launch_cg<CG, fwd_stages<CG>()>(gemm_kernel<Epi, CG>, grid, st, tA, tB, gp, ep);
     h->n_kernels++;
     h->n_gemm++;
     return e != cudaSuccess ? e : cudaGetLastError();

@@ -26,14 +26,15 @@ static opd_status_t launch_bwd(opd_handle_s* h, cudaStream_t st, const CUtensorM
                                const L2Window& win = L2Window{}) {
     int& cached = h->bwd_grid[h->cg][DENSE ? 1 : 0];      // per handle = per device; a failed query is not cached
     if (cached < 1) {
-        const int r = h->cg == 2 ? max_resident_groups<2>(bwd_kernel<2, DENSE>, h->num_sms)
-                                 : max_resident_groups<1>(bwd_kernel<1, DENSE>, h->num_sms);
+        const int r = h->cg == 2 ? max_resident_groups<2, bwd_stages<2>()>(bwd_kernel<2, DENSE>, h->num_sms)
+                                 : max_resident_groups<1, bwd_stages<1>()>(bwd_kernel<1, DENSE>, h->num_sms);
         if (r < 1) OPD_FAIL(h, OPD_ERR_CUDA, "the backward kernel cannot be made resident on device %d", h->device);
         cached = r * h->cg;
     }
     const int grid = cached;
-    if (h->cg == 2) OPD_CUDA(h, launch_cg_w<2>(bwd_kernel<2, DENSE>, grid, st, win, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
-    else OPD_CUDA(h, launch_cg_w<1>(bwd_kernel<1, DENSE>, grid, st, win, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
+    constexpr int S2 = bwd_stages<2>(), S1 = bwd_stages<1>();
+    if (h->cg == 2) OPD_CUDA(h, (launch_cg_w<2, S2>)(bwd_kernel<2, DENSE>, grid, st, win, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
+    else OPD_CUDA(h, (launch_cg_w<1, S1>)(bwd_kernel<1, DENSE>, grid, st, win, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
     return OPD_OK;
 }
 
@@ -124,10 +125,10 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         OPD_CUDA(h, cudaMemset2DAsync(a.grad_hidden, (size_t)a.ld_gh * esz, 0, (size_t)d * esz, T, st));
     }
     k_compact<<<1, 1024, 0, st>>>(a.mask, T, a.all_live ? 1 : 0, live_rows, n_live);
-    if (!fwd_only && !gw_accum) {
+    if (!fwd_only && !gw_accum && !p.sparse_bwd) {
         // An overwriting call needs no memset of grad_W: the grad_W tiles of the first token super-tile store (dense
-        // backward).  Only the sparse backward (scatter-adds) and a call without any live token start from zeros.
-        k_zero_matrix<<<h->num_sms * 4, 256, 0, st>>>(gw32, ldgw32, gw_rows, gw_cols, p.sparse_bwd ? nullptr : n_live);
+        // backward; the sparse backward writes every column exactly once).  Only a call without any live token zeroes it.
+        k_zero_matrix<<<h->num_sms * 4, 256, 0, st>>>(gw32, ldgw32, gw_rows, gw_cols, n_live);
         h->n_kernels++;
     }
     k_gather_rows<<<p.t_pad, 256, 0, st>>>(a.hidden, a.ld_hidden, fp32 ? 1 : 0, d, p.t_pad, live_rows, n_live, xc, (long)p.xc_plane);
@@ -236,30 +237,39 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     // alpha_t == 0 on every row: the gradient lives on the cached columns only, no softmax tile has to be re-formed
     const bool sparse_bwd = p.sparse_bwd;
     if (!fwd_only && sparse_bwd) {
-        const void* Wv = a.W;                                   // [V,d] view of W / grad_W: contiguous d-vectors per column
-        float* gwv = gw32;
-        long ldwv = ldw, ldgv = ldgw32;
+        const void* Wv = a.W;                                   // [V,d] view of W: contiguous d-vectors per column
+        long ldwv = ldw;
         if (wl == 0) {
             void* wt = ws + p.off_wt;
-            gwv = reinterpret_cast<float*>(ws + p.off_gwt);
             const dim3 tg(ceil_div(V, 32), ceil_div(d, 32));
-            if (fp32) k_transpose<float><<<tg, dim3(32, 8), 0, st>>>(static_cast<const float*>(a.W), ldw, d, V, static_cast<float*>(wt), (long)d, 0);
+            if (fp32) k_transpose<float><<<tg, dim3(32, 8), 0, st>>>(static_cast<const float*>(a.W), ldw, d, V, static_cast<float*>(wt), (long)d);
             else k_transpose<__nv_bfloat16><<<tg, dim3(32, 8), 0, st>>>(static_cast<const __nv_bfloat16*>(a.W), ldw, d, V,
-                                                                        static_cast<__nv_bfloat16*>(wt), (long)d, 0);
-            OPD_CUDA(h, cudaMemsetAsync(gwv, 0, sizeof(float) * (size_t)d * V, st));
-            Wv = wt; ldwv = d; ldgv = d;
+                                                                        static_cast<__nv_bfloat16*>(wt), (long)d);
+            Wv = wt; ldwv = d;
             h->n_kernels++;
         }
-        if (fp32) k_sparse_bwd<float><<<p.t_pad, 256, 0, st>>>(a.hidden, a.ld_hidden, Wv, ldwv, d, C, sorted_idx, beta, live_rows, n_live,
-                                                               a.grad_hidden, a.ld_gh, gwv, ldgv);
-        else k_sparse_bwd<__nv_bfloat16><<<p.t_pad, 256, 0, st>>>(a.hidden, a.ld_hidden, Wv, ldwv, d, C, sorted_idx, beta, live_rows, n_live,
-                                                                  a.grad_hidden, a.ld_gh, gwv, ldgv);
-        h->n_kernels++;
-        if (wl == 0) {                                          // grad_W[d,V] += gWt^T
-            const dim3 tg(ceil_div(d, 32), ceil_div(V, 32));
-            k_transpose<float><<<tg, dim3(32, 8), 0, st>>>(gwv, (long)d, V, d, gw32, ldgw32, 1);
-            h->n_kernels++;
+        if (fp32) k_sparse_gh<float><<<p.t_pad, 256, 0, st>>>(Wv, ldwv, d, C, sorted_idx, beta, live_rows, n_live, a.grad_hidden, a.ld_gh);
+        else k_sparse_gh<__nv_bfloat16><<<p.t_pad, 256, 0, st>>>(Wv, ldwv, d, C, sorted_idx, beta, live_rows, n_live, a.grad_hidden, a.ld_gh);
+        // grad_W: sort the (column, entry) pairs by column (stable), then one block per group of 8 columns
+        const size_t N = p.sort_n;
+        uint32_t* kbuf[2] = {reinterpret_cast<uint32_t*>(ws + p.off_skeys), reinterpret_cast<uint32_t*>(ws + p.off_skeys) + N};
+        uint32_t* vbuf[2] = {kbuf[1] + N, kbuf[1] + 2 * N};
+        uint32_t* hist = reinterpret_cast<uint32_t*>(ws + p.off_shist);
+        k_sparse_keys<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(sorted_idx, C, N, n_live, V, kbuf[0], vbuf[0]);
+        int key_bits = 1;
+        while ((1u << key_bits) <= (unsigned)V && key_bits < 32) ++key_bits;                 // keys are in [0, V]
+        int cur = 0;
+        for (int shift = 0; shift < key_bits; shift += 8, cur ^= 1) {
+            k_radix_hist<<<p.sort_blocks, 256, 0, st>>>(kbuf[cur], N, shift, hist, p.sort_blocks);
+            k_radix_scan<<<1, 1024, 0, st>>>(hist, (size_t)256 * p.sort_blocks);
+            k_radix_scatter<<<p.sort_blocks, 256, 0, st>>>(kbuf[cur], vbuf[cur], N, shift, hist, p.sort_blocks, kbuf[cur ^ 1], vbuf[cur ^ 1]);
+            h->n_kernels += 3;
         }
+        if (fp32) k_sparse_gw<float><<<V / 8, 256, 0, st>>>(kbuf[cur], vbuf[cur], N, V, C, beta, live_rows, a.hidden, a.ld_hidden, d,
+                                                             gw32, ldgw32, wl, gw_accum ? 1 : 0);
+        else k_sparse_gw<__nv_bfloat16><<<V / 8, 256, 0, st>>>(kbuf[cur], vbuf[cur], N, V, C, beta, live_rows, a.hidden, a.ld_hidden, d,
+                                                                gw32, ldgw32, wl, gw_accum ? 1 : 0);
+        h->n_kernels += 3;
         OPD_CUDA(h, cudaGetLastError());
     }
     if (!fwd_only && !sparse_bwd) {
@@ -271,6 +281,7 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         bp.d = d; bp.V = V; bp.Tb = p.Tb; bp.Vb = p.Vb; bp.nvb = ceil_div(V, p.Vb); bp.wl = wl; bp.planes = p.planes; bp.gbufs = p.gs_bufs;
         bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super; bp.ticket = counters + 2 * p.n_super;
         bp.dw_store_first = gw_accum ? 0 : 1;
+        bp.order = env_int("OPD_BWD_ORDER", 0) & 15;
         bp.g = GEpi::Params{gs, p.Tb, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V, 0ull};
         { const int gh_ = env_int("OPD_HINT_GST", 0); bp.g.st_hint = gh_ ? hint_policy(gh_) : 0ull; }
         bp.dx = dxp;

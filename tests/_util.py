@@ -10,7 +10,7 @@ import numpy as np
 import torch
 
 from oracle import opd_oracle as O
-from paper_2606_24143_b200 import synth
+from gen import synth
 
 GRAD_TOL = {"bf16": 1e-2, "fp32": 1e-4}
 LOSS_RTOL = 2e-3

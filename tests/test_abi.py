@@ -48,7 +48,7 @@ def test_enum_values_match_header():
 
 def test_workspace_plan_has_no_logits_sized_buffer(lib):
     """Host-only: opd_workspace_bytes at the BASELINE.json shapes stays far below T*V*2 bytes."""
-    from paper_2606_24143_b200 import synth
+    from gen import synth
     assert b"sm_100a" in lib.opd_version()
     for c in (2, 3, 4, 5):
         cfg = synth.CONFIGS[c]

@@ -5,7 +5,7 @@ import pytest
 import torch
 
 from oracle import opd_oracle as O
-from paper_2606_24143_b200 import synth
+from gen import synth
 from tests._util import GRAD_TOL, LOSS_RTOL, check_grad, f64
 
 pytestmark = pytest.mark.gpu

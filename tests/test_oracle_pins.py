@@ -10,7 +10,7 @@ import pytest
 import torch
 
 from oracle import opd_oracle as O
-from paper_2606_24143_b200 import synth
+from gen import synth
 
 
 def tiny(seed, T=4, d=6, V=12, C=3, dup=False, mask=None):

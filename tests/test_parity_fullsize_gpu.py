@@ -14,7 +14,7 @@ import pytest
 import torch
 
 from oracle import opd_oracle as O
-from paper_2606_24143_b200 import synth
+from gen import synth
 from tests._util import GRAD_TOL, LOGP_ATOL, LOSS_RTOL, check_grad, compare_all, f64, oracle_for, pick
 
 pytestmark = pytest.mark.gpu

@@ -7,7 +7,7 @@ import pytest
 import torch
 
 from oracle import opd_oracle as O
-from paper_2606_24143_b200 import synth
+from gen import synth
 from tests._util import GRAD_TOL, LOGP_ATOL, check_grad, check_loss, compare_all, f64, oracle_for, pick
 
 pytestmark = pytest.mark.gpu
@@ -407,11 +407,12 @@ def test_autograd_entry(handle):
     assert abs(l2.item() - loss.item()) <= 1e-6
 
 
-@pytest.mark.parametrize("mode", [O.RKL_MC, O.MIXED])
+@pytest.mark.parametrize("mode", [O.RKL_MC, O.MIXED, O.RKL_TOPK, O.FKL_TOPK])
 def test_results_are_bitwise_reproducible(handle, mode, monkeypatch):
     """The summation order is fixed (tiles are reduced into the fp32 accumulators in super-tile order, enforced by the
-    dependency counters): repeated calls give bit-identical losses and gradients. A race in the barrier / counter protocol
-    of the persistent kernels would show up here."""
+    dependency counters, whichever CTA runs a tile; the sparse backward of OPD_RKL_TOPK sums every grad_W column in sorted
+    (token, slot) order without atomics): repeated calls give bit-identical losses and gradients in every mode. A race in
+    the barrier / counter protocol of the persistent kernels would show up here."""
     monkeypatch.setenv("OPD_TB", "256"); monkeypatch.setenv("OPD_VB", "512")      # many super-tiles -> many dependencies
     cfg = dict(RAGGED, T=1500, V=4104)
     inp = synth.make_inputs(cfg, c=18, device=DEV)

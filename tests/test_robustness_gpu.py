@@ -8,7 +8,7 @@ import pytest
 import torch
 
 from oracle import opd_oracle as O
-from paper_2606_24143_b200 import synth
+from gen import synth
 from tests._util import check_grad, check_loss, compare_all, f64, oracle_for, pick
 
 pytestmark = pytest.mark.gpu
@@ -192,9 +192,6 @@ def test_seeded_soak(handle, opd, monkeypatch):
             r = handle.loss_fwd_bwd(inp["hidden"], W, idx, lam, old, m, mode, kk, want_lse=True, want_student_logp=True)
             torch.cuda.synchronize()
             outs.append(_outputs(r))
-        # grad_W of the purely sparse backward (OPD_RKL_TOPK) is summed with fp32 atomics: equal up to summation order only
-        exact = (0, 1, 2) if mode == O.RKL_TOPK else (0, 1, 2, 3)
-        assert all(torch.equal(outs[0][q], outs[1][q]) for q in exact), (case, cfg, mode)
-        assert torch.allclose(outs[0][3], outs[1][3], rtol=1e-4, atol=1e-6 * outs[0][3].abs().max().item())
+        assert all(torch.equal(a, b) for a, b in zip(*outs)), (case, cfg, mode)
         if case % 3 == 0:
             compare_all(r, oracle_for(inp, idx, lam, old, mode, kk), f64(m), dtype)

@@ -11,7 +11,8 @@ import torch.distributed as dist
 import torch.multiprocessing as mp
 
 from oracle import opd_oracle as O
-from paper_2606_24143_b200 import shard, synth
+from gen import synth
+from paper_2606_24143_b200 import shard
 
 CFG = dict(dtype="fp32", T=96, d=16, V=64, k=4, K=3, sigma=0.05, mask="random10")
 
