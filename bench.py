@@ -30,7 +30,7 @@ UNIT = "live tokens/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from one committed `ncu --set full` capture of this
 # workload (a citation: bench.py never runs under a profiler, so the line carries "traffic_measured": false)
 NCU_TRAFFIC = {
-    "C4": dict(bwd_kernel=157_306_721_000, fwd_kernel=37_047_861_000, source="profiles/r01d_final_c4.md"),
+    "C4": dict(bwd_kernel=150_634_613_000, fwd_kernel=20_625_665_000, source="profiles/r02_final_c4.md"),
 }
 
 
@@ -359,10 +359,12 @@ def main():
         outs = [host_out(), host_out()]
         del gw, gh
         torch.cuda.empty_cache()
-        n_e2e = max(2, min(args.steps, 5))
+        n_e2e = max(2, min(args.steps, 20))      # the fill (first copy-in) and drain (last copy-out) of the pipeline are inside the timed region
+
+        e2e_flags = 0
 
         def submit(i):
-            h.host_submit(i % 2, hh["hidden"], hh["W"], hidx, hlam, hold, hh["mask"], mode, kk, outs[i % 2])
+            h.host_submit(i % 2, hh["hidden"], hh["W"], hidx, hlam, hold, hh["mask"], mode, kk, outs[i % 2], flags=e2e_flags)
 
         # every step copies its inputs from pinned host memory and its results (loss, per-token KL, both gradients) back;
         # the two staging slots overlap step i's kernels with the copy-in of step i+1 and the copy-out of step i-1
@@ -389,6 +391,21 @@ def main():
                    steps=n_e2e, ms_per_step=dt * 1e3, loss=float(o["loss"].item()),
                    api="opd_loss_fwd_bwd_host_submit/_wait, 2 staging slots (copies of neighbouring steps overlap the kernels)",
                    unpipelined_ms_per_step=dt_sync * 1e3)
+        # the same with a bf16 grad_W (OPD_F_GRADW_BF16): half the bytes of the largest copy back
+        e2e_flags = opd.F_GRADW_BF16
+        for o_ in outs:
+            o_["grad_W"] = torch.empty(d, V, dtype=torch.bfloat16).pin_memory()
+        submit(0); h.host_wait(0)
+        barrier()
+        t2 = time.perf_counter()
+        submit(0)
+        for i in range(1, n_e2e):
+            submit(i)
+            _, up16, down16 = h.host_wait((i - 1) % 2)
+        _, up16, down16 = h.host_wait((n_e2e - 1) % 2)
+        barrier()
+        dt16 = (time.perf_counter() - t2) / n_e2e
+        e2e["bf16_grad_W"] = dict(value=n_live / dt16, ms_per_step=dt16 * 1e3, h2d_bytes_per_step=int(up16), d2h_bytes_per_step=int(down16))
 
     if rank != 0:
         if dist is not None:

@@ -145,7 +145,10 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int 
             if (best_waste < 0 || waste < best_waste) { best_waste = waste; tb = cand; }
         }
     }
-    const int vb = env_int("OPD_VB", 4096);
+    // Vocabulary columns per super-tile = K depth of a grad_hidden tile: 8192 for large batches (half as many fp32 partial-sum
+    // passes: DRAM writes 50 -> 40 GB per C4 launch, tensor pipe 86 -> 89.5% busy under ncu, profiles/r02_supertile_sweep.md),
+    // 4096 otherwise (keeps the G ring, and with it the workspace, below 5% of the logits for small T)
+    const int vb = env_int("OPD_VB", p.t_pad >= 32768 ? 8192 : 4096);
     p.Tb = std::min(p.t_pad, std::max(TM, tb / TM * TM));
     p.Vb = std::min(p.num_n * BN, std::max(BN, vb / BN * BN));
     p.est_blocks = ceil_div(T, 128);

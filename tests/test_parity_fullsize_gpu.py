@@ -58,7 +58,11 @@ def sampled_check(handle, cfg, c, mode, n_rows=12):
     gmax = gw.abs().max().item()
     colsum = gw.double().sum(dim=1)
     V = gw.shape[1]
-    assert colsum.abs().max().item() <= 1e-2 * gmax * np.sqrt(V)        # bf16 rounding of G: random-walk bound
+    # every row of G sums to 0 up to the bf16 rounding of its entries (relative 2^-9 each): sum_v grad_W[k,v] is a random walk
+    # over the live tokens of those per-row residuals, about 2^-9 sqrt(n_live * C) |x| |beta| / N against a largest entry of a few
+    # |x| |beta| / N, so a bound of 1e-2 gmax sqrt(n_live) leaves a factor of about 4 (the element-wise column checks below
+    # are the primary grad_W test)
+    assert colsum.abs().max().item() <= 1e-2 * gmax * np.sqrt(live.size)
     lhs = (inp["W"].double() * gw.double()).sum(dim=1)
     rhs = (inp["hidden"].double() * gh.double()).sum(dim=0)
     assert (lhs - rhs).abs().max().item() <= 2e-2 * max(lhs.abs().max().item(), 1e-30)
