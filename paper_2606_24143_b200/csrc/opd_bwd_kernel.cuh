@@ -6,7 +6,7 @@
 //   G(s)   logits of super-tile s recomputed -> G tile (bf16) into buffer s%R of the G ring (consumed from L2)
 //   DX(s)  grad_hidden[tb] (+)= G(s) . W[:,vb]^T        DW(s)  grad_W[:,vb] += Xc[tb]^T . G(s)
 //
-// CTA pairs claim items dynamically, in list order, from a global ticket counter (ticket_claim / ticket_read in
+// CTA pairs claim items dynamically, in list order, from a global ticket counter (ticket_take / ticket_publish / ticket_read in
 // opd_gemm.cuh); an item only depends on earlier items, through two counters per super-tile in global memory
 // (release by the epilogue after its stores, acquire by whoever consumes):
 //   g_done[s] == #G tiles      before the TMA producer loads G(s) for a DX/DW tile
@@ -53,90 +53,85 @@ enum { T_G = 0, T_DX = 1, T_DW = 2, T_Q = 3 };
 
 struct BwdTile {
     int type, s, tb0, vb0, Tb_eff, Vb_eff, vi, m_blk, n_blk;
+    int ng;                    // G tiles of super-tile s (what a DX / DW tile waits for)
 };
 
 // DENSE: block b holds Q(b), G(b-1), DX(b-2), DW(b-2) (the Q tiles of a super-tile run one block ahead of its G tiles);
 // otherwise block b holds G(b), DX(b-1), DW(b-1).
+// The decoder keeps the tile counts and extents of the current block's super-tiles (one integer division per new block),
+// so that decoding an item costs a few compares and one division: every warp role decodes every item of its CTA, the MMA
+// issuer between two tiles (while the tensor pipe drains its queue).
 template <int CG, bool DENSE>
 struct BwdSched {
     static constexpr int GOFF = DENSE ? 1 : 0;
     static constexpr int TM = BM * CG;
-    int S, nvb, Tb, Vb, V, d, wl, n_live;
+    struct Super { int s, ti, vi, tb_eff, vb_eff, mt, nt, ng, ndx, ndw; };
+    int S, nvb, Tb, Vb, V, d, wl, n_live, dm, dn;
     int order;      // tile order knobs (result-neutral): bit 0 grad_W tiles before grad_hidden tiles inside a block,
                     // bits 1-3: n-fastest raster of the G / grad_hidden / grad_W tiles (default m fastest)
     int blk;        // current block
     long base;      // items before the current block
+    int sz;         // items of the current block
+    Super q, g, c;  // super-tiles whose Q / G / (DX, DW) tiles the current block holds (s = -1: none)
+    __device__ __forceinline__ void super_info(int s, Super& o) const {
+        o.s = s;
+        if (s < 0 || s >= S) { o.s = -1; o.ng = o.ndx = o.ndw = 0; return; }
+        o.ti = s / nvb; o.vi = s - o.ti * nvb;
+        o.tb_eff = min(Tb, n_live - o.ti * Tb);
+        o.vb_eff = min(Vb, V - o.vi * Vb);
+        o.mt = (o.tb_eff + TM - 1) / TM;
+        o.nt = (o.vb_eff + BN - 1) / BN;
+        o.ng = o.mt * o.nt;
+        o.ndx = o.mt * dn;
+        o.ndw = wl == 0 ? dm * o.nt : ((o.vb_eff + TM - 1) / TM) * dn;
+    }
+    __device__ __forceinline__ void load_block() {
+        if (DENSE) super_info(blk, q); else { q.s = -1; q.ng = 0; }
+        super_info(blk - GOFF, g);
+        super_info(blk - GOFF - 1, c);
+        sz = q.ng + g.ng + c.ndx + c.ndw;
+    }
     __device__ __forceinline__ void init(const BwdParams& p) {
         n_live = *p.n_live;
         nvb = p.nvb; Tb = p.Tb; Vb = p.Vb; V = p.V; d = p.d; wl = p.wl; order = p.order;
+        dm = (d + TM - 1) / TM; dn = (d + BN - 1) / BN;
         S = ((n_live + Tb - 1) / Tb) * nvb;
         blk = 0; base = 0;
-    }
-    __device__ __forceinline__ void dims(int s, int& mt, int& nt, int& tb_eff, int& vb_eff) const {
-        const int ti = s / nvb, vi = s - ti * nvb;
-        tb_eff = min(Tb, n_live - ti * Tb);
-        vb_eff = min(Vb, V - vi * Vb);
-        mt = (tb_eff + TM - 1) / TM;
-        nt = (vb_eff + BN - 1) / BN;
+        load_block();
     }
     // tile counts (a tile = one CTA's or one CTA pair's TM x 256 output block)
-    __device__ __forceinline__ int nG(int s) const { int mt, nt, a, b; dims(s, mt, nt, a, b); return mt * nt; }
-    __device__ __forceinline__ int nDX(int s) const { int mt, nt, a, b; dims(s, mt, nt, a, b); return mt * ((d + BN - 1) / BN); }
-    __device__ __forceinline__ int nDW(int s) const {
-        int mt, nt, a, b; dims(s, mt, nt, a, b);
-        return wl == 0 ? ((d + TM - 1) / TM) * nt : ((b + TM - 1) / TM) * ((d + BN - 1) / BN);
-    }
-    __device__ __forceinline__ int block_size(int b) const {
-        const int g = b - GOFF, c = b - GOFF - 1;
-        return (DENSE && b < S ? nG(b) : 0) + (g >= 0 && g < S ? nG(g) : 0) + (c >= 0 && c < S ? nDX(c) + nDW(c) : 0);
-    }
+    __device__ __forceinline__ int nG(int s) const { Super o; super_info(s, o); return o.ng; }
+    __device__ __forceinline__ int nDX(int s) const { Super o; super_info(s, o); return o.ndx; }
+    __device__ __forceinline__ int nDW(int s) const { Super o; super_info(s, o); return o.ndw; }
     // decode `item` (monotonically increasing between calls); false when the list is exhausted
     __device__ __forceinline__ bool get(long item, BwdTile& t) {
         if (S <= 0) return false;
-        while (blk <= S + GOFF) {
-            const int sz = block_size(blk);
-            if (item < base + sz) break;
+        while (blk <= S + GOFF && item >= base + sz) {
             base += sz; ++blk;
+            if (blk <= S + GOFF) {                   // shift: the next block's (DX, DW) super-tile is this block's G super-tile
+                if (DENSE) { c = g; g = q; super_info(blk, q); } else { c = g; super_info(blk, g); }
+                sz = q.ng + g.ng + c.ndx + c.ndw;
+            }
         }
         if (blk > S + GOFF) return false;
         int r = static_cast<int>(item - base);
-        int rows;
-        const int g = blk - GOFF;
-        t.type = -1;
-        if (DENSE && blk < S) {
-            const int nq = nG(blk);
-            if (r < nq) { t.type = T_Q; t.s = blk; } else r -= nq;
+        const Super* u;
+        if (DENSE && r < q.ng) { t.type = T_Q; u = &q; }
+        else if ((r -= q.ng) < g.ng) { t.type = T_G; u = &g; }
+        else {
+            r -= g.ng; u = &c;
+            if (order & 1) { if (r < c.ndw) t.type = T_DW; else { t.type = T_DX; r -= c.ndw; } }
+            else { if (r < c.ndx) t.type = T_DX; else { t.type = T_DW; r -= c.ndx; } }
         }
-        if (t.type < 0 && g >= 0 && g < S) {
-            const int ng = nG(g);
-            if (r < ng) { t.type = T_G; t.s = g; } else r -= ng;
-        }
-        if (t.type < 0) {
-            t.s = g - 1;
-            if (order & 1) {
-                const int ndw = nDW(t.s);
-                if (r < ndw) t.type = T_DW; else { t.type = T_DX; r -= ndw; }
-            } else {
-                const int ndx = nDX(t.s);
-                if (r < ndx) t.type = T_DX; else { t.type = T_DW; r -= ndx; }
-            }
-        }
-        int mt, nt;
-        dims(t.s, mt, nt, t.Tb_eff, t.Vb_eff);
-        const int ti = t.s / nvb;
-        t.vi = t.s - ti * nvb;
-        t.tb0 = ti * Tb; t.vb0 = t.vi * Vb;
-        if (t.type == T_DW) rows = wl == 0 ? (d + TM - 1) / TM : (t.Vb_eff + TM - 1) / TM;
-        else rows = mt;
+        t.s = u->s; t.vi = u->vi; t.Tb_eff = u->tb_eff; t.Vb_eff = u->vb_eff; t.ng = u->ng;
+        t.tb0 = u->ti * Tb; t.vb0 = u->vi * Vb;
+        const int rows = t.type == T_DW ? (wl == 0 ? dm : (u->vb_eff + TM - 1) / TM) : u->mt;
         const int tbit = t.type == T_DX ? 4 : (t.type == T_DW ? 8 : 2);
         if (order & tbit) {                          // n fastest: concurrently running CTAs share the A panel
-            int cols;
-            if (t.type == T_DX) cols = (d + BN - 1) / BN;
-            else if (t.type == T_DW) cols = wl == 0 ? nt : (d + BN - 1) / BN;
-            else cols = nt;
-            t.n_blk = r % cols; t.m_blk = r / cols;
-        } else {
-            t.m_blk = r % rows; t.n_blk = r / rows;  // m fastest: concurrently running CTAs share the B panel
+            const int cols = t.type == T_DX ? dn : (t.type == T_DW ? (wl == 0 ? u->nt : dn) : u->nt);
+            t.m_blk = r / cols; t.n_blk = r - t.m_blk * cols;
+        } else {                                     // m fastest: concurrently running CTAs share the B panel
+            t.n_blk = r / rows; t.m_blk = r - t.n_blk * rows;
         }
         return true;
     }
@@ -189,13 +184,25 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
         // =========================== TMA producer ===========================
         if (elect_one()) {
             BwdSched<CG, DENSE> sc; sc.init(bp);
-            BwdTile t;
-            int it = 0;
-            for (int n = 0;; ++n) {
-                // CG = 1: the producer claims the next item itself; CG = 2: both producers read what the peer's warp 1 claimed
-                const uint32_t item = CG == 1 ? ticket_claim<CG, ST>(P, bp.ticket, n) : ticket_read<CG, ST>(P, n);
-                if (!sc.get(item, t)) break;
-                if (!on(t.type)) continue;
+            BwdTile t, nxt;
+            int it = 0, n = 0, g_ready = -1;
+            // next enabled item of this CTA (pair).  CG = 1: the producer claims it itself; CG = 2: both producers read
+            // what the peer's warp 1 claimed.  Never called again once the list is exhausted.
+            auto fetch = [&](BwdTile& o) -> bool {
+                if constexpr (CG == 1) {
+                    for (;;) {                               // claim; publish what this launch runs (and the end of the list)
+                        const uint32_t item = ticket_take(bp.ticket);
+                        const bool ok = sc.get(item, o);
+                        if (ok && !on(o.type)) continue;
+                        ticket_publish<CG, ST>(P, n++, item);
+                        return ok;
+                    }
+                } else {
+                    return sc.get(ticket_read<CG, ST>(P, n++), o);
+                }
+            };
+            bool have = fetch(t), have_next = false;
+            while (have) {
                 TileOp op;
                 int pa_off = 0, pb_off = 0;
                 const int buf = t.s % bp.gbufs;
@@ -226,11 +233,13 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                     op.pa[i] = static_cast<unsigned char>(pa_off + (nseg == 1 ? 0 : PA[i]));
                     op.pb[i] = static_cast<unsigned char>(pb_off + (nseg == 1 ? 0 : PB[i]));
                 }
-                if ((t.type == T_DX || t.type == T_DW) && on(T_G)) {   // the G super-tile must be complete before TMA reads it
-                    wait_counter(bp.g_done + t.s, CG * sc.nG(t.s));
-                    fence_proxy_async_all();
+                if ((t.type == T_DX || t.type == T_DW) && on(T_G) && t.s != g_ready) {   // the G super-tile must be complete
+                    wait_counter(bp.g_done + t.s, CG * t.ng);                             // before TMA reads it (checked once
+                    fence_proxy_async_all();                                              // per super-tile, not per tile)
+                    g_ready = t.s;
                 }
-                produce_tile<CG, ST>(P, op, it);
+                produce_tile<CG, ST>(P, op, it, [&] { have_next = fetch(nxt); });
+                t = nxt; have = have_next;
             }
         }
     } else if (warp == 1) {
@@ -238,24 +247,31 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
         if (CG == 2 && rank == 1 && elect_one()) {
             BwdSched<CG, DENSE> sc; sc.init(bp);
             BwdTile t;
-            for (int n = 0;; ++n)
-                if (!sc.get(ticket_claim<CG, ST>(P, bp.ticket, n), t)) break;
+            for (int n = 0;;) {
+                const uint32_t item = ticket_take(bp.ticket);
+                const bool ok = sc.get(item, t);
+                if (ok && !on(t.type)) continue;         // tile types this launch does not run are never published
+                ticket_publish<CG, ST>(P, n++, item);
+                if (!ok) break;                          // the end of the list is published too: every reader stops on it
+            }
         }
         // =========================== MMA issuer ===========================
         if (rank == 0 && elect_one()) {
             BwdSched<CG, DENSE> sc; sc.init(bp);
-            BwdTile t;
-            int it = 0, lt = 0;
-            for (int n = 0;; ++n) {
-                if (!sc.get(ticket_read<CG, ST>(P, n), t)) break;
-                if (!on(t.type)) continue;
+            BwdTile t, nxt;
+            int it = 0, lt = 0, n = 0;
+            auto fetch = [&](BwdTile& o) -> bool { return sc.get(ticket_read<CG, ST>(P, n++), o); };
+            bool have = fetch(t), have_next = false;
+            while (have) {
                 int a_mn, b_mn, K;
                 if (t.type == T_G) { a_mn = 0; b_mn = (bp.wl == 0); K = bp.d; }
                 else if (DENSE && t.type == T_Q) { a_mn = 0; b_mn = (bp.wl_t == 0); K = bp.dT; }
                 else if (t.type == T_DX) { a_mn = 0; b_mn = (bp.wl == 1); K = t.Vb_eff; }
                 else { a_mn = 1; b_mn = 1; K = t.Tb_eff; }
-                mma_tile<CG, ST>(P, a_mn, b_mn, ((K + BK - 1) / BK) * nseg, lt, it);
+                // the next tile is fetched and decoded after this tile's first MMAs are queued, not between two tiles
+                mma_tile<CG, ST>(P, a_mn, b_mn, ((K + BK - 1) / BK) * nseg, lt, it, [&] { have_next = fetch(nxt); });
                 ++lt;
+                t = nxt; have = have_next;
             }
         }
     } else {
@@ -266,6 +282,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
         BwdSched<CG, DENSE> sc; sc.init(bp);
         BwdTile t;
         int lt = 0;
+        int c_ready = -1, gq_ready = -1, q_ready = -1;              // dependencies already seen complete (warp-uniform)
         auto wait_for = [&](const int* counter, int expected) {      // warp-level acquire of a dependency counter
             if (lane == 0) { wait_counter(counter, expected); fence_proxy_async_all(); }
             __syncwarp();
@@ -275,17 +292,17 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             if (lane == 0) item = ticket_read<CG, ST>(P, n);
             item = __shfl_sync(0xffffffffu, item, 0);
             if (!sc.get(item, t)) break;
-            if (!on(t.type)) continue;
             const int m_blk = t.m_blk * CG + rank;    // this CTA's 128-row block inside the GEMM
             GemmParams gp{};                      // the fields the epilogues read
             gp.tok_off = t.tb0;
             // wait for the previous writer / readers of what this epilogue is about to write (and, dense, for its Q tile)
+            // (each dependency is checked once per super-tile, not once per tile: c_done completes in super-tile order)
             if (t.type == T_Q) {
-                if (t.s >= 2 && on(T_G)) wait_for(bp.g_done + t.s - 2, CG * sc.nG(t.s - 2));
+                if (t.s >= 2 && on(T_G) && t.s - 2 != gq_ready) { wait_for(bp.g_done + t.s - 2, CG * sc.nG(t.s - 2)); gq_ready = t.s - 2; }
             } else {
                 const int dep = (t.type == T_G) ? t.s - bp.gbufs : t.s - 1;
-                if (dep >= 0 && on(T_DX) && on(T_DW)) wait_for(bp.c_done + dep, CG * (sc.nDX(dep) + sc.nDW(dep)));
-                if (DENSE && t.type == T_G && on(T_Q)) wait_for(bp.q_done + t.s, CG * sc.nG(t.s));
+                if (dep > c_ready && on(T_DX) && on(T_DW)) { wait_for(bp.c_done + dep, CG * (sc.nDX(dep) + sc.nDW(dep))); c_ready = dep; }
+                if (DENSE && t.type == T_G && on(T_Q) && t.s != q_ready) { wait_for(bp.q_done + t.s, CG * t.ng); q_ready = t.s; }
             }
             if (DENSE && t.type == T_Q) {
                 gp.b_off = t.vb0; gp.N = t.Vb_eff;

@@ -146,19 +146,19 @@ struct Pipe {
 // in shared memory.  Items are claimed in list order, so everything an item depends on has been claimed by a CTA that is
 // already running: the kernel makes progress with any number of resident CTAs (no co-residency requirement).
 // The claimer runs in CTA rank CG - 1 (its copy of the `sempty` barriers is the live one); it runs up to SCHED_Q tickets
-// ahead of the slowest reader.
+// ahead of the slowest reader.  Only items the launch really runs are published (the claimer drops disabled tile types),
+// so a reader that fetches its next tile in the middle of the current one never needs more than one queue slot ahead.
+__device__ __forceinline__ uint32_t ticket_take(int* counter) { return static_cast<uint32_t>(atomicAdd(counter, 1)); }
 template <int CG, int ST>
-__device__ __forceinline__ uint32_t ticket_claim(const Pipe<CG, ST>& P, int* counter, int n) {
+__device__ __forceinline__ void ticket_publish(const Pipe<CG, ST>& P, int n, uint32_t t) {
     const int q = n % SCHED_Q;
     mbar_wait_cluster(&P.sempty_bar[q], ((n / SCHED_Q) & 1) ^ 1);
-    const uint32_t t = static_cast<uint32_t>(atomicAdd(counter, 1));
     P.sticket[q] = t;
     if constexpr (CG == 2) {
         st_shared_cluster_u32(mapa_rank(smem_u32(&P.sticket[q]), 0), t);
         mbar_arrive_cluster(mapa_rank(smem_u32(&P.sfull_bar[q]), 0));
     }
     mbar_arrive(&P.sfull_bar[q]);
-    return t;
 }
 // called by one lane of a reader; every reader consumes every ticket exactly once, in order
 template <int CG, int ST>
@@ -184,12 +184,19 @@ struct TileOp {
 };
 
 // TMA producer (one elected lane): stream all k-blocks of all segments of `t` through the ring.
-template <int CG, int ST>
-__device__ __forceinline__ void produce_tile(const Pipe<CG, ST>& P, const TileOp& t, int& it) {
+struct NoMid { __device__ __forceinline__ void operator()() const {} };
+
+// `mid` runs once, after the loads of the tile's second k-block have been issued (after the last one for shorter tiles): the
+// persistent kernels fetch and decode their NEXT tile there, while the ring still holds work for the tensor pipe.
+template <int CG, int ST, class Mid = NoMid>
+__device__ __forceinline__ void produce_tile(const Pipe<CG, ST>& P, const TileOp& t, int& it, Mid&& mid = Mid{}) {
     using C = Cfg<CG, ST>;
     const int kblocks = (t.K + BK - 1) / BK;
+    const int mid_at = min(2, kblocks * t.nseg);
+    int issued = 0;
     for (int seg = 0; seg < t.nseg; ++seg) {
         for (int kb_i = 0; kb_i < kblocks; ++kb_i, ++it) {
+            if (issued++ == mid_at) mid();
             const int s = it % C::STAGES;
             const uint32_t ph = (it / C::STAGES) & 1;
             mbar_wait(&P.empty_bar[s], ph ^ 1);
@@ -228,11 +235,12 @@ __device__ __forceinline__ void produce_tile(const Pipe<CG, ST>& P, const TileOp
             }
         }
     }
+    if (issued <= mid_at) mid();
 }
 
 // MMA issuer (one elected lane of the CTA / of the pair leader): all MMAs of one tile into accumulator stage lt & 1.
-template <int CG, int ST>
-__device__ __forceinline__ void mma_tile(const Pipe<CG, ST>& P, int a_mn, int b_mn, int kiters, int lt, int& it) {
+template <int CG, int ST, class Mid = NoMid>
+__device__ __forceinline__ void mma_tile(const Pipe<CG, ST>& P, int a_mn, int b_mn, int kiters, int lt, int& it, Mid&& mid = Mid{}) {
     using C = Cfg<CG, ST>;
     const uint32_t idesc = make_idesc_bf16(C::TILE_M, BN, a_mn, b_mn);
     const uint32_t a_kstep = a_mn ? (UMMA_K * MN_BOX * 2) : (UMMA_K * 2);   // bytes per UMMA_K step
@@ -244,7 +252,9 @@ __device__ __forceinline__ void mma_tile(const Pipe<CG, ST>& P, int a_mn, int b_
     mbar_wait(&P.tempty_bar[as], aph ^ 1);
     tc_fence_after();
     const uint32_t tacc = P.tmem_base + as * BN;
+    const int mid_at = min(2, kiters - 1);
     for (int ki = 0; ki < kiters; ++ki, ++it) {
+        if (ki == mid_at) mid();                   // MMAs of the first k-blocks are queued: time to decode the next tile
         const int s = it % C::STAGES;
         const uint32_t ph = (it / C::STAGES) & 1;
         mbar_wait(&P.full_bar[s], ph);
