@@ -68,7 +68,8 @@ struct BwdSched {
     struct Super { int s, ti, vi, tb_eff, vb_eff, mt, nt, ng, ndx, ndw; };
     int S, nvb, Tb, Vb, V, d, wl, n_live, dm, dn;
     int order;      // tile order knobs (result-neutral): bit 0 grad_W tiles before grad_hidden tiles inside a block,
-                    // bits 1-3: n-fastest raster of the G / grad_hidden / grad_W tiles (default m fastest)
+                    // bits 1-3: n-fastest raster of the G / grad_hidden / grad_W tiles (default m fastest),
+                    // bit 4: G tiles of a block split around its DX / DW tiles (default: all G tiles first)
     int blk;        // current block
     long base;      // items before the current block
     int sz;         // items of the current block
@@ -116,13 +117,17 @@ struct BwdSched {
         if (blk > S + GOFF) return false;
         int r = static_cast<int>(item - base);
         const Super* u;
+        // order bit 4 (experiment, measured neutral at C4 and 6-7% slower at C2 / C3, profiles/r02_experiments.md): the G tiles
+        // of a block split around its DX / DW tiles, [G first half, DX, DW, G second half], so that half a super-tile of G
+        // tiles lies between any tile and the tiles it waits for at the block boundaries
+        const int gh = (!DENSE && (order & 16)) ? (g.ng + 1) / 2 : g.ng;
         if (DENSE && r < q.ng) { t.type = T_Q; u = &q; }
-        else if ((r -= q.ng) < g.ng) { t.type = T_G; u = &g; }
-        else {
-            r -= g.ng; u = &c;
+        else if ((r -= q.ng) < gh) { t.type = T_G; u = &g; }
+        else if (r - gh < c.ndx + c.ndw) {
+            r -= gh; u = &c;
             if (order & 1) { if (r < c.ndw) t.type = T_DW; else { t.type = T_DX; r -= c.ndw; } }
             else { if (r < c.ndx) t.type = T_DX; else { t.type = T_DW; r -= c.ndx; } }
-        }
+        } else { r -= c.ndx + c.ndw; t.type = T_G; u = &g; }
         t.s = u->s; t.vi = u->vi; t.Tb_eff = u->tb_eff; t.Vb_eff = u->vb_eff; t.ng = u->ng;
         t.tb0 = u->ti * Tb; t.vb0 = u->vi * Vb;
         const int rows = t.type == T_DW ? (wl == 0 ? dm : (u->vb_eff + TM - 1) / TM) : u->mt;

@@ -125,7 +125,8 @@ inline int cta_group_setting() {
     return cg == 1 ? 1 : 2;
 }
 
-inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int mode = 1) {
+// vb / gbufs: vocabulary columns per super-tile and depth of the G ring (chosen by make_plan)
+inline Plan make_plan_cfg(int T, int d, int V, int C, int fp32, unsigned flags, int mode, int vb, int gbufs) {
     Plan p{};
     p.T = T; p.d = d; p.V = V; p.C = C; p.planes = fp32 ? 3 : 1;
     const int TM = BM * cta_group_setting();              // tile rows of the GEMM core (CTA or CTA pair)
@@ -145,10 +146,6 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int 
             if (best_waste < 0 || waste < best_waste) { best_waste = waste; tb = cand; }
         }
     }
-    // Vocabulary columns per super-tile = K depth of a grad_hidden tile: 8192 for large batches (half as many fp32 partial-sum
-    // passes: DRAM writes 50 -> 40 GB per C4 launch, tensor pipe 86 -> 89.5% busy under ncu, profiles/r02_supertile_sweep.md),
-    // 4096 otherwise (keeps the G ring, and with it the workspace, below 5% of the logits for small T)
-    const int vb = env_int("OPD_VB", p.t_pad >= 32768 ? 8192 : 4096);
     p.Tb = std::min(p.t_pad, std::max(TM, tb / TM * TM));
     p.Vb = std::min(p.num_n * BN, std::max(BN, vb / BN * BN));
     p.est_blocks = ceil_div(T, 128);
@@ -183,7 +180,7 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int 
     p.off_seq_l1 = take(sizeof(float) * (size_t)p.t_pad);                               // per-token terms of opd_set_seq_diagnostics
     p.off_seq_var1 = take(sizeof(float) * (size_t)p.t_pad);
     p.gs_plane = (size_t)p.Tb * p.Vb;
-    p.gs_bufs = std::min(3, std::max(2, env_int("OPD_G_BUFS", 2)));
+    p.gs_bufs = std::min(3, std::max(2, gbufs));
     p.n_super = ceil_div(p.t_pad, p.Tb) * ceil_div(V, p.Vb);
     p.off_counters = take(bwd ? sizeof(int) * (2 * (size_t)p.n_super + 1) : 0);      // g_done, c_done, tile ticket
     // The per-tile LSE partials are dead once the estimators have run, the G ring and the grad_hidden partial
@@ -198,6 +195,32 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int 
     p.off_block_sums = take(sizeof(double) * (size_t)p.est_blocks);
     p.total = o;
     return p;
+}
+
+// Chooses the super-tile width Vb (= K depth of a grad_hidden tile) and the depth of the G ring under a workspace budget of
+// 4.8% of the bf16 logits (no buffer of the order of T x V), from the sweeps of profiles/r02_experiments.md:
+//   T >= 32768: the widest of 16384 / 12288 / 8192 / 4096 columns that fits, two G buffers (wider = fewer fp32 partial-sum passes:
+//               C4 8192 columns, 2.5% faster than 4096; C5 16384 columns, 2.6% faster than 8192);
+//   smaller T:  4096 columns and THREE G buffers (no wait at the block boundaries: C3 +2%, C2 +4%) if that fits, else
+//               2048 columns x 3 buffers for tiny problems, else 4096 x 2.
+// OPD_VB / OPD_G_BUFS override the choice (tuning, tests).
+inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int mode = 1) {
+    const int vb_env = env_int("OPD_VB", 0), gb_env = env_int("OPD_G_BUFS", 0);
+    auto plan = [&](int vb, int gb) { return make_plan_cfg(T, d, V, C, fp32, flags, mode, vb_env > 0 ? vb_env : vb, gb_env > 0 ? gb_env : gb); };
+    const double logits = 2.0 * (double)T * (double)V;
+    const double budget = 0.048 * logits;
+    const int t_pad = ceil_div(T, BM * cta_group_setting()) * BM * cta_group_setting();
+    if (t_pad >= 32768) {
+        for (int vb : {16384, 12288, 8192}) {
+            const Plan p = plan(vb, 2);
+            if ((double)p.total <= budget) return p;
+        }
+        return plan(4096, 2);
+    }
+    const Plan p3 = plan(4096, 3);
+    if ((double)p3.total <= budget) return p3;
+    if (logits < 1e9) return plan(2048, 3);
+    return plan(4096, 2);
 }
 
 // ---------------------------------------------------------------- GEMM launcher

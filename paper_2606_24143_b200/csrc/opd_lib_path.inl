@@ -281,7 +281,7 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         bp.d = d; bp.V = V; bp.Tb = p.Tb; bp.Vb = p.Vb; bp.nvb = ceil_div(V, p.Vb); bp.wl = wl; bp.planes = p.planes; bp.gbufs = p.gs_bufs;
         bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super; bp.ticket = counters + 2 * p.n_super;
         bp.dw_store_first = gw_accum ? 0 : 1;
-        bp.order = env_int("OPD_BWD_ORDER", 0) & 15;
+        bp.order = env_int("OPD_BWD_ORDER", 0) & 31;
         bp.g = GEpi::Params{gs, p.Tb, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V, 0ull};
         { const int gh_ = env_int("OPD_HINT_GST", 0); bp.g.st_hint = gh_ ? hint_policy(gh_) : 0ull; }
         bp.dx = dxp;
