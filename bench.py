@@ -30,7 +30,7 @@ UNIT = "live tokens/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from one committed `ncu --set full` capture of this
 # workload (a citation: bench.py never runs under a profiler, so the line carries "traffic_measured": false)
 NCU_TRAFFIC = {
-    "C4": dict(bwd_kernel=150_634_613_000, fwd_kernel=20_625_665_000, source="profiles/r02_final_c4.md"),
+    "C4": dict(bwd_kernel=151_675_632_000, fwd_kernel=10_745_648_000, source="profiles/r02_final_c4.md"),
 }
 
 
