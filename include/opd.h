@@ -156,14 +156,15 @@ opd_status_t opd_loss_fwd_bwd_host_wait(opd_handle_t h, int slot, size_t* h2d_by
 
 /* cache producers -------------------------------------------------------------------------------
  * The steps either side of the learner path that build the finite caches it consumes, on the same
- * streamed contraction (the logits are never stored).  hidden / W / dtype / strides as for opd_loss_fwd_bwd; every row
- * is scored (no mask).  Outputs are device arrays with row strides ld_idx / ld_logp (>= k resp. K); lse_out [T] may be NULL.
+ * streamed contraction (the logits are never stored).  hidden / W / dtype / strides as for opd_loss_fwd_bwd.  mask [T] bytes
+ * (may be NULL = every row): rows with mask 0 (padding) are not scored and their rows of the outputs are not written.
+ * Outputs are device arrays with row strides ld_idx / ld_logp (>= k resp. K); lse_out [T] may be NULL.
  *
  * opd_cache_topk    S_t = TopK(softmax(hidden_t . W), k), the support the scoring model selects:
  *                   idx_out [T,k] in descending order of probability (ties: lowest index first),
  *                   logp_out [T,k] the full-vocabulary-normalised log-probs on it.  1 <= k <= min(64, V).
- *                   Synchronises the stream at the end (OPD_ERR_WORKSPACE if more than max(4k,256) logits of a row tie at
- *                   its selection threshold).
+ *                   Synchronises the stream at the end (OPD_ERR_WORKSPACE if more than max(4k,256) logits of a scored row
+ *                   tie at its selection threshold, e.g. an all-zero padding row that was not masked).
  * opd_cache_sample  K draws per row from softmax(hidden_t . W), iid WITH replacement, by inverse-CDF
  *                   from the caller's uniforms u_tj in [0,1) (uniforms [T,K], row stride ld_u): a_tj is the first index v
  *                   whose cumulative probability sum_{v'<=v} p(v') reaches u_tj (cumulated in vocabulary order, fp32);
@@ -171,11 +172,11 @@ opd_status_t opd_loss_fwd_bwd_host_wait(opd_handle_t h, int slot, size_t* h2d_by
  * opd_cache_workspace_bytes  device scratch either call needs (pass 0 for the one not used). */
 size_t opd_cache_workspace_bytes(int T, int d, int V, opd_dtype_t dtype, int k_top, int K_samples);
 opd_status_t opd_cache_topk(opd_handle_t h, void* cuda_stream, int T, int d, int V, opd_dtype_t dtype,
-    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, int k,
+    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, const unsigned char* mask, int k,
     int* idx_out, long ld_idx, float* logp_out, long ld_logp, float* lse_out);
 opd_status_t opd_cache_sample(opd_handle_t h, void* cuda_stream, int T, int d, int V, opd_dtype_t dtype,
-    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, int K, const float* uniforms, long ld_u,
-    int* idx_out, long ld_idx, float* logp_out, long ld_logp, float* lse_out);
+    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, const unsigned char* mask, int K,
+    const float* uniforms, long ld_u, int* idx_out, long ld_idx, float* logp_out, long ld_logp, float* lse_out);
 
 /* dense two-head KL -------------------------------------------------------------------------------
  * Dense full-vocabulary forward KL with the teacher's distribution recomputed from TRANSMITTED TEACHER HIDDEN STATES

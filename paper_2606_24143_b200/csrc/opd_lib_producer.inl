@@ -49,7 +49,7 @@ extern "C" size_t opd_cache_workspace_bytes(int T, int d, int V, opd_dtype_t dty
 
 // which = 0: top-k (n = k), which = 1: samples (n = K, u = uniforms)
 static opd_status_t run_producer(opd_handle_s* h, cudaStream_t st, int which, int T, int d, int V, opd_dtype_t dtype,
-                                 const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, int n,
+                                 const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, const unsigned char* mask, int n,
                                  const float* u, long ld_u, int* idx_out, long ld_idx, float* logp_out, long ld_logp, float* lse_out) {
     if (!h->arch_ok) OPD_FAIL(h, OPD_ERR_ARCH, "device %d is not compute capability 10.x (sm_100a required, no fallback)", h->device);
     if (dtype != OPD_BF16 && dtype != OPD_FP32) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unknown dtype %d", (int)dtype);
@@ -91,9 +91,9 @@ static opd_status_t run_producer(opd_handle_s* h, cudaStream_t st, int which, in
     float* tgt_res = reinterpret_cast<float*>(ws + p.off_res);
     unsigned char* perm = ws + p.off_perm;
 
-    // operand staging: every row is live (the producers score whole batches)
+    // operand staging: rows with mask == 0 are not scored (mask == NULL: every row is)
     OPD_CUDA(h, cudaMemsetAsync(overflow, 0, 4, st));
-    k_compact<<<1, 1024, 0, st>>>(nullptr, T, 1, live_rows, n_live);
+    k_compact<<<1, 1024, 0, st>>>(mask, T, mask ? 0 : 1, live_rows, n_live);
     k_gather_rows<<<p.t_pad, 256, 0, st>>>(hidden, ld_hidden, fp32 ? 1 : 0, d, p.t_pad, live_rows, n_live, xc, (long)p.xc_plane);
     h->n_kernels += 2;
     const __nv_bfloat16* wq = static_cast<const __nv_bfloat16*>(W);
@@ -130,15 +130,15 @@ static opd_status_t run_producer(opd_handle_s* h, cudaStream_t st, int which, in
         OPD_CUDA(h, cudaMemsetAsync(count, 0, sizeof(int) * (size_t)T, st));
         CollectEpi::Params ep{theta, count, cand, p.cap, V};
         OPD_CUDA(h, launch_gemm<CollectEpi>(h, st, m_xc_k, m_w_fwd, gp, ep));
-        k_topk_select<<<ceil_div(T, 8), 256, 0, st>>>(cand, count, p.cap, T, n, lse, idx_out, ld_idx, logp_out, ld_logp, overflow);
+        k_topk_select<<<ceil_div(T, 8), 256, 0, st>>>(cand, count, p.cap, T, n, lse, live_rows, n_live, idx_out, ld_idx, logp_out, ld_logp, overflow);
         h->n_kernels++;
     } else {
-        k_sample_targets<<<ceil_div(T, 128), 128, 0, st>>>(partials, p.num_n, p.t_pad, T, n, lse, u, ld_u, tgt_tile, tgt_res, perm);
-        SampleEpi::Params ep{tgt_tile, tgt_res, perm, lse, n, V, idx_out, ld_idx, logp_out, ld_logp};
+        k_sample_targets<<<ceil_div(T, 128), 128, 0, st>>>(partials, p.num_n, p.t_pad, T, n, lse, live_rows, n_live, u, ld_u, tgt_tile, tgt_res, perm);
+        SampleEpi::Params ep{tgt_tile, tgt_res, perm, lse, n, V, idx_out, ld_idx, logp_out, ld_logp, live_rows};
         OPD_CUDA(h, launch_gemm<SampleEpi>(h, st, m_xc_k, m_w_fwd, gp, ep));
         h->n_kernels++;
     }
-    if (lse_out) OPD_CUDA(h, cudaMemcpyAsync(lse_out, lse, sizeof(float) * (size_t)T, cudaMemcpyDeviceToDevice, st));
+    if (lse_out) { k_scatter_rows_f32<<<ceil_div(T, 256), 256, 0, st>>>(lse, live_rows, n_live, T, lse_out); h->n_kernels++; }
     OPD_CUDA(h, cudaGetLastError());
     if (which == 0) {   // candidate-list overflow (more than `cap` logits tie at / exceed the threshold) is an error, not a silent truncation
         int ov = 0;
@@ -151,17 +151,17 @@ static opd_status_t run_producer(opd_handle_s* h, cudaStream_t st, int which, in
 }
 
 extern "C" opd_status_t opd_cache_topk(opd_handle_t h, void* cuda_stream, int T, int d, int V, opd_dtype_t dtype,
-    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, int k,
+    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, const unsigned char* mask, int k,
     int* idx_out, long ld_idx, float* logp_out, long ld_logp, float* lse_out) {
     if (!h) return OPD_ERR_BAD_ARG;
-    return run_producer(h, static_cast<cudaStream_t>(cuda_stream), 0, T, d, V, dtype, hidden, ld_hidden, W, ldw_k, ldw_v, k,
+    return run_producer(h, static_cast<cudaStream_t>(cuda_stream), 0, T, d, V, dtype, hidden, ld_hidden, W, ldw_k, ldw_v, mask, k,
                         nullptr, 0, idx_out, ld_idx, logp_out, ld_logp, lse_out);
 }
 
 extern "C" opd_status_t opd_cache_sample(opd_handle_t h, void* cuda_stream, int T, int d, int V, opd_dtype_t dtype,
-    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, int K, const float* uniforms, long ld_u,
-    int* idx_out, long ld_idx, float* logp_out, long ld_logp, float* lse_out) {
+    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, const unsigned char* mask, int K,
+    const float* uniforms, long ld_u, int* idx_out, long ld_idx, float* logp_out, long ld_logp, float* lse_out) {
     if (!h) return OPD_ERR_BAD_ARG;
-    return run_producer(h, static_cast<cudaStream_t>(cuda_stream), 1, T, d, V, dtype, hidden, ld_hidden, W, ldw_k, ldw_v, K,
+    return run_producer(h, static_cast<cudaStream_t>(cuda_stream), 1, T, d, V, dtype, hidden, ld_hidden, W, ldw_k, ldw_v, mask, K,
                         uniforms, ld_u, idx_out, ld_idx, logp_out, ld_logp, lse_out);
 }

@@ -54,6 +54,13 @@ __global__ void __launch_bounds__(256) k_lse_theta(const float2* __restrict__ pa
     if (lane == 0) theta[row] = pv;
 }
 
+// out[live_rows[i]] = in[i] for the live compact rows (lse_out in the caller's row order)
+__global__ void __launch_bounds__(256) k_scatter_rows_f32(const float* __restrict__ in, const int* __restrict__ live_rows,
+                                                          const int* __restrict__ n_live, int T, float* __restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < T && i < *n_live) out[live_rows[i]] = in[i];
+}
+
 // ------------------------------------------------------------------------------------------ CollectEpi (top-k pass B)
 struct CollectEpi {
     struct Params {
@@ -101,11 +108,13 @@ struct CollectEpi {
 // Rank the candidates of each row: the k largest logits, ties -> lowest column first (the order a stable descending
 // sort gives), written in descending order with their log-probs.  One warp per row.
 __global__ void __launch_bounds__(256) k_topk_select(const float2* __restrict__ cand, const int* __restrict__ count, int cap, int T, int k,
-                                                     const float* __restrict__ lse, int* __restrict__ idx_out, long ld_idx,
+                                                     const float* __restrict__ lse, const int* __restrict__ live_rows, const int* __restrict__ n_live,
+                                                     int* __restrict__ idx_out, long ld_idx,
                                                      float* __restrict__ logp_out, long ld_logp, int* __restrict__ overflow) {
     const int lane = threadIdx.x & 31;
-    const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (row >= T) return;
+    const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);      // compact row
+    if (row >= T || row >= *n_live) return;
+    const int tok = live_rows[row];                                            // its row in the caller's arrays
     int n = count[row];
     if (n > cap) { if (lane == 0) atomicMax(overflow, n); n = cap; }
     const float2* c = cand + static_cast<size_t>(row) * cap;
@@ -119,13 +128,13 @@ __global__ void __launch_bounds__(256) k_topk_select(const float2* __restrict__ 
             rank += (vj > vi) || (vj == vi && __float_as_int(c[j].y) < ci);
         }
         if (rank < k) {
-            idx_out[static_cast<size_t>(row) * ld_idx + rank] = ci;
-            logp_out[static_cast<size_t>(row) * ld_logp + rank] = vi - l;
+            idx_out[static_cast<size_t>(tok) * ld_idx + rank] = ci;
+            logp_out[static_cast<size_t>(tok) * ld_logp + rank] = vi - l;
         }
     }
     for (int r = n + lane; r < k; r += 32) {      // fewer than k candidates (only if V < k)
-        idx_out[static_cast<size_t>(row) * ld_idx + r] = -1;
-        logp_out[static_cast<size_t>(row) * ld_logp + r] = -INFINITY;
+        idx_out[static_cast<size_t>(tok) * ld_idx + r] = -1;
+        logp_out[static_cast<size_t>(tok) * ld_logp + r] = -INFINITY;
     }
 }
 
@@ -135,12 +144,13 @@ __global__ void __launch_bounds__(256) k_topk_select(const float2* __restrict__ 
 //   draw with target c = u * (sum_n m_n) lies in the first tile n with cum_n >= c;  residual = c - cum_{n-1}.
 // One thread per row (K <= 64, num_n tiles).
 __global__ void __launch_bounds__(128) k_sample_targets(const float2* __restrict__ partials, int num_n, int t_pad, int T, int K,
-                                                        const float* __restrict__ lse, const float* __restrict__ u, long ld_u,
+                                                        const float* __restrict__ lse, const int* __restrict__ live_rows,
+                                                        const int* __restrict__ n_live, const float* __restrict__ u, long ld_u,
                                                         int* __restrict__ tgt_tile, float* __restrict__ tgt_res,
                                                         unsigned char* __restrict__ perm) {
-    const int row = blockIdx.x * blockDim.x + threadIdx.x;
-    if (row >= T) return;
-    const float* ur = u + static_cast<size_t>(row) * ld_u;
+    const int row = blockIdx.x * blockDim.x + threadIdx.x;                    // compact row
+    if (row >= T || row >= *n_live) return;
+    const float* ur = u + static_cast<size_t>(live_rows[row]) * ld_u;         // the uniforms are in the caller's row order
     int* tt = tgt_tile + static_cast<size_t>(row) * K;
     float* tr = tgt_res + static_cast<size_t>(row) * K;
     unsigned char* pr = perm + static_cast<size_t>(row) * K;
@@ -185,14 +195,16 @@ struct SampleEpi {
         int V;
         int* idx_out; long ld_idx;
         float* logp_out; long ld_logp;
+        const int* live_rows;    // compact row -> row of the caller's arrays
     };
-    struct State { int cursor; float lse; };
+    struct State { int cursor; float lse; int tok; };
     static __device__ __forceinline__ State prepare(const Params& p, const GemmParams&, int m_blk, int n_blk, int row_in_tile, int M_eff) {
-        State st{p.K, 0.f};
+        State st{p.K, 0.f, 0};
         const int row = m_blk * BM + row_in_tile;
         if (row < M_eff) {
             st.cursor = lower_bound_slot(p.tgt_tile + static_cast<size_t>(row) * p.K, p.K, n_blk);
             st.lse = p.lse[row];
+            st.tok = p.live_rows[row];
         }
         return st;
     }
@@ -229,8 +241,8 @@ struct SampleEpi {
                 for (int i = 31; i >= 0; --i) pos = (cum + pre[i] >= res) ? i : pos;
                 pos = min(pos, nv - 1);
                 const float z = select32(v, pos);
-                p.idx_out[static_cast<size_t>(row) * p.ld_idx + pr[st.cursor]] = col0 + pos;
-                p.logp_out[static_cast<size_t>(row) * p.ld_logp + pr[st.cursor]] = z - st.lse;
+                p.idx_out[static_cast<size_t>(st.tok) * p.ld_idx + pr[st.cursor]] = col0 + pos;
+                p.logp_out[static_cast<size_t>(st.tok) * p.ld_logp + pr[st.cursor]] = z - st.lse;
                 ++st.cursor;
                 mine = st.cursor < p.K && tt[st.cursor] == n_blk;
                 res = mine ? tr[st.cursor] : 0.f;
@@ -239,8 +251,8 @@ struct SampleEpi {
             last_col = col0 + nv - 1; last_z = select32(v, nv - 1);
         }
         while (mine) {                                                 // rounding: residual beyond the tile's mass
-            p.idx_out[static_cast<size_t>(row) * p.ld_idx + pr[st.cursor]] = last_col;
-            p.logp_out[static_cast<size_t>(row) * p.ld_logp + pr[st.cursor]] = last_z - st.lse;
+            p.idx_out[static_cast<size_t>(st.tok) * p.ld_idx + pr[st.cursor]] = last_col;
+            p.logp_out[static_cast<size_t>(st.tok) * p.ld_logp + pr[st.cursor]] = last_z - st.lse;
             ++st.cursor;
             mine = st.cursor < p.K && tt[st.cursor] == n_blk;
         }

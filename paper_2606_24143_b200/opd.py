@@ -79,10 +79,10 @@ def load_library():
     lib.opd_last_launch_stats.restype = c_int
     lib.opd_cache_workspace_bytes.argtypes = [c_int, c_int, c_int, c_int, c_int, c_int]
     lib.opd_cache_workspace_bytes.restype = c_size_t
-    lib.opd_cache_topk.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_long, c_void_p, c_long, c_long, c_int,
+    lib.opd_cache_topk.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_long, c_void_p, c_long, c_long, c_void_p, c_int,
                                    c_void_p, c_long, c_void_p, c_long, c_void_p]
     lib.opd_cache_topk.restype = c_int
-    lib.opd_cache_sample.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_long, c_void_p, c_long, c_long, c_int,
+    lib.opd_cache_sample.argtypes = [c_void_p, c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_long, c_void_p, c_long, c_long, c_void_p, c_int,
                                      c_void_p, c_long, c_void_p, c_long, c_void_p, c_long, c_void_p]
     lib.opd_cache_sample.restype = c_int
     lib.opd_dense_kl_workspace_bytes.argtypes = [c_int, c_int, c_int, c_int, c_int, c_uint]
@@ -366,34 +366,53 @@ class Handle:
         return out, up.value, down.value
 
     # ------------------------------------------------------------------ cache producers
-    def cache_topk(self, hidden, W, k):
-        """opd_cache_topk -> (idx [T,k] int32, logp [T,k] float32, lse [T] float32): the scoring model's top-k support."""
+    @staticmethod
+    def _producer_args(hidden, W, mask):
+        if hidden.dim() != 2 or not hidden.is_cuda or hidden.stride(1) != 1:
+            raise OpdError(ERR_BAD_ARG, "hidden must be a [T,d] CUDA tensor with a unit inner stride")
+        if W.dtype != hidden.dtype or W.device != hidden.device:
+            raise OpdError(ERR_BAD_ARG, "hidden and W must have the same dtype and device")
+        if mask is not None:
+            if mask.dtype == torch.bool:
+                mask = mask.view(torch.uint8)
+            if mask.dtype != torch.uint8 or mask.dim() != 1 or mask.shape[0] != hidden.shape[0] or mask.device != hidden.device:
+                raise OpdError(ERR_BAD_ARG, "mask must be a [T] uint8 / bool tensor on hidden's device")
+            mask = mask.contiguous()
+        return mask
+
+    def cache_topk(self, hidden, W, k, mask=None):
+        """opd_cache_topk -> (idx [T,k] int32, logp [T,k] float32, lse [T] float32): the scoring model's top-k support.
+        Rows with mask == 0 are not scored (idx -1, logp -inf, lse 0 there)."""
+        mask = self._producer_args(hidden, W, mask)
         T, d = hidden.shape
         V = W.shape[1]
         ldk, ldv = _w_strides(W, d)
         dev = hidden.device
-        idx = torch.empty(T, k, dtype=torch.int32, device=dev)
-        logp = torch.empty(T, k, dtype=torch.float32, device=dev)
-        lse = torch.empty(T, dtype=torch.float32, device=dev)
+        idx = torch.full((T, k), -1, dtype=torch.int32, device=dev)
+        logp = torch.full((T, k), float("-inf"), dtype=torch.float32, device=dev)
+        lse = torch.zeros(T, dtype=torch.float32, device=dev)
         s = torch.cuda.current_stream(dev).cuda_stream
         self._check(self.lib.opd_cache_topk(self._h, c_void_p(s), T, d, V, _dtype_code(hidden), _ptr(hidden), hidden.stride(0), _ptr(W),
-                                            ldk, ldv, k, _ptr(idx), k, _ptr(logp), k, _ptr(lse)))
+                                            ldk, ldv, _ptr(mask), k, _ptr(idx), k, _ptr(logp), k, _ptr(lse)))
         return idx, logp, lse
 
-    def cache_sample(self, hidden, W, uniforms):
+    def cache_sample(self, hidden, W, uniforms, mask=None):
         """opd_cache_sample -> (idx [T,K] int32, logp [T,K] float32, lse [T]): K inverse-CDF draws per row from
-        softmax(hidden . W) for the uniforms [T,K] (float32, in [0,1))."""
+        softmax(hidden . W) for the uniforms [T,K] (float32, in [0,1)). Rows with mask == 0 are not scored."""
+        mask = self._producer_args(hidden, W, mask)
         T, d = hidden.shape
         V = W.shape[1]
+        if uniforms.dtype != torch.float32 or tuple(uniforms.shape[:1]) != (T,) or uniforms.stride(1) != 1 or uniforms.device != hidden.device:
+            raise OpdError(ERR_BAD_ARG, "uniforms must be a [T,K] float32 tensor on hidden's device with a unit inner stride")
         K = uniforms.shape[1]
         ldk, ldv = _w_strides(W, d)
         dev = hidden.device
-        idx = torch.empty(T, K, dtype=torch.int32, device=dev)
-        logp = torch.empty(T, K, dtype=torch.float32, device=dev)
-        lse = torch.empty(T, dtype=torch.float32, device=dev)
+        idx = torch.full((T, K), -1, dtype=torch.int32, device=dev)
+        logp = torch.full((T, K), float("-inf"), dtype=torch.float32, device=dev)
+        lse = torch.zeros(T, dtype=torch.float32, device=dev)
         s = torch.cuda.current_stream(dev).cuda_stream
         self._check(self.lib.opd_cache_sample(self._h, c_void_p(s), T, d, V, _dtype_code(hidden), _ptr(hidden), hidden.stride(0), _ptr(W),
-                                              ldk, ldv, K, _ptr(uniforms), uniforms.stride(0), _ptr(idx), K, _ptr(logp), K, _ptr(lse)))
+                                              ldk, ldv, _ptr(mask), K, _ptr(uniforms), uniforms.stride(0), _ptr(idx), K, _ptr(logp), K, _ptr(lse)))
         return idx, logp, lse
 
     # ------------------------------------------------------------------ dense two-head KL

@@ -143,3 +143,33 @@ def test_cache_sample_frequencies_and_learner_roundtrip(handle):
     finally:
         handle.set_diagnostics(None, None)
     assert (rho - 1).abs().max().item() <= 2e-4
+
+
+def test_producers_skip_masked_rows(handle):
+    """mask argument of the producers: padding rows (all-zero hidden states: all V logits tie, which overflows the
+    candidate list of opd_cache_topk) are not scored when masked and fail the batch when they are not; the scored rows
+    give exactly what the unmasked call gives for them; rows with mask 0 are left unwritten."""
+    from paper_2606_24143_b200 import opd
+    T, d, V, k, K = 520, 256, 8200, 8, 6
+    X, W = inputs("bf16", T, d, V, 31)
+    base_idx, base_lp, base_lse = handle.cache_topk(X, W, k)
+    u = torch.rand(T, K, generator=torch.Generator(device=DEV).manual_seed(5), device=DEV)
+    sbase_idx, sbase_lp, _ = handle.cache_sample(X, W, u)
+    torch.cuda.synchronize()
+    mask = torch.ones(T, dtype=torch.uint8, device=DEV)
+    dead = torch.tensor([0, 7, 255, 256, 300, T - 1], device=DEV)
+    mask[dead] = 0
+    Xp = X.clone(); Xp[dead] = 0                        # padding rows
+    with pytest.raises(opd.OpdError) as e:
+        handle.cache_topk(Xp, W, k)
+    assert e.value.status == opd.ERR_WORKSPACE
+    idx, lp, lse = handle.cache_topk(Xp, W, k, mask=mask)
+    sidx, slp, slse = handle.cache_sample(Xp, W, u, mask=mask != 0)
+    torch.cuda.synchronize()
+    live = mask != 0
+    assert torch.equal(idx[live], base_idx[live]) and torch.equal(lp[live], base_lp[live]) and torch.equal(lse[live], base_lse[live])
+    assert torch.equal(sidx[live], sbase_idx[live]) and torch.equal(slp[live], sbase_lp[live]) and torch.equal(slse[live], base_lse[live])
+    assert (idx[dead] == -1).all() and torch.isinf(lp[dead]).all() and (lse[dead] == 0).all() and (sidx[dead] == -1).all()
+    none = handle.cache_topk(Xp, W, k, mask=torch.zeros_like(mask))
+    torch.cuda.synchronize()
+    assert (none[0] == -1).all()
