@@ -32,6 +32,7 @@ struct BwdParams {
     int* c_done;               // [S]
     int* ticket;               // [1] next unclaimed item of the tile list (zeroed by the host before the launch)
     int order;                 // BwdSched::order
+    int dx_group;              // BwdSched::dx_group
     int dw_store_first;        // 1: the grad_W tiles of the first token super-tile store instead of reduce-add (grad_W is
                                //    overwritten, not accumulated into: no memset and no read-modify-write for that pass)
     int type_mask;             // bit t set = run tiles of type t.  All types of the variant = the normal run; a tile waits
@@ -70,6 +71,7 @@ struct BwdSched {
     int order;      // tile order knobs (result-neutral): bit 0 grad_W tiles before grad_hidden tiles inside a block,
                     // bits 1-3: n-fastest raster of the G / grad_hidden / grad_W tiles (default m fastest),
                     // bit 4: G tiles of a block split around its DX / DW tiles (default: all G tiles first)
+    int dx_group;   // row tiles per raster group of the grad_hidden tiles (0: all rows of the super-tile)
     int blk;        // current block
     long base;      // items before the current block
     int sz;         // items of the current block
@@ -94,7 +96,7 @@ struct BwdSched {
     }
     __device__ __forceinline__ void init(const BwdParams& p) {
         n_live = *p.n_live;
-        nvb = p.nvb; Tb = p.Tb; Vb = p.Vb; V = p.V; d = p.d; wl = p.wl; order = p.order;
+        nvb = p.nvb; Tb = p.Tb; Vb = p.Vb; V = p.V; d = p.d; wl = p.wl; order = p.order; dx_group = p.dx_group;
         dm = (d + TM - 1) / TM; dn = (d + BN - 1) / BN;
         S = ((n_live + Tb - 1) / Tb) * nvb;
         blk = 0; base = 0;
@@ -135,6 +137,14 @@ struct BwdSched {
         if (order & tbit) {                          // n fastest: concurrently running CTAs share the A panel
             const int cols = t.type == T_DX ? dn : (t.type == T_DW ? (wl == 0 ? u->nt : dn) : u->nt);
             t.m_blk = r / cols; t.n_blk = r - t.m_blk * cols;
+        } else if (t.type == T_DX && dx_group > 0 && dx_group < rows) {
+            // grad_hidden tiles in groups of dx_group row tiles, m fastest inside a group: the G row panels of one group
+            // (dx_group x Vb x 512 bytes) stay in L2 while the W slices stream past, instead of all of G per wave
+            const int per_group = dx_group * dn;
+            const int gi = r / per_group;
+            const int rr = r - gi * per_group;
+            const int gm = min(dx_group, rows - gi * dx_group);
+            t.n_blk = rr / gm; t.m_blk = gi * dx_group + (rr - t.n_blk * gm);
         } else {                                     // m fastest: concurrently running CTAs share the B panel
             t.n_blk = r / rows; t.m_blk = r - t.n_blk * rows;
         }

@@ -183,6 +183,7 @@ extern "C" opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, 
     bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super; bp.q_done = q_done;
     bp.ticket = counters + 2 * p.n_super;
     bp.dw_store_first = (flags & OPD_F_GRADW_ACCUM) ? 0 : 1;
+    bp.dx_group = p.Vb > 4096 ? 8 : 0;
     bp.dx = dxp; bp.dw = dwp;
     bp.hint_x = bp.hint_w = bp.hint_g = L2_EVICT_NORMAL;
     bp.dT = dT; bp.wl_t = wlt; bp.qbytes = q32 ? 4 : 2; bp.q_buf_bytes = dp.q_buf_bytes;

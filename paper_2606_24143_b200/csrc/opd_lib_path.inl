@@ -282,6 +282,8 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super; bp.ticket = counters + 2 * p.n_super;
         bp.dw_store_first = gw_accum ? 0 : 1;
         bp.order = env_int("OPD_BWD_ORDER", 0) & 31;
+        // super-tiles wider than 4096 columns: grad_hidden tiles in groups of 8 row tiles (10 GB fewer G re-reads per C4 launch)
+        bp.dx_group = env_int("OPD_DX_GROUP", p.Vb > 4096 ? 8 : 0);
         bp.g = GEpi::Params{gs, p.Tb, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V, 0ull};
         { const int gh_ = env_int("OPD_HINT_GST", 0); bp.g.st_hint = gh_ ? hint_policy(gh_) : 0ull; }
         bp.dx = dxp;
