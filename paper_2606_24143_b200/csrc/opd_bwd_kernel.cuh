@@ -48,6 +48,9 @@ struct BwdParams {
     QEpi::Params q;            // qs points at Q ring buffer 0; buffer b at + b * q_buf_bytes
     size_t q_buf_bytes;
     GDenseEpi::Params gd;
+#ifdef OPD_TRACE
+    unsigned long long* trace; // [3 roles][4 tile types][8] cycle sums + [96..] per-CTA kernel cycles (tracing builds only)
+#endif
 };
 
 enum { T_G = 0, T_DX = 1, T_DW = 2, T_Q = 3 };
@@ -216,8 +219,16 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                     return sc.get(ticket_read<CG, ST>(P, n++), o);
                 }
             };
+#ifdef OPD_TRACE
+            long long trp[4][8] = {};
+            const long long k0 = clock64();
+#endif
             bool have = fetch(t), have_next = false;
             while (have) {
+#ifdef OPD_TRACE
+                long long* tr = trp[t.type];
+                const long long t0 = clock64();
+#endif
                 TileOp op;
                 int pa_off = 0, pb_off = 0;
                 const int buf = t.s % bp.gbufs;
@@ -249,13 +260,31 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                     op.pb[i] = static_cast<unsigned char>(pb_off + (nseg == 1 ? 0 : PB[i]));
                 }
                 if ((t.type == T_DX || t.type == T_DW) && on(T_G) && t.s != g_ready) {   // the G super-tile must be complete
+#ifdef OPD_TRACE
+                    const long long w0 = clock64();
+#endif
                     wait_counter(bp.g_done + t.s, CG * t.ng);                             // before TMA reads it (checked once
                     fence_proxy_async_all();                                              // per super-tile, not per tile)
                     g_ready = t.s;
+#ifdef OPD_TRACE
+                    tr[3] += clock64() - w0;
+#endif
                 }
+#ifdef OPD_TRACE
+                produce_tile<CG, ST>(P, op, it, [&] { have_next = fetch(nxt); }, tr);
+                tr[0] += 1; tr[1] += clock64() - t0;
+#else
                 produce_tile<CG, ST>(P, op, it, [&] { have_next = fetch(nxt); });
+#endif
                 t = nxt; have = have_next;
             }
+#ifdef OPD_TRACE
+            if (bp.trace) {
+                for (int ty = 0; ty < 4; ++ty) for (int k = 0; k < 8; ++k)
+                    if (trp[ty][k]) atomicAdd(bp.trace + (1 * 4 + ty) * 8 + k, (unsigned long long)trp[ty][k]);
+                atomicAdd(bp.trace + 96 + 1, (unsigned long long)(clock64() - k0));
+            }
+#endif
         }
     } else if (warp == 1) {
         // =========================== tile claimer (peer CTA of a pair; this warp has no other work there) =========
@@ -276,18 +305,38 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             BwdTile t, nxt;
             int it = 0, lt = 0, n = 0;
             auto fetch = [&](BwdTile& o) -> bool { return sc.get(ticket_read<CG, ST>(P, n++), o); };
+#ifdef OPD_TRACE
+            long long trm[4][8] = {};
+            const long long k0 = clock64();
+#endif
             bool have = fetch(t), have_next = false;
             while (have) {
+#ifdef OPD_TRACE
+                long long* tr = trm[t.type];
+                const long long t0 = clock64();
+#endif
                 int a_mn, b_mn, K;
                 if (t.type == T_G) { a_mn = 0; b_mn = (bp.wl == 0); K = bp.d; }
                 else if (DENSE && t.type == T_Q) { a_mn = 0; b_mn = (bp.wl_t == 0); K = bp.dT; }
                 else if (t.type == T_DX) { a_mn = 0; b_mn = (bp.wl == 1); K = t.Vb_eff; }
                 else { a_mn = 1; b_mn = 1; K = t.Tb_eff; }
                 // the next tile is fetched and decoded after this tile's first MMAs are queued, not between two tiles
+#ifdef OPD_TRACE
+                mma_tile<CG, ST>(P, a_mn, b_mn, ((K + BK - 1) / BK) * nseg, lt, it, [&] { have_next = fetch(nxt); }, tr);
+                tr[0] += 1; tr[1] += clock64() - t0; tr[6] += ((K + BK - 1) / BK) * nseg;
+#else
                 mma_tile<CG, ST>(P, a_mn, b_mn, ((K + BK - 1) / BK) * nseg, lt, it, [&] { have_next = fetch(nxt); });
+#endif
                 ++lt;
                 t = nxt; have = have_next;
             }
+#ifdef OPD_TRACE
+            if (bp.trace) {
+                for (int ty = 0; ty < 4; ++ty) for (int k = 0; k < 8; ++k)
+                    if (trm[ty][k]) atomicAdd(bp.trace + (0 * 4 + ty) * 8 + k, (unsigned long long)trm[ty][k]);
+                atomicAdd(bp.trace + 96 + 0, (unsigned long long)(clock64() - k0));
+            }
+#endif
         }
     } else {
         // =========================== epilogue warps ===========================
@@ -298,15 +347,43 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
         BwdTile t;
         int lt = 0;
         int c_ready = -1, gq_ready = -1, q_ready = -1;              // dependencies already seen complete (warp-uniform)
+#ifdef OPD_TRACE
+        long long tre[4][8] = {};
+        long long* tr = tre[0];
+        const long long k0 = clock64();
+#endif
         auto wait_for = [&](const int* counter, int expected) {      // warp-level acquire of a dependency counter
+#ifdef OPD_TRACE
+            const long long w0 = clock64();
+#endif
             if (lane == 0) { wait_counter(counter, expected); fence_proxy_async_all(); }
             __syncwarp();
+#ifdef OPD_TRACE
+            tr[2] += clock64() - w0;
+#endif
+        };
+        auto acquire = [&]() -> uint32_t {
+#ifdef OPD_TRACE
+            const long long w0 = clock64();
+            const uint32_t ta = epi_acquire<CG, ST>(P, lt, quarter);
+            tr[3] += clock64() - w0;
+            return ta;
+#else
+            return epi_acquire<CG, ST>(P, lt, quarter);
+#endif
         };
         for (int n = 0;; ++n) {
             uint32_t item = 0;
+#ifdef OPD_TRACE
+            const long long t0 = clock64();
+#endif
             if (lane == 0) item = ticket_read<CG, ST>(P, n);
             item = __shfl_sync(0xffffffffu, item, 0);
             if (!sc.get(item, t)) break;
+#ifdef OPD_TRACE
+            tr = tre[t.type];
+            tr[5] += clock64() - t0;          // ticket wait + decode
+#endif
             const int m_blk = t.m_blk * CG + rank;    // this CTA's 128-row block inside the GEMM
             GemmParams gp{};                      // the fields the epilogues read
             gp.tok_off = t.tb0;
@@ -324,7 +401,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 QEpi::Params ep = bp.q;
                 ep.qs = static_cast<uint8_t*>(ep.qs) + static_cast<size_t>(t.s & 1) * bp.q_buf_bytes;
                 QEpi::State st = QEpi::prepare(ep, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
-                const uint32_t taddr = epi_acquire<CG, ST>(P, lt, quarter);
+                const uint32_t taddr = acquire();
                 QEpi::run(ep, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, nullptr, epi_tid);
             } else if (DENSE && t.type == T_G) {
                 gp.b_off = t.vb0; gp.N = t.Vb_eff;
@@ -333,36 +410,49 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 ep.qs = static_cast<const uint8_t*>(ep.qs) + static_cast<size_t>(t.s & 1) * bp.q_buf_bytes;
                 if (!on(T_DX)) ep.rows = 0;                     // forward-only: nothing consumes G
                 GDenseEpi::State st = GDenseEpi::prepare(ep, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
-                const uint32_t taddr = epi_acquire<CG, ST>(P, lt, quarter);
+                const uint32_t taddr = acquire();
                 GDenseEpi::run(ep, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, nullptr, epi_tid);
             } else if (t.type == T_G) {
                 gp.b_off = t.vb0; gp.N = t.Vb_eff;
                 GEpi::Params ep = bp.g;
                 ep.gs += static_cast<size_t>(t.s % bp.gbufs) * bp.planes * ep.plane_stride;
                 GEpi::State st = GEpi::prepare(ep, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
-                const uint32_t taddr = epi_acquire<CG, ST>(P, lt, quarter);
+                const uint32_t taddr = acquire();
                 GEpi::run(ep, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, nullptr, epi_tid);
             } else if (t.type == T_DX) {
                 gp.N = bp.d; gp.first = (t.vi == 0); gp.last = (t.vi == bp.nvb - 1);
                 DxEpi::State st = DxEpi::prepare(bp.dx, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
-                const uint32_t taddr = epi_acquire<CG, ST>(P, lt, quarter);
+                const uint32_t taddr = acquire();
                 DxEpi::run(bp.dx, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, P.epi_smem, epi_tid);
             } else {
                 int M_eff;
                 if (bp.wl == 0) { gp.N = t.Vb_eff; gp.row_off = 0; gp.col_off = t.vb0; M_eff = bp.d; }
                 else { gp.N = bp.d; gp.row_off = t.vb0; gp.col_off = 0; M_eff = t.Vb_eff; }
                 gp.first = bp.dw_store_first && t.tb0 == 0;          // first token super-tile: plain stores
-                const uint32_t taddr = epi_acquire<CG, ST>(P, lt, quarter);
+                const uint32_t taddr = acquire();
                 DwEpi::run(bp.dw, gp, NoState{}, taddr, m_blk, t.n_blk, row_in_tile, M_eff, P.epi_smem, epi_tid);
             }
             epi_release<CG, ST>(P, lt, lane);                       // TMEM stage free for the MMA warp
             ++lt;
+#ifdef OPD_TRACE
+            const long long p0 = clock64();
+#endif
             // publish: all 128 epilogue threads' global stores, then one release increment
             __threadfence();
             fence_proxy_async_all();
             asm volatile("bar.sync 1, 128;" ::: "memory");
             if (epi_tid == 0) atomicAdd((t.type == T_G ? bp.g_done : (t.type == T_Q ? bp.q_done : bp.c_done)) + t.s, 1);
+#ifdef OPD_TRACE
+            tr[0] += 1; tr[1] += clock64() - t0; tr[4] += clock64() - p0;
+#endif
         }
+#ifdef OPD_TRACE
+        if (bp.trace && epi_tid == 0) {
+            for (int ty = 0; ty < 4; ++ty) for (int k = 0; k < 8; ++k)
+                if (tre[ty][k]) atomicAdd(bp.trace + (2 * 4 + ty) * 8 + k, (unsigned long long)tre[ty][k]);
+            atomicAdd(bp.trace + 96 + 2, (unsigned long long)(clock64() - k0));
+        }
+#endif
     }
     P.teardown(warp);
 }

@@ -188,18 +188,26 @@ struct NoMid { __device__ __forceinline__ void operator()() const {} };
 
 // `mid` runs once, after the loads of the tile's second k-block have been issued (after the last one for shorter tiles): the
 // persistent kernels fetch and decode their NEXT tile there, while the ring still holds work for the tensor pipe.
+// Tracing builds (-DOPD_TRACE, profiles/r02_trace.md): `tr` accumulates the cycles a role spends in its waits.
 template <int CG, int ST, class Mid = NoMid>
-__device__ __forceinline__ void produce_tile(const Pipe<CG, ST>& P, const TileOp& t, int& it, Mid&& mid = Mid{}) {
+__device__ __forceinline__ void produce_tile(const Pipe<CG, ST>& P, const TileOp& t, int& it, Mid&& mid = Mid{}, long long* tr = nullptr) {
     using C = Cfg<CG, ST>;
     const int kblocks = (t.K + BK - 1) / BK;
     const int mid_at = min(2, kblocks * t.nseg);
     int issued = 0;
     for (int seg = 0; seg < t.nseg; ++seg) {
         for (int kb_i = 0; kb_i < kblocks; ++kb_i, ++it) {
+#ifdef OPD_TRACE
+            if (issued++ == mid_at) { const long long t0 = clock64(); mid(); if (tr) tr[4] += clock64() - t0; }
+            const int s = it % C::STAGES;
+            const uint32_t ph = (it / C::STAGES) & 1;
+            if (tr) mbar_wait_timed(&P.empty_bar[s], ph ^ 1, tr[2]); else mbar_wait(&P.empty_bar[s], ph ^ 1);
+#else
             if (issued++ == mid_at) mid();
             const int s = it % C::STAGES;
             const uint32_t ph = (it / C::STAGES) & 1;
             mbar_wait(&P.empty_bar[s], ph ^ 1);
+#endif
             uint8_t* sA = P.smem + s * C::STAGE_BYTES;
             uint8_t* sB = sA + C::A_STAGE_BYTES;
             const int kca = t.ka + kb_i * BK, kcb = t.kb + kb_i * BK;
@@ -240,7 +248,7 @@ __device__ __forceinline__ void produce_tile(const Pipe<CG, ST>& P, const TileOp
 
 // MMA issuer (one elected lane of the CTA / of the pair leader): all MMAs of one tile into accumulator stage lt & 1.
 template <int CG, int ST, class Mid = NoMid>
-__device__ __forceinline__ void mma_tile(const Pipe<CG, ST>& P, int a_mn, int b_mn, int kiters, int lt, int& it, Mid&& mid = Mid{}) {
+__device__ __forceinline__ void mma_tile(const Pipe<CG, ST>& P, int a_mn, int b_mn, int kiters, int lt, int& it, Mid&& mid = Mid{}, long long* tr = nullptr) {
     using C = Cfg<CG, ST>;
     const uint32_t idesc = make_idesc_bf16(C::TILE_M, BN, a_mn, b_mn);
     const uint32_t a_kstep = a_mn ? (UMMA_K * MN_BOX * 2) : (UMMA_K * 2);   // bytes per UMMA_K step
@@ -249,15 +257,25 @@ __device__ __forceinline__ void mma_tile(const Pipe<CG, ST>& P, int a_mn, int b_
     const uint32_t b_lbo = b_mn ? MN_BOX_BYTES : 16;
     const int as = lt & 1;
     const uint32_t aph = (lt >> 1) & 1;
+#ifdef OPD_TRACE
+    if (tr) mbar_wait_timed(&P.tempty_bar[as], aph ^ 1, tr[2]); else
+#endif
     mbar_wait(&P.tempty_bar[as], aph ^ 1);
     tc_fence_after();
     const uint32_t tacc = P.tmem_base + as * BN;
     const int mid_at = min(2, kiters - 1);
     for (int ki = 0; ki < kiters; ++ki, ++it) {
+#ifdef OPD_TRACE
+        if (ki == mid_at) { const long long t0 = clock64(); mid(); if (tr) tr[4] += clock64() - t0; }
+        const int s = it % C::STAGES;
+        const uint32_t ph = (it / C::STAGES) & 1;
+        if (tr) mbar_wait_timed(&P.full_bar[s], ph, tr[ki < C::STAGES ? 5 : 3]); else mbar_wait(&P.full_bar[s], ph);
+#else
         if (ki == mid_at) mid();                   // MMAs of the first k-blocks are queued: time to decode the next tile
         const int s = it % C::STAGES;
         const uint32_t ph = (it / C::STAGES) & 1;
         mbar_wait(&P.full_bar[s], ph);
+#endif
         tc_fence_after();
         const uint32_t a0 = smem_u32(P.smem + s * C::STAGE_BYTES);
         const uint32_t b0 = a0 + C::A_STAGE_BYTES;

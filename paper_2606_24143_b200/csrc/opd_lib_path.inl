@@ -315,8 +315,30 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
                                  h->l2_bytes, h->l2_persist_max, h->l2_window_max, h->l2_persist, win.bytes, win.hit_ratio);
             }
         }
+#ifdef OPD_TRACE
+        static unsigned long long* trace_buf = nullptr;     // tracing build: cycle sums per warp role and tile type, printed per call
+        if (!trace_buf) OPD_CUDA(h, cudaMalloc(&trace_buf, 128 * 8));
+        OPD_CUDA(h, cudaMemsetAsync(trace_buf, 0, 128 * 8, st));
+        bp.trace = env_int("OPD_TRACE", 0) ? trace_buf : nullptr;
+#endif
         opd_status_t ls = launch_bwd<false>(h, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_xc_k, m_w_fwd, bp, win);
         if (ls != OPD_OK) return ls;
+#ifdef OPD_TRACE
+        if (bp.trace) {
+            unsigned long long tb[128];
+            OPD_CUDA(h, cudaMemcpyAsync(tb, trace_buf, sizeof(tb), cudaMemcpyDeviceToHost, st));
+            OPD_CUDA(h, cudaStreamSynchronize(st));
+            static const char* roles[3] = {"mma", "tma", "epi"};
+            static const char* types[4] = {"G", "DX", "DW", "Q"};
+            std::fprintf(stderr, "[opd trace] kernel cycles summed over CTAs: mma %llu tma %llu epi %llu\n", tb[96], tb[97], tb[98]);
+            for (int r = 0; r < 3; ++r) for (int ty = 0; ty < 4; ++ty) {
+                const unsigned long long* v = tb + (r * 4 + ty) * 8;
+                if (!v[0]) continue;
+                std::fprintf(stderr, "[opd trace] %s %-2s n=%llu total=%llu s2=%llu s3=%llu s4=%llu s5=%llu s6=%llu\n", roles[r], types[ty],
+                             v[0], v[1], v[2], v[3], v[4], v[5], v[6]);
+            }
+        }
+#endif
         h->n_kernels++; h->n_gemm++;
         OPD_CUDA(h, cudaGetLastError());
     }
