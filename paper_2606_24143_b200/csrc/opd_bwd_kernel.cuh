@@ -6,9 +6,9 @@
 //   G(s)   logits of super-tile s recomputed -> G tile (bf16) into buffer s%R of the G ring (consumed from L2)
 //   DX(s)  grad_hidden[tb] (+)= G(s) . W[:,vb]^T        DW(s)  grad_W[:,vb] += Xc[tb]^T . G(s)
 //
-// CTA pairs claim items dynamically, in list order, from a global ticket counter (ticket_take / ticket_publish / ticket_read in
-// opd_gemm.cuh); an item only depends on earlier items, through two counters per super-tile in global memory
-// (release by the epilogue after its stores, acquire by whoever consumes):
+// CTA pairs claim items dynamically, in list order, from a global ticket counter (the tile queue of opd_gemm.cuh: one thread
+// per pair claims, decodes and publishes the tile, every warp role copies it); an item only depends on earlier items,
+// through two counters per super-tile in global memory (release by the epilogue after its stores, acquire by whoever consumes):
 //   g_done[s] == #G tiles      before the TMA producer loads G(s) for a DX/DW tile
 //   c_done[s-1] complete       before a DX/DW(s) epilogue touches the fp32 accumulators (previous writer)
 //   c_done[s-R] complete       before a G(s) epilogue overwrites ring buffer s%R (previous readers; R = ring depth)
@@ -55,10 +55,15 @@ struct BwdParams {
 
 enum { T_G = 0, T_DX = 1, T_DW = 2, T_Q = 3 };
 
+// One decoded item of the tile list: what the claimer publishes through the tile queue (SCHED_WORDS words).
 struct BwdTile {
     int type, s, tb0, vb0, Tb_eff, Vb_eff, vi, m_blk, n_blk;
     int ng;                    // G tiles of super-tile s (what a DX / DW tile waits for)
+    int dep_cnt;               // CTA-level epilogues the counter this tile's epilogue waits on must have seen (0: no wait):
+                               //   G / DX / DW: c_done of the previous writer / readers; Q (dense): g_done of super-tile s - 2
+    int valid;                 // 0: the list is exhausted (published once, every reader stops on it)
 };
+static_assert(sizeof(BwdTile) == SCHED_WORDS * 4, "BwdTile is what the tile queue carries");
 
 // DENSE: block b holds Q(b), G(b-1), DX(b-2), DW(b-2) (the Q tiles of a super-tile run one block ahead of its G tiles);
 // otherwise block b holds G(b), DX(b-1), DW(b-1).
@@ -198,26 +203,58 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
     const int PA[6] = {0, 0, 1, 0, 2, 1};
     const int PB[6] = {0, 1, 0, 2, 0, 1};
 
+    // ---- tile queue.  The claimer takes the next item of the list, decodes it (BwdSched: the integer divisions live here)
+    // and publishes the decoded tile; every other role copies 48 bytes out of shared memory.
+    auto claim_next = [&](BwdSched<CG, DENSE>& sc, int& n, BwdTile& o) -> bool {
+        for (;;) {
+            const uint32_t item = ticket_take(bp.ticket);
+            const bool ok = sc.get(item, o);
+            if (ok && !on(o.type)) continue;             // tile types this launch does not run are never published
+            o.valid = ok ? 1 : 0;
+            o.dep_cnt = 0;
+            if (ok) {
+                if (DENSE && o.type == T_Q) {
+                    if (o.s >= 2 && on(T_G)) o.dep_cnt = CG * sc.nG(o.s - 2);
+                } else {
+                    const int dep = (o.type == T_G) ? o.s - bp.gbufs : o.s - 1;
+                    if (dep >= 0 && on(T_DX) && on(T_DW)) o.dep_cnt = CG * (sc.nDX(dep) + sc.nDW(dep));
+                }
+            }
+            tile_publish<CG, ST>(P, n++, reinterpret_cast<const uint32_t(&)[SCHED_WORDS]>(o));
+            return ok;                                   // the end of the list is published too: every reader stops on it
+        }
+    };
+#ifdef OPD_TRACE
+    long long q_wait = 0, q_copy = 0, q_arrive = 0;      // this thread's cycles in the three steps of read_next
+#endif
+    auto read_next = [&](int& n, BwdTile& o) -> bool {   // single-thread readers (TMA producer, MMA issuer)
+#ifdef OPD_TRACE
+        const long long c0 = clock64();
+        tile_wait<CG, ST>(P, n);
+        const long long c1 = clock64();
+        tile_copy<CG, ST>(P, n, reinterpret_cast<uint32_t(&)[SCHED_WORDS]>(o));
+        const long long c2 = clock64();
+        tile_consumed<CG, ST>(P, n);
+        const long long c3 = clock64();
+        q_wait += c1 - c0; q_copy += c2 - c1; q_arrive += c3 - c2;
+#else
+        tile_wait<CG, ST>(P, n);
+        tile_copy<CG, ST>(P, n, reinterpret_cast<uint32_t(&)[SCHED_WORDS]>(o));
+        tile_consumed<CG, ST>(P, n);
+#endif
+        ++n;
+        return o.valid != 0;
+    };
+
     if (warp == 0) {
         // =========================== TMA producer ===========================
         if (elect_one()) {
-            BwdSched<CG, DENSE> sc; sc.init(bp);
+            BwdSched<CG, DENSE> sc;
+            if constexpr (CG == 1) sc.init(bp);              // CG = 1: the producer is the claimer
             BwdTile t, nxt;
             int it = 0, n = 0, g_ready = -1;
-            // next enabled item of this CTA (pair).  CG = 1: the producer claims it itself; CG = 2: both producers read
-            // what the peer's warp 1 claimed.  Never called again once the list is exhausted.
             auto fetch = [&](BwdTile& o) -> bool {
-                if constexpr (CG == 1) {
-                    for (;;) {                               // claim; publish what this launch runs (and the end of the list)
-                        const uint32_t item = ticket_take(bp.ticket);
-                        const bool ok = sc.get(item, o);
-                        if (ok && !on(o.type)) continue;
-                        ticket_publish<CG, ST>(P, n++, item);
-                        return ok;
-                    }
-                } else {
-                    return sc.get(ticket_read<CG, ST>(P, n++), o);
-                }
+                if constexpr (CG == 1) return claim_next(sc, n, o); else return read_next(n, o);
             };
 #ifdef OPD_TRACE
             long long trp[4][8] = {};
@@ -283,6 +320,8 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 for (int ty = 0; ty < 4; ++ty) for (int k = 0; k < 8; ++k)
                     if (trp[ty][k]) atomicAdd(bp.trace + (1 * 4 + ty) * 8 + k, (unsigned long long)trp[ty][k]);
                 atomicAdd(bp.trace + 96 + 1, (unsigned long long)(clock64() - k0));
+                atomicAdd(bp.trace + 104, (unsigned long long)q_wait); atomicAdd(bp.trace + 105, (unsigned long long)q_copy);
+                atomicAdd(bp.trace + 106, (unsigned long long)q_arrive);
             }
 #endif
         }
@@ -291,20 +330,14 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
         if (CG == 2 && rank == 1 && elect_one()) {
             BwdSched<CG, DENSE> sc; sc.init(bp);
             BwdTile t;
-            for (int n = 0;;) {
-                const uint32_t item = ticket_take(bp.ticket);
-                const bool ok = sc.get(item, t);
-                if (ok && !on(t.type)) continue;         // tile types this launch does not run are never published
-                ticket_publish<CG, ST>(P, n++, item);
-                if (!ok) break;                          // the end of the list is published too: every reader stops on it
-            }
+            int n = 0;
+            while (claim_next(sc, n, t)) {}
         }
         // =========================== MMA issuer ===========================
         if (rank == 0 && elect_one()) {
-            BwdSched<CG, DENSE> sc; sc.init(bp);
             BwdTile t, nxt;
             int it = 0, lt = 0, n = 0;
-            auto fetch = [&](BwdTile& o) -> bool { return sc.get(ticket_read<CG, ST>(P, n++), o); };
+            auto fetch = [&](BwdTile& o) -> bool { return read_next(n, o); };
 #ifdef OPD_TRACE
             long long trm[4][8] = {};
             const long long k0 = clock64();
@@ -320,7 +353,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 else if (DENSE && t.type == T_Q) { a_mn = 0; b_mn = (bp.wl_t == 0); K = bp.dT; }
                 else if (t.type == T_DX) { a_mn = 0; b_mn = (bp.wl == 1); K = t.Vb_eff; }
                 else { a_mn = 1; b_mn = 1; K = t.Tb_eff; }
-                // the next tile is fetched and decoded after this tile's first MMAs are queued, not between two tiles
+                // the next tile is read once this tile's first MMAs are queued, not between two tiles
 #ifdef OPD_TRACE
                 mma_tile<CG, ST>(P, a_mn, b_mn, ((K + BK - 1) / BK) * nseg, lt, it, [&] { have_next = fetch(nxt); }, tr);
                 tr[0] += 1; tr[1] += clock64() - t0; tr[6] += ((K + BK - 1) / BK) * nseg;
@@ -335,6 +368,8 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 for (int ty = 0; ty < 4; ++ty) for (int k = 0; k < 8; ++k)
                     if (trm[ty][k]) atomicAdd(bp.trace + (0 * 4 + ty) * 8 + k, (unsigned long long)trm[ty][k]);
                 atomicAdd(bp.trace + 96 + 0, (unsigned long long)(clock64() - k0));
+                atomicAdd(bp.trace + 100, (unsigned long long)q_wait); atomicAdd(bp.trace + 101, (unsigned long long)q_copy);
+                atomicAdd(bp.trace + 102, (unsigned long long)q_arrive);
             }
 #endif
         }
@@ -343,7 +378,6 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
         const int quarter = warp & 3;
         const int row_in_tile = quarter * 32 + lane;
         const int epi_tid = (warp - 2) * 32 + lane;
-        BwdSched<CG, DENSE> sc; sc.init(bp);
         BwdTile t;
         int lt = 0;
         int c_ready = -1, gq_ready = -1, q_ready = -1;              // dependencies already seen complete (warp-uniform)
@@ -373,16 +407,19 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
 #endif
         };
         for (int n = 0;; ++n) {
-            uint32_t item = 0;
 #ifdef OPD_TRACE
             const long long t0 = clock64();
 #endif
-            if (lane == 0) item = ticket_read<CG, ST>(P, n);
-            item = __shfl_sync(0xffffffffu, item, 0);
-            if (!sc.get(item, t)) break;
+            // each epilogue warp is one reader of the tile queue: lane 0 waits, every lane copies, lane 0 hands the slot back
+            if (lane == 0) tile_wait<CG, ST>(P, n);
+            __syncwarp();
+            tile_copy<CG, ST>(P, n, reinterpret_cast<uint32_t(&)[SCHED_WORDS]>(t));
+            __syncwarp();
+            if (lane == 0) tile_consumed<CG, ST>(P, n);
+            if (!t.valid) break;
 #ifdef OPD_TRACE
             tr = tre[t.type];
-            tr[5] += clock64() - t0;          // ticket wait + decode
+            tr[5] += clock64() - t0;          // queue wait + copy
 #endif
             const int m_blk = t.m_blk * CG + rank;    // this CTA's 128-row block inside the GEMM
             GemmParams gp{};                      // the fields the epilogues read
@@ -390,10 +427,10 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             // wait for the previous writer / readers of what this epilogue is about to write (and, dense, for its Q tile)
             // (each dependency is checked once per super-tile, not once per tile: c_done completes in super-tile order)
             if (t.type == T_Q) {
-                if (t.s >= 2 && on(T_G) && t.s - 2 != gq_ready) { wait_for(bp.g_done + t.s - 2, CG * sc.nG(t.s - 2)); gq_ready = t.s - 2; }
+                if (t.dep_cnt > 0 && t.s - 2 != gq_ready) { wait_for(bp.g_done + t.s - 2, t.dep_cnt); gq_ready = t.s - 2; }
             } else {
                 const int dep = (t.type == T_G) ? t.s - bp.gbufs : t.s - 1;
-                if (dep > c_ready && on(T_DX) && on(T_DW)) { wait_for(bp.c_done + dep, CG * (sc.nDX(dep) + sc.nDW(dep))); c_ready = dep; }
+                if (t.dep_cnt > 0 && dep > c_ready) { wait_for(bp.c_done + dep, t.dep_cnt); c_ready = dep; }
                 if (DENSE && t.type == T_G && on(T_Q) && t.s != q_ready) { wait_for(bp.q_done + t.s, CG * t.ng); q_ready = t.s; }
             }
             if (DENSE && t.type == T_Q) {

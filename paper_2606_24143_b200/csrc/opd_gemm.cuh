@@ -37,7 +37,8 @@ constexpr int MAX_STAGES = 6;
 #ifndef OPD_BWD_STAGES
 #define OPD_BWD_STAGES 6
 #endif
-constexpr int SCHED_Q = 4;                 // depth of the tile-ticket queue of the dynamically scheduled kernels
+constexpr int SCHED_Q = 8;                 // depth of the tile queue of the dynamically scheduled kernels
+constexpr int SCHED_WORDS = 12;            // 32-bit words of one decoded tile descriptor in the queue (48 bytes)
 
 template <int CG> __host__ __device__ constexpr int fwd_stages() { return CG == 1 ? 4 : OPD_FWD_STAGES; }
 template <int CG> __host__ __device__ constexpr int bwd_stages() { return CG == 1 ? 4 : OPD_BWD_STAGES; }
@@ -96,8 +97,8 @@ struct Pipe {
     using C = Cfg<CG, ST>;
     uint8_t* smem;
     uint64_t *full_bar, *empty_bar, *tfull_bar, *tempty_bar;
-    uint64_t *sfull_bar, *sempty_bar;     // tile-ticket queue (bwd_kernel): ticket q published / consumed by every reader
-    uint32_t* sticket;                    // [SCHED_Q] claimed tickets (a copy in each CTA of a pair)
+    uint64_t *sfull_bar, *sempty_bar;     // tile queue (bwd_kernel): slot q published / consumed by every reader
+    uint32_t* sticket;                    // [SCHED_Q][SCHED_WORDS] decoded tiles (a copy in each CTA of a pair)
     uint32_t* tmem_slot;
     uint8_t* epi_smem;
     uint32_t tmem_base;
@@ -140,34 +141,52 @@ struct Pipe {
     }
 };
 
-// ------------------------------------------------------------------------------------------------ tile tickets
+// ------------------------------------------------------------------------------------------------ tile queue
 // Dynamic tile scheduling for kernels whose tiles wait on tiles of other CTAs: ONE thread of a CTA (pair) claims the next
-// item of the tile list from a global counter and publishes it to every warp role of the CTA (pair) through a small queue
-// in shared memory.  Items are claimed in list order, so everything an item depends on has been claimed by a CTA that is
-// already running: the kernel makes progress with any number of resident CTAs (no co-residency requirement).
-// The claimer runs in CTA rank CG - 1 (its copy of the `sempty` barriers is the live one); it runs up to SCHED_Q tickets
-// ahead of the slowest reader.  Only items the launch really runs are published (the claimer drops disabled tile types),
-// so a reader that fetches its next tile in the middle of the current one never needs more than one queue slot ahead.
+// item of the tile list from a global counter, DECODES it, and publishes the decoded descriptor (SCHED_WORDS words) to every
+// warp role of the CTA (pair) through a small queue in shared memory.  Items are claimed in list order, so everything an
+// item depends on has been claimed by a CTA that is already running: the kernel makes progress with any number of resident
+// CTAs (no co-residency requirement).  The claimer runs in CTA rank CG - 1 (its copy of the `sempty` barriers is the live
+// one), up to SCHED_Q tiles ahead of the slowest reader; readers only copy 48 bytes out of shared memory, so nothing
+// but two barrier operations sits between two tiles of the TMA producer or the MMA issuer (the round trip of the global
+// atomic and the integer divisions of the decoder are the claimer's: profiles/r02_trace.md).  Only items the launch
+// really runs are published (the claimer drops disabled tile types).
 __device__ __forceinline__ uint32_t ticket_take(int* counter) { return static_cast<uint32_t>(atomicAdd(counter, 1)); }
+__device__ __forceinline__ void st_shared_cluster_v4(uint32_t cluster_addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("st.shared::cluster.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(cluster_addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
 template <int CG, int ST>
-__device__ __forceinline__ void ticket_publish(const Pipe<CG, ST>& P, int n, uint32_t t) {
+__device__ __forceinline__ void tile_publish(const Pipe<CG, ST>& P, int n, const uint32_t (&w)[SCHED_WORDS]) {
     const int q = n % SCHED_Q;
     mbar_wait_cluster(&P.sempty_bar[q], ((n / SCHED_Q) & 1) ^ 1);
-    P.sticket[q] = t;
+    uint32_t* slot = P.sticket + q * SCHED_WORDS;
+#pragma unroll
+    for (int i = 0; i < SCHED_WORDS; i += 4) *reinterpret_cast<uint4*>(slot + i) = make_uint4(w[i], w[i + 1], w[i + 2], w[i + 3]);
     if constexpr (CG == 2) {
-        st_shared_cluster_u32(mapa_rank(smem_u32(&P.sticket[q]), 0), t);
+        const uint32_t remote = mapa_rank(smem_u32(slot), 0);
+#pragma unroll
+        for (int i = 0; i < SCHED_WORDS; i += 4) st_shared_cluster_v4(remote + i * 4, w[i], w[i + 1], w[i + 2], w[i + 3]);
         mbar_arrive_cluster(mapa_rank(smem_u32(&P.sfull_bar[q]), 0));
     }
     mbar_arrive(&P.sfull_bar[q]);
 }
-// called by one lane of a reader; every reader consumes every ticket exactly once, in order
+// Called by one thread of a reader (wait = true) and, for warp-wide readers, by the other lanes after a __syncwarp
+// (wait = false); every reader consumes every slot exactly once, in order, and signals it with tile_consumed.
 template <int CG, int ST>
-__device__ __forceinline__ uint32_t ticket_read(const Pipe<CG, ST>& P, int n) {
-    const int q = n % SCHED_Q;
-    mbar_wait_cluster(&P.sfull_bar[q], (n / SCHED_Q) & 1);
-    const uint32_t t = *reinterpret_cast<volatile uint32_t*>(&P.sticket[q]);
-    mbar_arrive_cluster(mapa_rank(smem_u32(&P.sempty_bar[q]), CG - 1));
-    return t;
+__device__ __forceinline__ void tile_wait(const Pipe<CG, ST>& P, int n) {
+    mbar_wait_cluster(&P.sfull_bar[n % SCHED_Q], (n / SCHED_Q) & 1);
+}
+template <int CG, int ST>
+__device__ __forceinline__ void tile_copy(const Pipe<CG, ST>& P, int n, uint32_t (&w)[SCHED_WORDS]) {
+    const volatile uint4* slot = reinterpret_cast<const volatile uint4*>(P.sticket + (n % SCHED_Q) * SCHED_WORDS);
+#pragma unroll
+    for (int i = 0; i < SCHED_WORDS / 4; ++i) {
+        w[4 * i] = slot[i].x; w[4 * i + 1] = slot[i].y; w[4 * i + 2] = slot[i].z; w[4 * i + 3] = slot[i].w;
+    }
+}
+template <int CG, int ST>
+__device__ __forceinline__ void tile_consumed(const Pipe<CG, ST>& P, int n) {
+    mbar_arrive_remote(mapa_rank(smem_u32(&P.sempty_bar[n % SCHED_Q]), CG - 1));     // a read-done signal: no cluster release
 }
 
 // One tile's operand stream as the TMA producer of ONE CTA sees it.
@@ -263,7 +282,9 @@ __device__ __forceinline__ void mma_tile(const Pipe<CG, ST>& P, int a_mn, int b_
     mbar_wait(&P.tempty_bar[as], aph ^ 1);
     tc_fence_after();
     const uint32_t tacc = P.tmem_base + as * BN;
-    const int mid_at = min(2, kiters - 1);
+    // `mid` (the persistent kernels read their next tile there) runs where the issuer would block anyway: the ring's
+    // stages have all been issued and the next one only fills once the tensor pipe has retired this tile's first k-block
+    const int mid_at = min(C::STAGES, kiters - 1);
     for (int ki = 0; ki < kiters; ++ki, ++it) {
 #ifdef OPD_TRACE
         if (ki == mid_at) { const long long t0 = clock64(); mid(); if (tr) tr[4] += clock64() - t0; }
@@ -304,7 +325,7 @@ __device__ __forceinline__ void epi_release(const Pipe<CG, ST>& P, int lt, int l
     __syncwarp();
     if (lane == 0) {
         if constexpr (CG == 1) mbar_arrive(&P.tempty_bar[lt & 1]);
-        else mbar_arrive_cluster(mapa_rank(smem_u32(&P.tempty_bar[lt & 1]), 0));
+        else mbar_arrive_remote(mapa_rank(smem_u32(&P.tempty_bar[lt & 1]), 0));      // read-done signal (see mbar_arrive_remote)
     }
 }
 

@@ -331,6 +331,8 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
             static const char* roles[3] = {"mma", "tma", "epi"};
             static const char* types[4] = {"G", "DX", "DW", "Q"};
             std::fprintf(stderr, "[opd trace] kernel cycles summed over CTAs: mma %llu tma %llu epi %llu\n", tb[96], tb[97], tb[98]);
+            std::fprintf(stderr, "[opd trace] queue reads (wait / copy / arrive cycles): mma %llu %llu %llu  tma %llu %llu %llu\n",
+                         tb[100], tb[101], tb[102], tb[104], tb[105], tb[106]);
             for (int r = 0; r < 3; ++r) for (int ty = 0; ty < 4; ++ty) {
                 const unsigned long long* v = tb + (r * 4 + ty) * 8;
                 if (!v[0]) continue;

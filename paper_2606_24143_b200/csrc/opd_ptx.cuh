@@ -68,6 +68,15 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
+// Same without a cluster-scope release: for "I am done READING" signals (a shared-memory slot or a TMEM accumulator stage
+// handed back to its writer in the peer CTA).  The signalling thread has no writes to publish, and the reads it hands back
+// have returned their values before the arrive can issue (tcgen05.ld: after tcgen05.wait::ld + fence::before_thread_sync),
+// so the default .release.cta form is enough -- the same instruction CUTLASS's pipelines use for a consumer's release to a
+// remote producer.  The .release.cluster form above compiles to MEMBAR.ALL.GPU + ERRBAR in front of the arrive, which
+// costs the issuing thread 1000-2200 cycles per call (profiles/r02_trace.md): fine for the claimer, not for the MMA issuer.
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     uint32_t a = smem_u32(bar);
     asm volatile(
