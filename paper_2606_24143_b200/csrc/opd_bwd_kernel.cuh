@@ -8,10 +8,15 @@
 //
 // CTA pairs claim items dynamically, in list order, from a global ticket counter (the tile queue of opd_gemm.cuh: one thread
 // per pair claims, decodes and publishes the tile, every warp role copies it); an item only depends on earlier items,
-// through two counters per super-tile in global memory (release by the epilogue after its stores, acquire by whoever consumes):
-//   g_done[s] == #G tiles      before the TMA producer loads G(s) for a DX/DW tile
-//   c_done[s-1] complete       before a DX/DW(s) epilogue touches the fp32 accumulators (previous writer)
-//   c_done[s-R] complete       before a G(s) epilogue overwrites ring buffer s%R (previous readers; R = ring depth)
+// through three counters per super-tile in global memory (release by the publisher warp once the epilogue's stores are out,
+// acquire by whoever consumes):
+//   g_done[s] == #G tiles          before the TMA producer loads G(s) for a DX/DW tile
+//   dx_done[s-1] complete          before a DX(s) epilogue touches the fp32 partial sums of grad_hidden (previous writer; at a
+//                                  token super-tile boundary: the previous reader)
+//   dw_done[s-nvb] complete        before a DW(s) epilogue reduces into its grad_W panel (previous token super-tile, same columns)
+//   dx_done, dw_done[s-R] complete before a G(s) epilogue overwrites ring buffer s%R (previous readers; R = ring depth)
+// (one counter for DX and DW made every DX(s) epilogue wait for the long DW(s-1) tiles that were claimed just before it and
+// share nothing with it: 18% of the epilogue warps' time at T = 4096, d = 1024.)
 // One launch instead of one per GEMM and super-tile (about 900 at C4): no partial last waves, no pipeline refills.
 // Because an item's dependencies were all claimed before it, by CTAs that are running, the kernel needs no particular
 // number of resident CTAs: it completes next to other kernels, under MPS or with SM-limited contexts (the host still sizes
@@ -29,9 +34,11 @@ struct BwdParams {
     int planes;                // 1 (bf16) or 3 (fp32 inputs as three bf16 terms)
     const int* n_live;
     int* g_done;               // [S]
-    int* c_done;               // [S]
+    int* dx_done;              // [S]
+    int* dw_done;              // [S]
     int* ticket;               // [1] next unclaimed item of the tile list (zeroed by the host before the launch)
     int order;                 // BwdSched::order
+    int q_depth;               // tiles a CTA (pair) may hold claimed but not yet started by its epilogue (1..SCHED_Q)
     int dx_group;              // BwdSched::dx_group
     int dw_store_first;        // 1: the grad_W tiles of the first token super-tile store instead of reduce-add (grad_W is
                                //    overwritten, not accumulated into: no memset and no read-modify-write for that pass)
@@ -59,8 +66,9 @@ enum { T_G = 0, T_DX = 1, T_DW = 2, T_Q = 3 };
 struct BwdTile {
     int type, s, tb0, vb0, Tb_eff, Vb_eff, vi, m_blk, n_blk;
     int ng;                    // G tiles of super-tile s (what a DX / DW tile waits for)
-    int dep_cnt;               // CTA-level epilogues the counter this tile's epilogue waits on must have seen (0: no wait):
-                               //   G / DX / DW: c_done of the previous writer / readers; Q (dense): g_done of super-tile s - 2
+    int dep_cnt;               // CTA-level epilogues the counter(s) this tile's epilogue waits on must have seen (0: no wait):
+                               //   DX: dx_done[s - 1]; DW: dw_done[s - nvb]; G: dx_done[s - R] in the low and dw_done[s - R] in the
+                               //   high 16 bits; Q (dense): g_done[s - 2]
     int valid;                 // 0: the list is exhausted (published once, every reader stops on it)
 };
 static_assert(sizeof(BwdTile) == SCHED_WORDS * 4, "BwdTile is what the tile queue carries");
@@ -174,7 +182,7 @@ __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.pr
 // DENSE adds the teacher-head Q tiles of the dense two-head KL (opd_dense.cuh); m_tx_k / m_wt_fwd are then the teacher's
 // compacted hidden states and head (unused copies of the student's maps otherwise).
 template <int CG, bool DENSE>
-__global__ void __launch_bounds__(GEMM_THREADS, 1)
+__global__ void __launch_bounds__(BWD_THREADS, 1)
 bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ CUtensorMap m_w_fwd,
            const __grid_constant__ CUtensorMap m_gs_k, const __grid_constant__ CUtensorMap m_w_dx,
            const __grid_constant__ CUtensorMap m_xc_mn, const __grid_constant__ CUtensorMap m_gs_mn,
@@ -193,7 +201,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
         if constexpr (DENSE) { prefetch_tmap(&m_tx_k); prefetch_tmap(&m_wt_fwd); }
     }
     Pipe<CG, ST> P;
-    P.setup(smem_raw, warp, lane);
+    P.setup(smem_raw, warp, lane, BWD_EPI_WARPS);
     const int rank = static_cast<int>(P.rank);
     const int mask = bp.type_mask;
     auto on = [mask](int type) { return ((mask >> type) & 1) != 0; };
@@ -206,6 +214,9 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
     // ---- tile queue.  The claimer takes the next item of the list, decodes it (BwdSched: the integer divisions live here)
     // and publishes the decoded tile; every other role copies 48 bytes out of shared memory.
     auto claim_next = [&](BwdSched<CG, DENSE>& sc, int& n, BwdTile& o) -> bool {
+        // A ticket is only taken once the tile q_depth places back has been picked up by every reader of this pair: tiles
+        // claimed far ahead sit in this pair's queue while other pairs wait for them (G tiles behind a long grad_W tile).
+        if (n >= bp.q_depth) { const int m = n - bp.q_depth; mbar_wait_cluster(&P.sempty_bar[m % SCHED_Q], (m / SCHED_Q) & 1); }
         for (;;) {
             const uint32_t item = ticket_take(bp.ticket);
             const bool ok = sc.get(item, o);
@@ -215,9 +226,13 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             if (ok) {
                 if (DENSE && o.type == T_Q) {
                     if (o.s >= 2 && on(T_G)) o.dep_cnt = CG * sc.nG(o.s - 2);
+                } else if (o.type == T_G) {
+                    const int dep = o.s - bp.gbufs;
+                    if (dep >= 0 && on(T_DX) && on(T_DW)) o.dep_cnt = (CG * sc.nDX(dep)) | ((CG * sc.nDW(dep)) << 16);
+                } else if (o.type == T_DX) {
+                    if (o.s >= 1 && on(T_DX)) o.dep_cnt = CG * sc.nDX(o.s - 1);
                 } else {
-                    const int dep = (o.type == T_G) ? o.s - bp.gbufs : o.s - 1;
-                    if (dep >= 0 && on(T_DX) && on(T_DW)) o.dep_cnt = CG * (sc.nDX(dep) + sc.nDW(dep));
+                    if (o.s >= bp.nvb && on(T_DW)) o.dep_cnt = CG * sc.nDW(o.s - bp.nvb);
                 }
             }
             tile_publish<CG, ST>(P, n++, reinterpret_cast<const uint32_t(&)[SCHED_WORDS]>(o));
@@ -373,14 +388,18 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             }
 #endif
         }
-    } else {
+    } else if (warp < 2 + BWD_EPI_WARPS) {
         // =========================== epilogue warps ===========================
+        // Two warps per TMEM lane quarter (warps w and w + 4 share a scheduler): half 0 takes columns 0-127 of a G tile and
+        // all of a Q / grad_hidden / grad_W tile (long main loops, staged through this half's shared-memory buffers), half 1
+        // columns 128-255 of a G tile.  Both halves follow every tile (queue slot, accumulator stage, publication).
         const int quarter = warp & 3;
+        const int half = (warp - 2) >> 2;
         const int row_in_tile = quarter * 32 + lane;
-        const int epi_tid = (warp - 2) * 32 + lane;
+        const int epi_tid = ((warp - 2) & 3) * 32 + lane;
         BwdTile t;
         int lt = 0;
-        int c_ready = -1, gq_ready = -1, q_ready = -1;              // dependencies already seen complete (warp-uniform)
+        int c_ready = -1, dx_ready = -1, dw_ready = -1, gq_ready = -1, q_ready = -1;   // dependencies already seen complete (warp-uniform)
 #ifdef OPD_TRACE
         long long tre[4][8] = {};
         long long* tr = tre[0];
@@ -406,6 +425,27 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             return epi_acquire<CG, ST>(P, lt, quarter);
 #endif
         };
+        // Publication of a finished tile (its dependency counter + 1, with release semantics at gpu scope) is the publisher
+        // warp's job: the fence it needs waits for the SM's outstanding stores (2000-5000 cycles per tile when the epilogue
+        // warps executed it, profiles/r02_trace.md), which the epilogue warps now spend on their next tile.  Each epilogue
+        // warp arrives on pub_full once its own stores are issued (per-thread stores; ordered before the arrive's release by
+        // the __syncwarp) or complete (TMA stores / reductions: all issued by lane 0, which waits for its bulk groups first).
+        // An epilogue warp is never more than two tiles ahead of another one (they meet at the TMEM stage hand-back: every
+        // warp waits for every tile's accumulator), so PUB_Q = 4 slots cannot mix arrivals of different rounds; warp 2 waits
+        // for the slot itself before it writes the pointer.
+        int pn = 0;
+        auto hand_over = [&](int* counter) {
+            __syncwarp();
+            if (lane == 0) {
+                bulk_wait<0>();
+                if (warp == 2) {
+                    mbar_wait(&P.pub_empty[pn % PUB_Q], ((pn / PUB_Q) & 1) ^ 1);
+                    *const_cast<int* volatile*>(P.pub_ptr + pn % PUB_Q) = counter;
+                }
+                mbar_arrive(&P.pub_full[pn % PUB_Q]);
+            }
+            ++pn;
+        };
         for (int n = 0;; ++n) {
 #ifdef OPD_TRACE
             const long long t0 = clock64();
@@ -416,7 +456,7 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             tile_copy<CG, ST>(P, n, reinterpret_cast<uint32_t(&)[SCHED_WORDS]>(t));
             __syncwarp();
             if (lane == 0) tile_consumed<CG, ST>(P, n);
-            if (!t.valid) break;
+            if (!t.valid) { hand_over(nullptr); break; }
 #ifdef OPD_TRACE
             tr = tre[t.type];
             tr[5] += clock64() - t0;          // queue wait + copy
@@ -424,16 +464,29 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
             const int m_blk = t.m_blk * CG + rank;    // this CTA's 128-row block inside the GEMM
             GemmParams gp{};                      // the fields the epilogues read
             gp.tok_off = t.tb0;
+#ifdef OPD_TRACE
+            gp.tr = tr;
+#endif
             // wait for the previous writer / readers of what this epilogue is about to write (and, dense, for its Q tile)
-            // (each dependency is checked once per super-tile, not once per tile: c_done completes in super-tile order)
-            if (t.type == T_Q) {
+            // (each dependency is checked once per super-tile, not once per tile: a CTA's tiles come in list order)
+            const bool works = !(half == 1 && (DENSE || t.type != T_G));      // this warp has columns of the tile to process
+            if (!works) {
+            } else if (t.type == T_Q) {
                 if (t.dep_cnt > 0 && t.s - 2 != gq_ready) { wait_for(bp.g_done + t.s - 2, t.dep_cnt); gq_ready = t.s - 2; }
+            } else if (t.type == T_G) {
+                const int dep = t.s - bp.gbufs;
+                if (t.dep_cnt > 0 && dep > c_ready) {
+                    wait_for(bp.dx_done + dep, t.dep_cnt & 0xffff); wait_for(bp.dw_done + dep, t.dep_cnt >> 16); c_ready = dep;
+                }
+                if (DENSE && on(T_Q) && t.s != q_ready) { wait_for(bp.q_done + t.s, CG * t.ng); q_ready = t.s; }
+            } else if (t.type == T_DX) {
+                if (t.dep_cnt > 0 && t.s - 1 > dx_ready) { wait_for(bp.dx_done + t.s - 1, t.dep_cnt); dx_ready = t.s - 1; }
             } else {
-                const int dep = (t.type == T_G) ? t.s - bp.gbufs : t.s - 1;
-                if (t.dep_cnt > 0 && dep > c_ready) { wait_for(bp.c_done + dep, t.dep_cnt); c_ready = dep; }
-                if (DENSE && t.type == T_G && on(T_Q) && t.s != q_ready) { wait_for(bp.q_done + t.s, CG * t.ng); q_ready = t.s; }
+                if (t.dep_cnt > 0 && t.s - bp.nvb > dw_ready) { wait_for(bp.dw_done + t.s - bp.nvb, t.dep_cnt); dw_ready = t.s - bp.nvb; }
             }
-            if (DENSE && t.type == T_Q) {
+            if (!works) {
+                (void)acquire();                                    // nothing to do for this tile: stay in step with the stage
+            } else if (DENSE && t.type == T_Q) {
                 gp.b_off = t.vb0; gp.N = t.Vb_eff;
                 QEpi::Params ep = bp.q;
                 ep.qs = static_cast<uint8_t*>(ep.qs) + static_cast<size_t>(t.s & 1) * bp.q_buf_bytes;
@@ -450,12 +503,12 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
                 const uint32_t taddr = acquire();
                 GDenseEpi::run(ep, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, nullptr, epi_tid);
             } else if (t.type == T_G) {
-                gp.b_off = t.vb0; gp.N = t.Vb_eff;
-                GEpi::Params ep = bp.g;
-                ep.gs += static_cast<size_t>(t.s % bp.gbufs) * bp.planes * ep.plane_stride;
-                GEpi::State st = GEpi::prepare(ep, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
+                gp.b_off = t.vb0; gp.N = t.Vb_eff; gp.row_off = t.s % bp.gbufs;      // ring buffer of this super-tile
+                gp.col_off = half * (BN / 2);                                            // this warp's half of the tile's columns
+                gp.N = BWD_EPI_WARPS == 8 ? BN / 2 : BN;                                 // tile columns this warp handles
+                GEpi::State st = GEpi::prepare(bp.g, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
                 const uint32_t taddr = acquire();
-                GEpi::run(ep, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, nullptr, epi_tid);
+                GEpi::run(bp.g, gp, st, taddr, m_blk, t.n_blk, row_in_tile, t.Tb_eff, P.epi_smem, epi_tid);
             } else if (t.type == T_DX) {
                 gp.N = bp.d; gp.first = (t.vi == 0); gp.last = (t.vi == bp.nvb - 1);
                 DxEpi::State st = DxEpi::prepare(bp.dx, gp, m_blk, t.n_blk, row_in_tile, t.Tb_eff);
@@ -474,22 +527,35 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
 #ifdef OPD_TRACE
             const long long p0 = clock64();
 #endif
-            // publish: all 128 epilogue threads' global stores, then one release increment
-            __threadfence();
-            fence_proxy_async_all();
-            asm volatile("bar.sync 1, 128;" ::: "memory");
-            if (epi_tid == 0) atomicAdd((t.type == T_G ? bp.g_done : (t.type == T_Q ? bp.q_done : bp.c_done)) + t.s, 1);
+            // hand the tile to the publisher warp: this warp's stores are issued (generic) or complete (TMA)
+            hand_over((t.type == T_G ? bp.g_done : (t.type == T_Q ? bp.q_done : (t.type == T_DX ? bp.dx_done : bp.dw_done))) + t.s);
 #ifdef OPD_TRACE
             tr[0] += 1; tr[1] += clock64() - t0; tr[4] += clock64() - p0;
 #endif
         }
 #ifdef OPD_TRACE
-        if (bp.trace && epi_tid == 0) {
+        if (bp.trace && warp == 2 && lane == 0) {
             for (int ty = 0; ty < 4; ++ty) for (int k = 0; k < 8; ++k)
                 if (tre[ty][k]) atomicAdd(bp.trace + (2 * 4 + ty) * 8 + k, (unsigned long long)tre[ty][k]);
             atomicAdd(bp.trace + 96 + 2, (unsigned long long)(clock64() - k0));
         }
 #endif
+    } else {
+        // =========================== publisher (last warp) ===========================
+        // One thread per CTA: when the four epilogue warps are done with a tile, make their stores visible at gpu scope
+        // (the generic-proxy stores of the SM it has observed through the barrier, and the completed bulk stores /
+        // reductions) and count the tile on its dependency counter.  Counters count CTA-level epilogues.
+        if (lane == 0) {
+            for (int n = 0;; ++n) {
+                mbar_wait(&P.pub_full[n % PUB_Q], (n / PUB_Q) & 1);
+                int* counter = *const_cast<int* volatile*>(P.pub_ptr + n % PUB_Q);
+                mbar_arrive(&P.pub_empty[n % PUB_Q]);
+                if (counter == nullptr) break;
+                fence_proxy_async_all();
+                __threadfence();
+                atomicAdd(counter, 1);
+            }
+        }
     }
     P.teardown(warp);
 }

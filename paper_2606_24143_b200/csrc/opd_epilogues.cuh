@@ -25,14 +25,23 @@ __device__ __forceinline__ void add_at32(float (&v)[32], int i, float b) {
 #pragma unroll
     for (int j = 0; j < 32; ++j) v[j] += (i == j) ? b : 0.f;
 }
-// first slot s in the ascending list idx[0..C) with idx[s] >= col  (C <= 64)
+// first slot s in the ascending list idx[0..C) with idx[s] >= col  (C <= 64) = the number of entries below col.
+// Counted over the whole row with independent (vector) loads: one memory latency per tile instead of the log2(C) + 1
+// dependent ones of a binary search (at d <= 2048 the epilogue of a tile has less time than that took).
 __device__ __forceinline__ int lower_bound_slot(const int* __restrict__ idx, int C, int col) {
-    int lo = 0, hi = C;
-    while (lo < hi) {
-        const int mid = (lo + hi) >> 1;
-        if (__ldg(idx + mid) < col) lo = mid + 1; else hi = mid;
+    int n = 0;
+    if ((C & 3) == 0) {
+        const int4* q = reinterpret_cast<const int4*>(idx);       // rows of [T][C] int32 are 16-byte aligned when C % 4 == 0
+#pragma unroll 4
+        for (int j = 0; j < C / 4; ++j) {
+            const int4 e = __ldg(q + j);
+            n += (e.x < col) + (e.y < col) + (e.z < col) + (e.w < col);
+        }
+    } else {
+#pragma unroll 4
+        for (int j = 0; j < C; ++j) n += __ldg(idx + j) < col;
     }
-    return lo;
+    return n;
 }
 
 struct NoState {};
@@ -73,15 +82,16 @@ struct FwdEpi {
         int V;
         float* dbg_logits;       // optional [T][V] dump (opd_debug_logits)
     };
-    struct State { int cursor; int next_col; };
+    struct State { int cursor; int next_col; int col_b; };      // col_b: the cached column after next_col (prefetched)
     static __device__ __forceinline__ State prepare(const Params& p, const GemmParams& gp, int m_blk, int n_blk,
                                                     int row_in_tile, int M_eff) {
-        State st{p.C, IDX_SENTINEL};
+        State st{p.C, IDX_SENTINEL, IDX_SENTINEL};
         const int row = m_blk * BM + row_in_tile;
         if (row < M_eff) {
             const int* idx = p.sorted_idx + static_cast<size_t>(row) * p.C;
             st.cursor = lower_bound_slot(idx, p.C, n_blk * BN);
             st.next_col = st.cursor < p.C ? __ldg(idx + st.cursor) : IDX_SENTINEL;
+            st.col_b = st.cursor + 1 < p.C ? __ldg(idx + st.cursor + 1) : IDX_SENTINEL;
         }
         return st;
     }
@@ -102,7 +112,8 @@ struct FwdEpi {
                 while (st.next_col < col0 + 32) {                    // cached column inside this chunk
                     p.zc[static_cast<size_t>(row) * p.C + st.cursor] = select32(v, st.next_col - col0);
                     ++st.cursor;
-                    st.next_col = st.cursor < p.C ? __ldg(idx + st.cursor) : IDX_SENTINEL;
+                    st.next_col = st.col_b;                           // the load below is only waited for at a later hit
+                    st.col_b = st.cursor + 1 < p.C ? __ldg(idx + st.cursor + 1) : IDX_SENTINEL;
                 }
             }
             if (p.dbg_logits != nullptr && live) {

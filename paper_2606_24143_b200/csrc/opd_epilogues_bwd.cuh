@@ -9,14 +9,56 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
     return *reinterpret_cast<uint32_t*>(&t);
 }
 
+// Software-pipelined walk over a tile's accumulator: the TMEM load of chunk c + 1 (32 fp32 columns of this thread's row) is
+// in flight while body(v, c) works on chunk c.  TMEM reads run at 64 B per cycle and SM (B300_MICROARCH.md: 4 KiB per
+// warp-wide tcgen05.ld), so a load that is waited for at once costs every chunk 60-250 cycles of idle epilogue warp.
+// nchunks is warp-uniform; every load issued has been waited for when this returns.
+template <class F>
+__device__ __forceinline__ void for_each_chunk(uint32_t taddr, int nchunks, F&& body, long long* tr = nullptr) {
+    float va[32], vb[32];
+    if (nchunks <= 0) return;
+    tmem_ld32(taddr, va);
+#ifdef OPD_TRACE
+    long long t0 = clock64(), t1;
+#define OPD_TR_STEP(slot) if (tr) { t1 = clock64(); tr[slot] += t1 - t0; t0 = t1; }
+#else
+#define OPD_TR_STEP(slot)
+#endif
+#pragma unroll 1
+    for (int c = 0; c < nchunks; c += 2) {
+        tmem_ld_wait_for(va);
+        if (c + 1 < nchunks) tmem_ld32(taddr + (c + 1) * 32, vb);
+        OPD_TR_STEP(6)
+        body(va, c);
+        OPD_TR_STEP(7)
+        if (c + 1 < nchunks) {
+            tmem_ld_wait_for(vb);
+            if (c + 2 < nchunks) tmem_ld32(taddr + (c + 2) * 32, va);
+            OPD_TR_STEP(6)
+            body(vb, c + 1);
+            OPD_TR_STEP(7)
+        }
+    }
+#undef OPD_TR_STEP
+}
+
 // ------------------------------------------------------------------------------------------ GEpi
 // S6: re-form G[t,v] = coef_t * exp(z[t,v] - lse_t) + sum_j beta_tj [a_tj == v]  with coef = alpha/N,
 // beta pre-scaled by 1/N (derivation: DESIGN.md "Backward"), round to bf16 and store it into the
 // super-tile Gs[Tb][ldg] (row-major, v contiguous) that the dX and dW contractions read back from L2.
 // Rows past the live count and columns past V are written as zeros: both contractions rely on it.
+// Per element: one FFMA and one MUFU.EX2 -- the coefficient is folded into the exponent,
+//     coef * 2^(z log2e - lse2) = sign(coef) * 2^(z log2e - (lse2 - log2|coef|)),
+// its sign is an XOR on the packed bf16 pair (beta is added in the sign-folded domain), coef = 0 and dead rows give
+// 2^-inf = +0 without a branch.  Each thread stores its row's 64 bytes per chunk as two 32-byte stores (whole sectors).
+// These row-per-thread stores are what bounds this epilogue (one LSU wavefront per sector, about 4000 cycles per tile);
+// staging the tile through shared memory for TMA stores has a quarter of the wavefronts but puts the completion wait of the
+// last store on every tile and measured no faster (profiles/r02_trace.md).
+// The cached columns of the row are found in prepare() with one pass of vector loads and the next two are kept in
+// registers, so that a hit inside a chunk costs no memory latency.
 struct GEpi {
     struct Params {
-        __nv_bfloat16* gs;       // [planes][rows][ldg]
+        __nv_bfloat16* gs;       // ring buffer 0: [planes][rows][ldg]
         int rows;                // allocated rows per plane (tile rows past it are not stored)
         long ldg;
         long plane_stride;       // elements
@@ -27,49 +69,49 @@ struct GEpi {
         const float* beta;       // [T][C] beta_tj / N in sorted-slot order
         int C;
         int V;
-        unsigned long long st_hint;   // L2 eviction policy of the G stores (0 = plain stores)
+        unsigned long long st_hint;   // L2 eviction policy of the G stores (0 = normal)
     };
-    struct State { int cursor; int next_col; float lse2; float coef; };
+    // next_col / beta_a: the row's next cached column at or after this tile and its coefficient; col_b / beta_b: the one after
+    struct State { int cursor; int next_col; int col_b; float beta_a; float beta_b; float off; uint32_t sgn; };
     static __device__ __forceinline__ State prepare(const Params& p, const GemmParams& gp, int m_blk, int n_blk,
                                                     int row_in_tile, int M_eff) {
-        State st{p.C, IDX_SENTINEL, 0.f, 0.f};
+        State st{p.C, IDX_SENTINEL, IDX_SENTINEL, 0.f, 0.f, INFINITY, 0u};
         const int lrow = m_blk * BM + row_in_tile;
         if (lrow < M_eff) {
             const int row = gp.tok_off + lrow;
             const int* idx = p.sorted_idx + static_cast<size_t>(row) * p.C;
-            st.cursor = lower_bound_slot(idx, p.C, gp.b_off + n_blk * BN);
-            st.next_col = st.cursor < p.C ? __ldg(idx + st.cursor) : IDX_SENTINEL;
-            st.lse2 = p.lse2[row];
-            st.coef = p.coef[row];
+            const float* beta = p.beta + static_cast<size_t>(row) * p.C;
+            st.cursor = lower_bound_slot(idx, p.C, gp.b_off + n_blk * BN + gp.col_off);
+            if (st.cursor < p.C) { st.next_col = __ldg(idx + st.cursor); st.beta_a = __ldg(beta + st.cursor); }
+            if (st.cursor + 1 < p.C) { st.col_b = __ldg(idx + st.cursor + 1); st.beta_b = __ldg(beta + st.cursor + 1); }
+            const float coef = p.coef[row];
+            st.off = p.lse2[row] - log2f(fabsf(coef));              // coef == 0: +inf, the row's softmax part is +0
+            st.sgn = coef < 0.f ? 0x80008000u : 0u;
         }
         return st;
     }
+    // gp.row_off: ring buffer of this super-tile; gp.col_off, gp.N: first and number of the tile columns this warp handles
     static __device__ __forceinline__ void run(const Params& p, const GemmParams& gp, State st, uint32_t taddr,
-                                               int m_blk, int n_blk, int row_in_tile, int M_eff, uint8_t*, int) {
+                                               int m_blk, int n_blk, int row_in_tile, int, uint8_t*, int) {
         const int lrow = m_blk * BM + row_in_tile;
-        const bool live = lrow < M_eff;
         const int row = gp.tok_off + lrow;
-        const int* idx = p.sorted_idx + static_cast<size_t>(row) * p.C;
+        const int* idx = p.sorted_idx + static_cast<size_t>(row) * p.C;          // dereferenced on live rows only (cursor < C)
         const float* beta = p.beta + static_cast<size_t>(row) * p.C;
-        __nv_bfloat16* out = p.gs + static_cast<size_t>(lrow) * p.ldg + n_blk * BN;
-#pragma unroll 1
-        for (int c = 0; c < BN / 32; ++c) {
-            float v[32];
-            tmem_ld32(taddr + c * 32, v);
-            tmem_ld_wait();
-            const int col0 = gp.b_off + n_blk * BN + c * 32;          // vocabulary column of v[0]
-            if (live) {
+        const float sgnf = st.sgn ? -1.f : 1.f;
+        __nv_bfloat16* out = p.gs + static_cast<size_t>(gp.row_off) * p.planes * p.plane_stride + static_cast<size_t>(lrow) * p.ldg +
+                             n_blk * BN + gp.col_off;
+        for_each_chunk(taddr + gp.col_off, gp.N / 32, [&](float (&v)[32], int c) {
+            const int col0 = gp.b_off + n_blk * BN + gp.col_off + c * 32;   // vocabulary column of v[0]
 #pragma unroll
-                for (int i = 0; i < 32; ++i) v[i] = st.coef * exp2f(fmaf(v[i], LOG2E, -st.lse2));
-            } else {
-#pragma unroll
-                for (int i = 0; i < 32; ++i) v[i] = 0.f;
-            }
+            for (int i = 0; i < 32; ++i) v[i] = ex2_approx(fmaf(v[i], LOG2E, -st.off));
             if (__any_sync(0xffffffffu, st.next_col < col0 + 32)) {
                 while (st.next_col < col0 + 32) {                    // duplicates add up
-                    add_at32(v, st.next_col - col0, __ldg(beta + st.cursor));
+                    add_at32(v, st.next_col - col0, sgnf * st.beta_a);
                     ++st.cursor;
-                    st.next_col = st.cursor < p.C ? __ldg(idx + st.cursor) : IDX_SENTINEL;
+                    st.next_col = st.col_b; st.beta_a = st.beta_b;    // the loads below are only waited for at a later hit
+                    const bool more = st.cursor + 1 < p.C;
+                    st.col_b = more ? __ldg(idx + st.cursor + 1) : IDX_SENTINEL;
+                    st.beta_b = more ? __ldg(beta + st.cursor + 1) : 0.f;
                 }
             }
             if (col0 + 32 > p.V) {
@@ -77,7 +119,17 @@ struct GEpi {
                 for (int i = 0; i < 32; ++i)
                     if (col0 + i >= p.V) v[i] = 0.f;
             }
-            if (lrow >= p.rows) continue;                             // row of a pair tile past the buffer
+            if (lrow >= p.rows) return;                               // rows of a pair tile past the buffer are not stored
+            if (p.planes == 1 && !p.st_hint) {                        // bf16 path: 64 bytes of this row, two 32-byte stores
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    uint32_t o[8];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) o[i] = pack_bf16x2(v[16 * q + 2 * i], v[16 * q + 2 * i + 1]) ^ st.sgn;
+                    st_global_v8(out + c * 32 + 16 * q, o);
+                }
+                return;
+            }
             for (int pl = 0; pl < p.planes; ++pl) {
                 uint32_t w[16];
 #pragma unroll
@@ -89,16 +141,19 @@ struct GEpi {
                         v[2 * i + 1] -= __high2float(t);
                     }
                 }
+                // the sign of coef goes onto the packed pairs (the residuals above were taken in the sign-folded domain)
                 uint4* dst = reinterpret_cast<uint4*>(out + pl * p.plane_stride + c * 32);
-                if (p.st_hint) {
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) st_global_v4_hint(dst + q, w[4 * q], w[4 * q + 1], w[4 * q + 2], w[4 * q + 3], p.st_hint);
-                } else {
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) dst[q] = make_uint4(w[4 * q], w[4 * q + 1], w[4 * q + 2], w[4 * q + 3]);
+                for (int q = 0; q < 4; ++q) {
+                    if (p.st_hint) st_global_v4_hint(dst + q, w[4 * q] ^ st.sgn, w[4 * q + 1] ^ st.sgn, w[4 * q + 2] ^ st.sgn, w[4 * q + 3] ^ st.sgn, p.st_hint);
+                    else dst[q] = make_uint4(w[4 * q] ^ st.sgn, w[4 * q + 1] ^ st.sgn, w[4 * q + 2] ^ st.sgn, w[4 * q + 3] ^ st.sgn);
                 }
             }
-        }
+#ifdef OPD_TRACE
+        }, gp.tr);
+#else
+        });
+#endif
     }
 };
 
@@ -161,19 +216,15 @@ struct DxEpi {
         const int lane = epi_tid & 31;
         uint8_t* wbuf = epi_smem + (epi_tid >> 5) * 8192;
         const float* acc = p.acc + static_cast<size_t>(lrow) * p.ld_acc + n_blk * BN;
-#pragma unroll 1
-        for (int c = 0; c < BN / 32; ++c) {
-            float v[32];
-            tmem_ld32(taddr + c * 32, v);
-            tmem_ld_wait();
-            const int col0 = n_blk * BN + c * 32;
-            if (col0 >= gp.N) break;                                  // d % 64 == 0: chunks are all-in or all-out (warp-uniform)
+        const int nchunks = min(BN / 32, (gp.N - n_blk * BN + 31) / 32);      // d % 64 == 0: chunks are all-in or all-out (warp-uniform)
 #ifdef OPD_EXPERIMENTS
-            if (p.dbg == 2) continue;
-            const bool reduce = !gp.first && p.dbg != 1;
+        if (p.dbg == 2) return;
+        const bool reduce = !gp.first && p.dbg != 1;
 #else
-            const bool reduce = !gp.first;
+        const bool reduce = !gp.first;
 #endif
+        for_each_chunk(taddr, nchunks, [&](float (&v)[32], int c) {
+            const int col0 = n_blk * BN + c * 32;
             if (!gp.last) {
                 stage_and_send(&p.m_acc, wbuf, c & 1, v, lane, col0, lrow - lane, reduce, p.hint);
             } else if (live) {
@@ -197,7 +248,7 @@ struct DxEpi {
                                            pack_bf16x2(v[8 * q + 4], v[8 * q + 5]), pack_bf16x2(v[8 * q + 6], v[8 * q + 7]));
                 }
             }
-        }
+        });
         if (!gp.last) drain_sends(lane);
     }
 };
@@ -223,21 +274,16 @@ struct DwEpi {
         uint8_t* wbuf = epi_smem + (epi_tid >> 5) * 8192;
         const int lrow0 = m_blk * BM + row_in_tile - lane;           // first tile row of this warp
         const bool warp_ok = lrow0 < M_eff;                          // extents are multiples of 32 except at tensor edges (clipped)
-#pragma unroll 1
-        for (int c = 0; c < BN / 32; ++c) {
-            float v[32];
-            tmem_ld32(taddr + c * 32, v);
-            tmem_ld_wait();
-            const int lc0 = n_blk * BN + c * 32;
-            if (lc0 >= gp.N) break;
+        const int nchunks = min(BN / 32, (gp.N - n_blk * BN + 31) / 32);
 #ifdef OPD_EXPERIMENTS
-            if (p.dbg == 2) continue;
-            const bool reduce = !gp.first && p.dbg != 1;
+        if (p.dbg == 2) return;
+        const bool reduce = !gp.first && p.dbg != 1;
 #else
-            const bool reduce = !gp.first;      // first token super-tile of an overwriting call: plain store
+        const bool reduce = !gp.first;      // first token super-tile of an overwriting call: plain store
 #endif
-            if (warp_ok) stage_and_send(&p.m_gw, wbuf, c & 1, v, lane, gp.col_off + lc0, gp.row_off + lrow0, reduce, p.hint);
-        }
+        for_each_chunk(taddr, nchunks, [&](float (&v)[32], int c) {
+            if (warp_ok) stage_and_send(&p.m_gw, wbuf, c & 1, v, lane, gp.col_off + n_blk * BN + c * 32, gp.row_off + lrow0, reduce, p.hint);
+        });
         drain_sends(lane);
     }
 };

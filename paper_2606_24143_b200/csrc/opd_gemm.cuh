@@ -23,6 +23,14 @@ constexpr int UMMA_K = 16;
 constexpr int MN_BOX = 64;                            // MN-major operands arrive as 64(mn) x 64(k) boxes
 constexpr int MN_BOX_BYTES = MN_BOX * BK * 2;         // 8 KiB
 constexpr int GEMM_THREADS = 192;                     // warp0 TMA, warp1 MMA(+TMEM alloc), warps2-5 epilogue
+#ifndef OPD_BWD_EPI_WARPS
+#define OPD_BWD_EPI_WARPS 4
+#endif
+constexpr int BWD_EPI_WARPS = OPD_BWD_EPI_WARPS;                      // bwd_kernel: two epilogue warps per TMEM lane quarter (each takes half the
+                                                      // columns of a G tile: with one warp per scheduler nothing overlaps the
+                                                      // TMEM reads, MUFU latency and scattered row stores of that warp)
+constexpr int BWD_THREADS = (2 + BWD_EPI_WARPS + 1) * 32;   // + the publisher of finished tiles (last warp)
+constexpr int PUB_Q = 4;                              // tiles the epilogue warps may run ahead of the publisher
 constexpr int EPI_SMEM_BYTES = 32768;                 // 4 epilogue warps x 2 staging buffers x (32 rows x 128 B)
 constexpr int TMEM_COLS = 512;                        // 2 accumulator stages x 256 columns
 constexpr int MAX_STAGES = 6;
@@ -40,6 +48,7 @@ constexpr int MAX_STAGES = 6;
 constexpr int SCHED_Q = 8;                 // depth of the tile queue of the dynamically scheduled kernels
 constexpr int SCHED_WORDS = 12;            // 32-bit words of one decoded tile descriptor in the queue (48 bytes)
 
+static_assert(256 + 2 * SCHED_Q * 8 + SCHED_Q * SCHED_WORDS * 4 <= 768 && 768 + 2 * PUB_Q * 8 + PUB_Q * 8 <= 1024, "barrier region is 1 KiB");
 template <int CG> __host__ __device__ constexpr int fwd_stages() { return CG == 1 ? 4 : OPD_FWD_STAGES; }
 template <int CG> __host__ __device__ constexpr int bwd_stages() { return CG == 1 ? 4 : OPD_BWD_STAGES; }
 
@@ -74,6 +83,9 @@ struct GemmParams {
     unsigned long long a_hint, b_hint;   // L2 eviction policy of the operand loads (0 = normal)
     int first, last;          // DxEpi: first / last vocabulary super-tile of this token super-tile
     int row_off, col_off;     // DwEpi: position of this GEMM's output inside grad_W
+#ifdef OPD_TRACE
+    long long* tr;            // tracing builds: cycle sums of the epilogue that runs this tile (slot 6: TMEM waits, 7: chunk bodies)
+#endif
 };
 
 __device__ __forceinline__ void tile_coords(int tile, int num_m, int num_n, int group_m, int& m_blk, int& n_blk) {
@@ -99,12 +111,14 @@ struct Pipe {
     uint64_t *full_bar, *empty_bar, *tfull_bar, *tempty_bar;
     uint64_t *sfull_bar, *sempty_bar;     // tile queue (bwd_kernel): slot q published / consumed by every reader
     uint32_t* sticket;                    // [SCHED_Q][SCHED_WORDS] decoded tiles (a copy in each CTA of a pair)
+    uint64_t *pub_full, *pub_empty;       // publisher queue (bwd_kernel): the 4 epilogue warps are done with tile n / slot reusable
+    int** pub_ptr;                        // [PUB_Q] dependency counter the publisher increments for that tile (null: stop)
     uint32_t* tmem_slot;
     uint8_t* epi_smem;
     uint32_t tmem_base;
     uint32_t rank;            // CTA rank in the pair (0 = leader; always 0 for CG = 1)
 
-    __device__ __forceinline__ void setup(uint8_t* smem_raw, int warp, int lane) {
+    __device__ __forceinline__ void setup(uint8_t* smem_raw, int warp, int lane, int epi_warps = 4) {
         smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
         full_bar = reinterpret_cast<uint64_t*>(smem + C::RING_BYTES);
         empty_bar = full_bar + MAX_STAGES;
@@ -114,15 +128,19 @@ struct Pipe {
         sfull_bar = reinterpret_cast<uint64_t*>(smem + C::RING_BYTES + 256);
         sempty_bar = sfull_bar + SCHED_Q;
         sticket = reinterpret_cast<uint32_t*>(sempty_bar + SCHED_Q);
+        pub_full = reinterpret_cast<uint64_t*>(smem + C::RING_BYTES + 768);
+        pub_empty = pub_full + PUB_Q;
+        pub_ptr = reinterpret_cast<int**>(pub_empty + PUB_Q);
         epi_smem = smem + C::RING_BYTES + 1024;
         rank = CG == 1 ? 0u : cluster_ctarank();
         if (warp == 0 && lane == 0) {
             for (int s = 0; s < C::STAGES; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
-            for (int s = 0; s < 2; ++s) { mbar_init(&tfull_bar[s], 1); mbar_init(&tempty_bar[s], 4 * CG); }
-            // readers of a ticket.  CG = 1: the MMA issuer and the 4 epilogue warps (the producer claims).  CG = 2: both
-            // producers, the MMA issuer and the 8 epilogue warps of the pair (the peer CTA's otherwise idle warp 1 claims,
+            for (int s = 0; s < 2; ++s) { mbar_init(&tfull_bar[s], 1); mbar_init(&tempty_bar[s], epi_warps * CG); }
+            // readers of a ticket.  CG = 1: the MMA issuer and the epilogue warps (the producer claims).  CG = 2: both
+            // producers, the MMA issuer and the epilogue warps of both CTAs of the pair (the peer CTA's otherwise idle warp 1 claims,
             // so that the round trip of the claim never sits between two tiles of the producer)
-            for (int s = 0; s < SCHED_Q; ++s) { mbar_init(&sfull_bar[s], 1); mbar_init(&sempty_bar[s], CG == 1 ? 5 : 11); }
+            for (int s = 0; s < SCHED_Q; ++s) { mbar_init(&sfull_bar[s], 1); mbar_init(&sempty_bar[s], CG == 1 ? 1 + epi_warps : 3 + 2 * epi_warps); }
+            for (int s = 0; s < PUB_Q; ++s) { mbar_init(&pub_full[s], epi_warps); mbar_init(&pub_empty[s], 1); }
             fence_mbar_init();
         }
         if (warp == 1) {

@@ -182,7 +182,7 @@ inline Plan make_plan_cfg(int T, int d, int V, int C, int fp32, unsigned flags, 
     p.gs_plane = (size_t)p.Tb * p.Vb;
     p.gs_bufs = std::min(3, std::max(2, gbufs));
     p.n_super = ceil_div(p.t_pad, p.Tb) * ceil_div(V, p.Vb);
-    p.off_counters = take(bwd ? sizeof(int) * (2 * (size_t)p.n_super + 1) : 0);      // g_done, c_done, tile ticket
+    p.off_counters = take(bwd ? sizeof(int) * (3 * (size_t)p.n_super + 1) : 0);      // g_done, dx_done, dw_done, tile ticket
     // The per-tile LSE partials are dead once the estimators have run, the G ring and the grad_hidden partial
     // sums only live in the backward: they share one region.
     const size_t partial_bytes = align_up(sizeof(float2) * (size_t)p.num_n * p.t_pad, 1024);
@@ -224,15 +224,15 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int 
 }
 
 // ---------------------------------------------------------------- GEMM launcher
-// Launch `kernel` on `grid` CTAs of GEMM_THREADS threads; CG = 2 launches clusters of two CTAs (a pair per tile).
+// Launch `kernel` on `grid` CTAs of `threads` threads; CG = 2 launches clusters of two CTAs (a pair per tile).
 // `window` (optional): an L2 access-policy window for this launch only (persisting hits inside [base, base + bytes)).
 struct L2Window { void* base = nullptr; size_t bytes = 0; float hit_ratio = 1.f; };
 template <int CG, int ST, class... KArgs, class... Args>
-inline cudaError_t launch_cg_w(void (*kernel)(KArgs...), int grid, cudaStream_t st, const L2Window& window, Args&&... args) {
+inline cudaError_t launch_cg_w(void (*kernel)(KArgs...), int grid, int threads, cudaStream_t st, const L2Window& window, Args&&... args) {
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<CG, ST>::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(GEMM_THREADS); cfg.dynamicSmemBytes = Cfg<CG, ST>::SMEM_BYTES; cfg.stream = st;
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = Cfg<CG, ST>::SMEM_BYTES; cfg.stream = st;
     cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
@@ -250,16 +250,16 @@ inline cudaError_t launch_cg_w(void (*kernel)(KArgs...), int grid, cudaStream_t 
 }
 template <int CG, int ST, class... KArgs, class... Args>
 inline cudaError_t launch_cg(void (*kernel)(KArgs...), int grid, cudaStream_t st, Args&&... args) {
-    return launch_cg_w<CG, ST>(kernel, grid, st, L2Window{}, std::forward<Args>(args)...);
+    return launch_cg_w<CG, ST>(kernel, grid, GEMM_THREADS, st, L2Window{}, std::forward<Args>(args)...);
 }
 
 // Number of clusters (CG = 2) / CTAs (CG = 1) of `kernel` that can be resident at the same time on the current device:
 // the persistent kernels size their grid with it (one wave; more CTAs would only queue behind the resident ones).
 template <int CG, int ST, class... KArgs>
-inline int max_resident_groups(void (*kernel)(KArgs...), int num_sms) {
+inline int max_resident_groups(void (*kernel)(KArgs...), int num_sms, int threads) {
     if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<CG, ST>::SMEM_BYTES) != cudaSuccess) return 0;
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(num_sms / CG * CG); cfg.blockDim = dim3(GEMM_THREADS); cfg.dynamicSmemBytes = Cfg<CG, ST>::SMEM_BYTES;
+    cfg.gridDim = dim3(num_sms / CG * CG); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = Cfg<CG, ST>::SMEM_BYTES;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CG; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;

@@ -26,7 +26,7 @@ static DensePlan make_dense_plan(int T, int d, int dT, int V, int fp32, unsigned
     p.off_acc_a = take(sizeof(float) * (size_t)p.base.t_pad);
     p.off_acc_b = take(sizeof(float) * (size_t)p.base.t_pad);
     p.off_lt = take(sizeof(float) * (size_t)p.base.t_pad);
-    p.off_qdone = take(sizeof(int) * (3 * (size_t)p.base.n_super + 1));      // q_done, g_done, c_done, tile ticket
+    p.off_qdone = take(sizeof(int) * (4 * (size_t)p.base.n_super + 1));      // q_done, g_done, dx_done, dw_done, tile ticket
     p.total = o;
     return p;
 }
@@ -180,10 +180,11 @@ extern "C" opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, 
     int* counters = q_done + p.n_super;
     BwdParams bp{};
     bp.d = d; bp.V = V; bp.Tb = p.Tb; bp.Vb = p.Vb; bp.nvb = ceil_div(V, p.Vb); bp.wl = wl; bp.planes = p.planes; bp.gbufs = p.gs_bufs;
-    bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super; bp.q_done = q_done;
-    bp.ticket = counters + 2 * p.n_super;
+    bp.n_live = n_live; bp.g_done = counters; bp.dx_done = counters + p.n_super; bp.dw_done = counters + 2 * p.n_super; bp.q_done = q_done;
+    bp.ticket = counters + 3 * p.n_super;
     bp.dw_store_first = (flags & OPD_F_GRADW_ACCUM) ? 0 : 1;
     bp.dx_group = p.Vb > 4096 ? 8 : 0;
+    bp.q_depth = std::min(SCHED_Q, std::max(1, env_int("OPD_Q_DEPTH", 3)));
     bp.dx = dxp; bp.dw = dwp;
     bp.hint_x = bp.hint_w = bp.hint_g = L2_EVICT_NORMAL;
     bp.dT = dT; bp.wl_t = wlt; bp.qbytes = q32 ? 4 : 2; bp.q_buf_bytes = dp.q_buf_bytes;
@@ -192,7 +193,7 @@ extern "C" opd_status_t opd_dense_kl_fwd_bwd(opd_handle_t h, void* cuda_stream, 
                               reverse ? 1 : 0, nullptr};
     const int fwd_types = (1 << T_Q) | (1 << T_G);
     auto launch = [&](int type_mask) -> opd_status_t {
-        OPD_CUDA(h, cudaMemsetAsync(q_done, 0, sizeof(int) * (3 * (size_t)p.n_super + 1), st));
+        OPD_CUDA(h, cudaMemsetAsync(q_done, 0, sizeof(int) * (4 * (size_t)p.n_super + 1), st));
         bp.type_mask = type_mask;
         opd_status_t ls = launch_bwd<true>(h, st, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp);
         if (ls == OPD_OK) { h->n_kernels++; h->n_gemm++; }

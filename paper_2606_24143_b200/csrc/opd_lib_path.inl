@@ -26,15 +26,15 @@ static opd_status_t launch_bwd(opd_handle_s* h, cudaStream_t st, const CUtensorM
                                const L2Window& win = L2Window{}) {
     int& cached = h->bwd_grid[h->cg][DENSE ? 1 : 0];      // per handle = per device; a failed query is not cached
     if (cached < 1) {
-        const int r = h->cg == 2 ? max_resident_groups<2, bwd_stages<2>()>(bwd_kernel<2, DENSE>, h->num_sms)
-                                 : max_resident_groups<1, bwd_stages<1>()>(bwd_kernel<1, DENSE>, h->num_sms);
+        const int r = h->cg == 2 ? max_resident_groups<2, bwd_stages<2>()>(bwd_kernel<2, DENSE>, h->num_sms, BWD_THREADS)
+                                 : max_resident_groups<1, bwd_stages<1>()>(bwd_kernel<1, DENSE>, h->num_sms, BWD_THREADS);
         if (r < 1) OPD_FAIL(h, OPD_ERR_CUDA, "the backward kernel cannot be made resident on device %d", h->device);
         cached = r * h->cg;
     }
     const int grid = cached;
     constexpr int S2 = bwd_stages<2>(), S1 = bwd_stages<1>();
-    if (h->cg == 2) OPD_CUDA(h, (launch_cg_w<2, S2>)(bwd_kernel<2, DENSE>, grid, st, win, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
-    else OPD_CUDA(h, (launch_cg_w<1, S1>)(bwd_kernel<1, DENSE>, grid, st, win, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
+    if (h->cg == 2) OPD_CUDA(h, (launch_cg_w<2, S2>)(bwd_kernel<2, DENSE>, grid, BWD_THREADS, st, win, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
+    else OPD_CUDA(h, (launch_cg_w<1, S1>)(bwd_kernel<1, DENSE>, grid, BWD_THREADS, st, win, m_xc_k, m_w_fwd, m_gs_k, m_w_dx, m_xc_mn, m_gs_mn, m_tx_k, m_wt_fwd, bp));
     return OPD_OK;
 }
 
@@ -276,12 +276,14 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         // one persistent kernel walks every super-tile: G re-formation, grad_hidden and grad_W tiles interleaved,
         // ordered by dependency counters in global memory (opd_bwd_kernel.cuh)
         int* counters = reinterpret_cast<int*>(ws + p.off_counters);
-        OPD_CUDA(h, cudaMemsetAsync(counters, 0, sizeof(int) * (2 * (size_t)p.n_super + 1), st));
+        OPD_CUDA(h, cudaMemsetAsync(counters, 0, sizeof(int) * (3 * (size_t)p.n_super + 1), st));
         BwdParams bp{};
         bp.d = d; bp.V = V; bp.Tb = p.Tb; bp.Vb = p.Vb; bp.nvb = ceil_div(V, p.Vb); bp.wl = wl; bp.planes = p.planes; bp.gbufs = p.gs_bufs;
-        bp.n_live = n_live; bp.g_done = counters; bp.c_done = counters + p.n_super; bp.ticket = counters + 2 * p.n_super;
+        bp.n_live = n_live; bp.g_done = counters; bp.dx_done = counters + p.n_super; bp.dw_done = counters + 2 * p.n_super;
+        bp.ticket = counters + 3 * p.n_super;
         bp.dw_store_first = gw_accum ? 0 : 1;
         bp.order = env_int("OPD_BWD_ORDER", 0) & 31;
+        bp.q_depth = std::min(SCHED_Q, std::max(1, env_int("OPD_Q_DEPTH", 3)));
         // super-tiles wider than 4096 columns: grad_hidden tiles in groups of 8 row tiles (10 GB fewer G re-reads per C4 launch)
         bp.dx_group = env_int("OPD_DX_GROUP", p.Vb > 4096 ? 8 : 0);
         bp.g = GEpi::Params{gs, p.Tb, (long)p.Vb, (long)p.gs_plane, p.planes, lse2, coef, sorted_idx, beta, C, V, 0ull};
@@ -336,8 +338,8 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
             for (int r = 0; r < 3; ++r) for (int ty = 0; ty < 4; ++ty) {
                 const unsigned long long* v = tb + (r * 4 + ty) * 8;
                 if (!v[0]) continue;
-                std::fprintf(stderr, "[opd trace] %s %-2s n=%llu total=%llu s2=%llu s3=%llu s4=%llu s5=%llu s6=%llu\n", roles[r], types[ty],
-                             v[0], v[1], v[2], v[3], v[4], v[5], v[6]);
+                std::fprintf(stderr, "[opd trace] %s %-2s n=%llu total=%llu s2=%llu s3=%llu s4=%llu s5=%llu s6=%llu s7=%llu\n", roles[r], types[ty],
+                             v[0], v[1], v[2], v[3], v[4], v[5], v[6], v[7]);
             }
         }
 #endif
