@@ -17,6 +17,10 @@ Recipe (shapes from BASELINE.json configs):
   top-k cache    idx = TopK(log q, k) chosen by the teacher, lam = log q[idx]
   MC cache       idx = a, lam = log q[a], old = log p_old[a]
   stale top-k    idx = TopK(log p_old, k) (the rollout-time student support S_old), lam = log q[idx]
+Stress variants (reported / tested, not bench configs): cfg["hidden_scale"] = 4 gives PEAKED rows (logits of
+standard deviation 4: a few columns hold most of the mass, most exponentials are tiny); cfg["order"] = "monotone" scales
+column v of the student heads by 0.5 + 1.5 v/V, so column norms grow with the index and the running maximum of a row keeps
+moving to later vocabulary tiles (online-max rescaling); a large sigma gives heavy importance-ratio tails.
 All cache values are fp32, indices int32.  Rollout settings follow PAPER.md:332 (temperature 1,
 no truncation).  These are stand-ins for the paper's Qwen3 workloads: V=151936 and
 d in {2048,2560,4096} are the 1.7B/4B/8B-class student heads.
@@ -92,14 +96,20 @@ def make_inputs(cfg: dict, c: int = 0, device="cpu", keep_teacher_rows: bool = F
     dt = _tdtype(cfg["dtype"])
     dev = torch.device(device)
     s = SEED0 + 1000 * c
-    hidden = torch.randn(T, d, generator=_gen(s + 0, dev), device=dev, dtype=torch.float32).to(dt)
+    hidden = (torch.randn(T, d, generator=_gen(s + 0, dev), device=dev, dtype=torch.float32) * float(cfg.get("hidden_scale", 1.0))).to(dt)
     W32 = torch.randn(d, V, generator=_gen(s + 1, dev), device=dev, dtype=torch.float32) * (d ** -0.5)
+    ramp = None
+    if cfg.get("order") == "monotone":
+        ramp = 0.5 + 1.5 * torch.arange(V, device=dev, dtype=torch.float32) / V
+        W32 = W32 * ramp
     W = W32.to(dt)
     WT = (torch.randn(d, V, generator=_gen(s + 2, dev), device=dev, dtype=torch.float32) * (d ** -0.5)).to(dt)
     if sig == 0:
         Wold = W
     else:
         E = torch.randn(d, V, generator=_gen(s + 3, dev), device=dev, dtype=torch.float32) * (d ** -0.5)
+        if ramp is not None:
+            E = E * ramp
         Wold = (W32 + sig * E).to(dt)
         del E
     del W32

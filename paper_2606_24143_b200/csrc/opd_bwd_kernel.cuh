@@ -208,8 +208,8 @@ bwd_kernel(const __grid_constant__ CUtensorMap m_xc_k, const __grid_constant__ C
 
     // segment tables of the three-term split (planes == 3), see set_segments()
     const int nseg = bp.planes == 1 ? 1 : 6;
-    const int PA[6] = {0, 0, 1, 0, 2, 1};
-    const int PB[6] = {0, 1, 0, 2, 0, 1};
+    const int PA[6] = {1, 2, 0, 1, 0, 0};      // smallest products first (set_segments)
+    const int PB[6] = {1, 0, 2, 0, 1, 0};
 
     // ---- tile queue.  The claimer takes the next item of the list, decodes it (BwdSched: the integer divisions live here)
     // and publishes the decoded tile; every other role copies 48 bytes out of shared memory.

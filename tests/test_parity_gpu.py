@@ -119,6 +119,30 @@ def test_ragged_shapes_and_super_tiles(handle, dtype, mode, tiles, monkeypatch):
         assert handle.launch_stats()["super_rows"] == tiles[0]
 
 
+STRESS = {
+    "peaked": dict(hidden_scale=4.0, sigma=0.05),                   # a few columns hold the mass, most exponentials are tiny
+    "monotone": dict(order="monotone", sigma=0.05),                 # the row maximum keeps moving to later vocabulary tiles
+    "peaked_monotone_stale": dict(hidden_scale=3.0, order="monotone", sigma=0.3),   # + heavy tails of rho = p_theta / p_old
+}
+
+
+@pytest.mark.parametrize("variant", sorted(STRESS))
+@pytest.mark.parametrize("dtype", ["bf16", "fp32"])
+@pytest.mark.parametrize("mode", [O.FKL_TOPK, O.RKL_MC])
+def test_stress_variants(handle, variant, dtype, mode):
+    """SURVEY 8(d) stress inputs: peaked rows, monotonically growing column norms (online-max rescaling in every tile of the
+    forward, exponents far below zero in the re-formed softmax tiles), stale caches with large importance ratios."""
+    cfg = dict(RAGGED, dtype=dtype, T=520, V=4360, **STRESS[variant])
+    inp = synth.make_inputs(cfg, c=11, device=DEV)
+    idx, lam, old, kk = pick(inp, cfg, mode)
+    r = run(handle, inp, idx, lam, old, mode, kk)
+    ref = oracle_for(inp, idx, lam, old, mode, kk)
+    if variant == "peaked_monotone_stale" and mode == O.RKL_MC:
+        rho = np.exp(ref["student_logp"][:, :kk] - f64(old))
+        assert np.nanmax(rho[f64(inp["mask"]) != 0]) > 3.0           # the tail is really there
+    compare_all(r, ref, f64(inp["mask"]), dtype)
+
+
 def test_degenerate_cases(handle, opd):
     cfg = dict(RAGGED, T=130, k=64, K=64)
     inp = synth.make_inputs(cfg, c=8, device=DEV)
