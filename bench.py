@@ -30,7 +30,7 @@ UNIT = "live tokens/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from one committed `ncu --set full` capture of this
 # workload (a citation: bench.py never runs under a profiler, so the line carries "traffic_measured": false)
 NCU_TRAFFIC = {
-    "C4": dict(bwd_kernel=151_675_632_000, fwd_kernel=10_745_648_000, source="profiles/r02_final_c4.md"),
+    "C4": dict(bwd_kernel=139_389_495_000, fwd_kernel=10_921_094_000, source="profiles/r02_final_c4.md"),
 }
 
 
@@ -47,6 +47,35 @@ def peaks():
         return dict(burst=float(j["bf16_tflops"]), sustained=float(j.get("bf16_tflops_sustained", j["bf16_tflops"])),
                     hbm=float(j["hbm_gbs"]), src="measured")
     return dict(burst=1590.0, sustained=1400.0, hbm=6650.0, src="fallback")
+
+
+def same_box_cublas(dev, seconds: float = 3.0):
+    """What the library GEMM does on THIS box right now, measured the way MEASURED_PEAKS.json was (torch.matmul bf16 8192^3:
+    best of 10 = burst, back to back for `seconds` = sustained).  Boxes of the pool differ by several per cent in what the
+    1000 W cap lets them sustain; this is context beside the driver-written peaks, never the roofline's denominator."""
+    n = 8192
+    a = torch.randn(n, n, device=dev, dtype=torch.bfloat16)
+    b = torch.randn(n, n, device=dev, dtype=torch.bfloat16)
+    c = torch.empty(n, n, device=dev, dtype=torch.bfloat16)
+    for _ in range(3):
+        torch.matmul(a, b, out=c)
+    torch.cuda.synchronize()
+    best = float("inf")
+    for _ in range(10):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); torch.matmul(a, b, out=c); e1.record(); torch.cuda.synchronize()
+        best = min(best, e0.elapsed_time(e1))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps, t0 = 0, time.perf_counter()
+    e0.record()
+    while time.perf_counter() - t0 < seconds:
+        for _ in range(20):
+            torch.matmul(a, b, out=c)
+        reps += 20
+        torch.cuda.synchronize()
+    e1.record(); torch.cuda.synchronize()
+    fl = 2.0 * n ** 3 / 1e12
+    return dict(burst=fl / (best * 1e-3), sustained=fl * reps / (e0.elapsed_time(e1) * 1e-3), how="torch.matmul bf16 8192^3 on this box, after the timed steps")
 
 
 def workload(cfg_id: int, args):
@@ -265,6 +294,7 @@ def main():
     ap.add_argument("--diag", action="store_true", help="also report rho statistics of the MC cache (opd_set_diagnostics)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-probe", action="store_true", help="skip the same-box cuBLAS measurement (3 s, after the timed steps)")
     ap.add_argument("--ref-seconds", type=float, default=12.0)
     args = ap.parse_args()
     if args.mode is None:
@@ -443,6 +473,10 @@ def main():
                                     traffic=tr["fwd_kernel"] if tr else None),
                     traffic_source=tr["source"] if tr else None)
     whole = flops_exec / (ms_per_step * 1e-3) / 1e12
+    box = None
+    if world == 1 and not args.no_probe:
+        box = same_box_cublas(dev)
+        box["executed_8dV_vs_same_box_sustained"] = 100 * whole / box["sustained"]
     cpu = None
     if not args.no_cpu:
         sub = dict(hidden=inp["hidden"][:4096], W=inp["W"], mask=inp["mask"][:4096])
@@ -457,7 +491,7 @@ def main():
                 config=config_dict(cfg, args.mode, idx.shape[1], inp["sigma"]),
                 launch=dict(live_tokens_per_gpu=n_live, super_tile=[stats["super_rows"], stats["super_cols"]], layout=args.layout),
                 pct_of_bf16_peak=dict(executed_8dV_vs_burst=100 * whole / pk["burst"], executed_8dV_vs_sustained=100 * whole / pk["sustained"],
-                                      model_6dV_vs_burst=100 * whole * 0.75 / pk["burst"], tflops_executed=whole, peaks=pk),
+                                      model_6dV_vs_burst=100 * whole * 0.75 / pk["burst"], tflops_executed=whole, peaks=pk, same_box_cublas=box),
                 phase_ms=pm, phase_ms_per_step=phase_steps, step_ms=step_ms, loss=loss_val, clocks=clocks, e2e=e2e, gpu_launches=stats["kernels"] * args.steps,
                 roofline=roofline, cpu_baseline=cpu, mc_diagnostics=diag)
     print(json.dumps(line), flush=True)
