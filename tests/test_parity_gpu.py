@@ -394,10 +394,11 @@ def test_call_is_cuda_graph_capturable(handle):
 
 
 @pytest.mark.parametrize("knobs", [dict(OPD_CTA_GROUP="1"), dict(OPD_G_BUFS="3", OPD_TB="256", OPD_VB="256"),
-                                   dict(OPD_GROUP_M="3", OPD_HINT_GW="1", OPD_HINT_G="2")])
+                                   dict(OPD_GROUP_M="3", OPD_HINT_GW="1", OPD_HINT_G="2"),
+                                   dict(OPD_Q_DEPTH="1", OPD_TB="256", OPD_VB="512"), dict(OPD_Q_DEPTH="8", OPD_TB="256", OPD_VB="256")])
 def test_tuning_knobs_do_not_change_results(handle, knobs, monkeypatch):
-    """The single-CTA tile configuration, a 3-deep G ring with the smallest super-tiles, another raster group and L2
-    hints give the same outputs as the defaults (within summation-order noise) and match the oracle."""
+    """The single-CTA tile configuration, a 3-deep G ring with the smallest super-tiles, another raster group, L2
+    hints and the extreme claim-ahead depths of the tile queue give the same outputs as the defaults (within summation-order noise) and match the oracle."""
     cfg = RAGGED
     inp = synth.make_inputs(cfg, c=16, device=DEV)
     idx, lam, old, kk = pick(inp, cfg, O.RKL_MC)
