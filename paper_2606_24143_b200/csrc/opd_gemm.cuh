@@ -26,9 +26,11 @@ constexpr int GEMM_THREADS = 192;                     // warp0 TMA, warp1 MMA(+T
 #ifndef OPD_BWD_EPI_WARPS
 #define OPD_BWD_EPI_WARPS 4
 #endif
-constexpr int BWD_EPI_WARPS = OPD_BWD_EPI_WARPS;                      // bwd_kernel: two epilogue warps per TMEM lane quarter (each takes half the
-                                                      // columns of a G tile: with one warp per scheduler nothing overlaps the
-                                                      // TMEM reads, MUFU latency and scattered row stores of that warp)
+// Epilogue warps of bwd_kernel: 4 (one per TMEM lane quarter), or 8 with -DOPD_BWD_EPI_WARPS=8 (two per quarter, each half of
+// a G tile's columns).  8 was measured no faster (the TMEM and LSU ports it would overlap are per SM, not per scheduler) and caps the
+// kernel at 168 registers per thread (profiles/r02_trace.md): an experiment, not the product configuration.
+constexpr int BWD_EPI_WARPS = OPD_BWD_EPI_WARPS;
+static_assert(BWD_EPI_WARPS == 4 || BWD_EPI_WARPS == 8, "one or two epilogue warps per TMEM lane quarter");
 constexpr int BWD_THREADS = (2 + BWD_EPI_WARPS + 1) * 32;   // + the publisher of finished tiles (last warp)
 constexpr int PUB_Q = 4;                              // tiles the epilogue warps may run ahead of the publisher
 constexpr int EPI_SMEM_BYTES = 32768;                 // 4 epilogue warps x 2 staging buffers x (32 rows x 128 B)

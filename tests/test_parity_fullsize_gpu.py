@@ -66,12 +66,18 @@ def sampled_check(handle, cfg, c, mode, n_rows=12):
     lhs = (inp["W"].double() * gw.double()).sum(dim=1)
     rhs = (inp["hidden"].double() * gh.double()).sum(dim=0)
     assert (lhs - rhs).abs().max().item() <= 2e-2 * max(lhs.abs().max().item(), 1e-30)
-    return r
+    # a second call at full size gives the same bits: the dependency counters fix the order of every fp32 reduction whatever CTA
+    # pair claims a tile (a race between a tile's stores and its publication would show up here first)
+    keep = (r["loss"].clone(), gh.clone(), gw.clone())
+    del r, gh, gw
+    r2 = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk)
+    torch.cuda.synchronize()
+    assert torch.equal(keep[0], r2["loss"]) and torch.equal(keep[1], r2["grad_hidden"]) and torch.equal(keep[2], r2["grad_W"])
 
 
 def test_C3_shape_sampled(handle):
-    r = sampled_check(handle, synth.CONFIGS[3], 3, O.RKL_MC)
-    r = sampled_check(handle, synth.CONFIGS[3], 3, O.FKL_TOPK)
+    sampled_check(handle, synth.CONFIGS[3], 3, O.RKL_MC)
+    sampled_check(handle, synth.CONFIGS[3], 3, O.FKL_TOPK)
 
 
 def test_C4_shape_sampled(handle):
