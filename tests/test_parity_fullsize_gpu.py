@@ -27,8 +27,10 @@ def handle():
     return opd.Handle(0)
 
 
-def sampled_check(handle, cfg, c, mode, n_rows=12):
+def sampled_check(handle, cfg, c, mode, n_rows=12, layout="dv"):
     inp = synth.make_inputs(cfg, c=c, device=DEV)
+    if layout == "vd":                                       # the same logical [d,V] matrix stored [V,d] like lm_head.weight
+        inp["W"] = inp["W"].t().contiguous().t()
     idx, lam, old, kk = pick(inp, cfg, mode)
     r = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, want_lse=True, want_student_logp=True)
     torch.cuda.synchronize()
@@ -78,6 +80,11 @@ def sampled_check(handle, cfg, c, mode, n_rows=12):
 def test_C3_shape_sampled(handle):
     sampled_check(handle, synth.CONFIGS[3], 3, O.RKL_MC)
     sampled_check(handle, synth.CONFIGS[3], 3, O.FKL_TOPK)
+
+
+def test_C3_shape_sampled_vd_storage(handle):
+    """W stored [V,d] (other TMA boxes / UMMA majorness in all three contractions), at the 1.7B-class shape."""
+    sampled_check(handle, synth.CONFIGS[3], 3, O.RKL_MC, layout="vd")
 
 
 def test_C4_shape_sampled(handle):
