@@ -85,6 +85,9 @@ struct GemmParams {
     unsigned long long a_hint, b_hint;   // L2 eviction policy of the operand loads (0 = normal)
     int first, last;          // DxEpi: first / last vocabulary super-tile of this token super-tile
     int row_off, col_off;     // DwEpi: position of this GEMM's output inside grad_W
+#ifdef OPD_EXPERIMENTS
+    int skip_b;               // TileOp::skip_b of a one-GEMM launch
+#endif
 #ifdef OPD_TRACE
     long long* tr;            // tracing builds: cycle sums of the epilogue that runs this tile (slot 6: TMEM waits, 7: chunk bodies)
 #endif
@@ -220,6 +223,9 @@ struct TileOp {
     int nseg;
     unsigned char pa[MAX_SEG], pb[MAX_SEG];   // plane per segment
     uint64_t a_hint, b_hint;  // L2 eviction policy of the operand loads
+#ifdef OPD_EXPERIMENTS
+    int skip_b = 0;           // timing experiment (wrong results): after the first ring fill the B operand is not loaded any more
+#endif
 };
 
 // TMA producer (one elected lane): stream all k-blocks of all segments of `t` through the ring.
@@ -267,14 +273,20 @@ __device__ __forceinline__ void produce_tile(const Pipe<CG, ST>& P, const TileOp
             } else {
                 // the leader's barrier counts the bytes of both CTAs (expect_tx may trail the peer's complete_tx:
                 // the phase cannot complete before the leader's own arrival)
-                if (P.rank == 0) mbar_arrive_expect_tx(&P.full_bar[s], 2 * C::STAGE_BYTES);
+#ifdef OPD_EXPERIMENTS
+                const bool skipb = t.skip_b && it >= C::STAGES;
+#else
+                constexpr bool skipb = false;
+#endif
+                if (P.rank == 0) mbar_arrive_expect_tx(&P.full_bar[s], skipb ? 2 * C::A_STAGE_BYTES : 2 * C::STAGE_BYTES);
                 const uint32_t bar = mapa_rank(smem_u32(&P.full_bar[s]), 0);
                 if (t.a_mn) {
                     for (int b = 0; b < BM / MN_BOX; ++b) tma_load_3d_pair(sA + b * MN_BOX_BYTES, t.tA, bar, t.a_c + b * MN_BOX, kca, pa, t.a_hint);
                 } else {
                     tma_load_3d_pair(sA, t.tA, bar, kca, t.a_c, pa, t.a_hint);
                 }
-                if (t.b_mn) {
+                if (skipb) {
+                } else if (t.b_mn) {
                     for (int b = 0; b < C::B_ROWS / MN_BOX; ++b) tma_load_3d_pair(sB + b * MN_BOX_BYTES, t.tB, bar, t.b_c + b * MN_BOX, kcb, pb, t.b_hint);
                 } else {
                     tma_load_3d_pair(sB, t.tB, bar, kcb, t.b_c, pb, t.b_hint);
@@ -390,6 +402,9 @@ gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             t.nseg = gp.nseg;
             t.a_hint = gp.a_hint ? gp.a_hint : L2_EVICT_NORMAL; t.b_hint = gp.b_hint ? gp.b_hint : L2_EVICT_NORMAL;
             for (int i = 0; i < MAX_SEG; ++i) { t.pa[i] = gp.sa[i]; t.pb[i] = gp.sb[i]; }
+#ifdef OPD_EXPERIMENTS
+            t.skip_b = gp.skip_b;
+#endif
             int it = 0;
             for (int tile = first_tile; tile < total_tiles; tile += tile_step) {
                 int m2, n_blk;

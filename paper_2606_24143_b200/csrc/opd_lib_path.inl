@@ -191,6 +191,9 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
         set_segments(gp, p.planes);
         gp.a_hint = hint_policy(env_int("OPD_HINT_FX", 0)); gp.b_hint = hint_policy(env_int("OPD_HINT_FW", 0));
         gp.tok_dim = TOK_M; gp.tok_off = 0; gp.n_live = n_live;
+#ifdef OPD_EXPERIMENTS
+        gp.skip_b = env_int("OPD_SKIP_B", 0);                 // timing experiment: what the W loads of the forward cost (wrong results)
+#endif
         FwdEpi::Params ep{partials, p.t_pad, sorted_idx, zc, C, V, a.dbg_logits};
         OPD_CUDA(h, launch_gemm<FwdEpi>(h, st, m_xc_k, m_w_fwd, gp, ep));
     }
