@@ -292,6 +292,7 @@ def main():
     ap.add_argument("--cache-width", type=int, default=0, help="override the config's k and K (C4's cost-vs-cache-size sweep)")
     ap.add_argument("--layout", default="dv", choices=["dv", "vd"], help="storage order of W: [d,V] row-major (BASELINE.json) or [V,d] (lm_head.weight)")
     ap.add_argument("--diag", action="store_true", help="also report rho statistics of the MC cache (opd_set_diagnostics)")
+    ap.add_argument("--fwd-only", action="store_true", help="diagnostic: time OPD_F_FWD_ONLY calls (S0-S5: pre-pass, forward contraction, estimators) back to back")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-probe", action="store_true", help="skip the same-box cuBLAS measurement (3 s, after the timed steps)")
@@ -326,6 +327,23 @@ def main():
     h = opd.Handle(local)
     if args.op != "loss":
         run_producer_bench(args, h, inp, cfg, dev, world, rank, dist)
+        return
+    if args.fwd_only:
+        # forward-only diagnostic (profiles/r02_experiments.md section 11): not the contract's line
+        f = lambda: h.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, flags=opd.F_FWD_ONLY)
+        for _ in range(max(args.warmup, 3)):
+            f()
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            f()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        print(json.dumps(dict(metric="OPD loss forward only (S0-S5) on 1 B200", ms_per_step=ms, tflops_executed=2.0 * d * V * n_live / ms / 1e9,
+                              steps=args.steps, config=config_dict(cfg, args.mode, idx.shape[1], inp["sigma"]), clocks=sampler.stop())), flush=True)
         return
     gh = torch.empty_like(inp["hidden"])
     if args.layout == "vd":          # same logical [d,V] matrices, [V,d] storage
