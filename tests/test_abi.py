@@ -73,11 +73,11 @@ def test_no_cpu_fallback():
 
 
 def test_wrong_gradient_switches_are_not_in_the_product_library(lib):
-    """OPD_BWD_TYPES / OPD_DBG_ACC / OPD_DENSE_BWD (timing experiments that return wrong gradients) are compiled in only with
+    """OPD_BWD_TYPES / OPD_DBG_ACC / OPD_DENSE_BWD / OPD_SKIP_B (timing experiments that return wrong gradients) are compiled in only with
     -DOPD_EXPERIMENTS: the default build never reads them, so a stray environment variable in a training job is inert."""
     from paper_2606_24143_b200 import opd
     blob = open(opd.LIB_PATH, "rb").read()
-    for name in (b"OPD_BWD_TYPES", b"OPD_DBG_ACC", b"OPD_DENSE_BWD"):
+    for name in (b"OPD_BWD_TYPES", b"OPD_DBG_ACC", b"OPD_DENSE_BWD", b"OPD_SKIP_B"):
         assert name not in blob, name
     assert b"OPD_TB" in blob          # result-neutral tuning knobs are still read
 
