@@ -124,6 +124,49 @@ opd_status_t opd_loss_fwd_bwd(opd_handle_t h, void* cuda_stream,
     void* grad_hidden, long ld_gh,
     void* grad_W, long ldgw_k, long ldgw_v);
 
+/* The same call for callers that must not allocate device memory -------------------------------------------------------
+ * Who this is for. opd_loss_fwd_bwd keeps its scratch in a buffer the handle obtains with cudaMalloc (and regrows with
+ * cudaFree + cudaMalloc when a bigger shape arrives). Two kinds of caller cannot live with that:
+ *   - a learner that shares the GPU with something that took the rest of HBM at start-up (an inference engine's KV pool, a
+ *     framework's caching allocator sized to the device): a raw cudaMalloc there simply fails, or succeeds and starves the
+ *     other tenant; such a caller gets all its device memory handed to it and has no spare pointer to lend as workspace;
+ *   - a caller inside a latency-critical loop that keeps several streams busy: cudaMalloc / cudaFree synchronise the whole
+ *     device, so one call with a new shape stalls every other stream of the process.
+ * opd_loss_fwd_bwd_static takes the arguments of opd_loss_fwd_bwd, computes the same results with the same kernels, and
+ * keeps ALL of its scratch in a fixed array of OPD_STATIC_SCRATCH_BYTES that is part of the library image (a file-scope
+ * `static __device__` array in opd_lib.cu). It calls no cudaMalloc, cudaFree or other allocating routine, and neither reads
+ * nor changes the handle's own workspace (the one opd_set_workspace / opd_loss_fwd_bwd use).
+ *   Cost: every GPU on which the library's kernels are loaded holds those OPD_STATIC_SCRATCH_BYTES (32 MiB) from module load
+ *     until the process exits, whether or not this entry point is ever called.
+ *   Limit: the call is refused (OPD_ERR_WORKSPACE, nothing launched, opd_last_error names both numbers) when
+ *     opd_workspace_bytes(T, d, V, C, dtype, mode, flags) > OPD_STATIC_SCRATCH_BYTES. That covers e.g. fp32 T=256, d=256,
+ *     V=4096 (15.7 MiB), bf16 T=1024, d=1024, V=32768 with gradients (18.2 MiB), and bf16 T=4096, d=1024, V=32768 with
+ *     OPD_F_FWD_ONLY (12.9 MiB); bigger problems must be cut into token chunks by the caller (OPD_F_GRADW_ACCUM + norm_override)
+ *     or go through opd_loss_fwd_bwd.
+ *   Set-up: the first call on each device looks up the device address of the array (cudaGetSymbolAddress, with the handle's
+ *     device current; this may load the library's device code on that GPU) and remembers it; later calls only launch. Make
+ *     that first call early, in ordinary eager execution, before any stream capture is begun.
+ *   Sharing: there is ONE array per GPU for the whole process, shared by every handle and every stream. Each call clears the
+ *     parts that must start at zero and overwrites the rest, so back-to-back calls on one stream are independent of what the
+ *     previous call left behind; but two calls whose kernels can be in flight on the same GPU at the same time (different
+ *     streams, different threads, different handles) race on it and both return garbage. Serialise them on one stream. */
+#define OPD_STATIC_SCRATCH_BYTES (32u << 20)
+opd_status_t opd_loss_fwd_bwd_static(opd_handle_t h, void* cuda_stream,
+    int T, int d, int V, opd_dtype_t dtype,
+    const void* hidden, long ld_hidden,
+    const void* W, long ldw_k, long ldw_v,
+    const int* cache_idx, long ld_cache,
+    const float* cache_teacher_logp,
+    const float* cache_old_logp,
+    const unsigned char* mask,
+    opd_mode_t mode, int k_or_K,
+    unsigned flags, float norm_override,
+    float* loss,
+    float* per_token_kl,
+    float* lse_out, float* student_logp_out,
+    void* grad_hidden, long ld_gh,
+    void* grad_W, long ldgw_k, long ldgw_v);
+
 /* Same computation with HOST buffers (pinned or pageable): copies the inputs to handle-owned device
  * buffers, runs opd_loss_fwd_bwd, copies loss / per_token_kl / grad_hidden / grad_W back and
  * synchronises. All arrays are dense (ld = inner extent); W is [d,V] row-major. Pointers that are NULL

@@ -1,6 +1,7 @@
 // libopd — C ABI (include/opd.h) of the fused OPD loss for sm_100a.  Single translation unit:
 //   nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -shared -Xcompiler -fPIC opd_lib.cu -o libopd.so
 #include "opd_host.cuh"
+#include <mutex>
 
 using namespace opd;
 
@@ -148,3 +149,74 @@ extern "C" opd_status_t opd_set_seq_diagnostics(opd_handle_t h, int n_seq, const
 #include "opd_lib_extra.inl"
 #include "opd_lib_producer.inl"
 #include "opd_lib_dense.inl"
+
+// ------------------------------------------------------------------------------------------------------------------
+// opd_loss_fwd_bwd_static: the hot path for callers that are not allowed to allocate device memory (include/opd.h says who
+// they are: tenants of a GPU whose free memory somebody else already took, and loops that cannot afford the device-wide
+// synchronisation inside cudaMalloc / cudaFree).  All scratch of the call lives in the array below, which is part of the
+// library's device image: the driver places it when the module is loaded on a GPU and it stays there until the process
+// ends.  One copy per GPU, shared by every handle, stream and thread of the process.
+static __device__ __align__(256) unsigned char g_static_scratch[OPD_STATIC_SCRATCH_BYTES];
+
+// In host code `g_static_scratch` is only the host-side shadow the runtime uses to identify the symbol; its value is not a
+// device address and must never reach a kernel.  The address the kernels get is the one cudaGetSymbolAddress reports for
+// the device that is current at the time, looked up once per device and kept here.
+static constexpr int STATIC_MAX_DEVICES = 64;
+static void* g_static_scratch_addr[STATIC_MAX_DEVICES] = {};
+static std::mutex g_static_scratch_mu;
+
+// Caller has made h->device current.  First call per device: resolve and remember the array's device address.
+static opd_status_t static_scratch_address(opd_handle_s* h, void** out) {
+    if (h->device < 0 || h->device >= STATIC_MAX_DEVICES)
+        OPD_FAIL(h, OPD_ERR_BAD_ARG, "opd_loss_fwd_bwd_static supports device ordinals below %d (handle is on %d)", STATIC_MAX_DEVICES, h->device);
+    std::lock_guard<std::mutex> lock(g_static_scratch_mu);
+    void*& slot = g_static_scratch_addr[h->device];
+    if (!slot) {
+        void* p = nullptr;
+        OPD_CUDA(h, cudaGetSymbolAddress(&p, g_static_scratch));
+        cudaPointerAttributes at{};
+        OPD_CUDA(h, cudaPointerGetAttributes(&at, p));
+        if (!p || at.type != cudaMemoryTypeDevice || at.device != h->device || (reinterpret_cast<uintptr_t>(p) & 255))
+            OPD_FAIL(h, OPD_ERR_CUDA, "the static scratch array did not resolve to 256-byte aligned memory of device %d", h->device);
+        slot = p;
+    }
+    *out = slot;
+    return OPD_OK;
+}
+
+extern "C" opd_status_t opd_loss_fwd_bwd_static(opd_handle_t h, void* cuda_stream, int T, int d, int V, opd_dtype_t dtype,
+    const void* hidden, long ld_hidden, const void* W, long ldw_k, long ldw_v, const int* cache_idx, long ld_cache,
+    const float* cache_teacher_logp, const float* cache_old_logp, const unsigned char* mask, opd_mode_t mode, int k_or_K,
+    unsigned flags, float norm_override, float* loss, float* per_token_kl, float* lse_out, float* student_logp_out,
+    void* grad_hidden, long ld_gh, void* grad_W, long ldgw_k, long ldgw_v) {
+    if (!h) return OPD_ERR_BAD_ARG;
+    if (!h->arch_ok) OPD_FAIL(h, OPD_ERR_ARCH, "device %d is not compute capability 10.x (sm_100a required, no fallback)", h->device);
+    // Size check first, on the host, before anything is launched.  (Shapes, modes and dtypes the library does not support
+    // at all fall through to run_path, which reports them without touching any workspace.)
+    int kf, Km;
+    const int C = cache_width(mode, k_or_K, &kf, &Km);
+    const bool plannable = T >= 1 && T < (1 << 24) && d >= 64 && d <= 16384 && d % 64 == 0 && V >= 256 && V < (1 << 24) && V % 8 == 0 &&
+                           C >= 1 && C <= 64 && (dtype == OPD_BF16 || dtype == OPD_FP32) && (int)mode >= 0 && (int)mode <= 3;
+    if (plannable) {
+        const size_t need = make_plan(T, d, V, C, dtype == OPD_FP32, flags, (int)mode).total;
+        if (need > (size_t)OPD_STATIC_SCRATCH_BYTES)
+            OPD_FAIL(h, OPD_ERR_WORKSPACE, "opd_loss_fwd_bwd_static: T=%d d=%d V=%d C=%d needs %zu bytes of scratch, the static array holds %zu "
+                     "(OPD_STATIC_SCRATCH_BYTES); split the tokens into chunks or use opd_loss_fwd_bwd", T, d, V, C, need,
+                     (size_t)OPD_STATIC_SCRATCH_BYTES);
+    }
+    OPD_ON_DEVICE(h);
+    void* scratch = nullptr;
+    opd_status_t s = static_scratch_address(h, &scratch);
+    if (s != OPD_OK) return s;
+    // Run the unchanged path with the static array standing in for the handle's workspace: marked as not owned and of
+    // fixed size, so nothing below can free or grow it (a plan that did not fit would be refused, never reallocated).
+    // run_path zeroes the pieces that must start at zero (bad-index flag, gathered logits, tile counters) on every call.
+    void* const keep_ws = h->ws; const size_t keep_bytes = h->ws_bytes; const bool keep_owned = h->ws_owned;
+    h->ws = scratch; h->ws_bytes = OPD_STATIC_SCRATCH_BYTES; h->ws_owned = false;
+    PathIO a{T, d, V, dtype, hidden, ld_hidden, W, ldw_k, ldw_v, cache_idx, ld_cache, cache_teacher_logp, cache_old_logp, mask,
+             mode, k_or_K, flags, norm_override, loss, per_token_kl, lse_out, student_logp_out, grad_hidden, ld_gh,
+             grad_W, ldgw_k, ldgw_v, nullptr, nullptr, false, false};
+    s = run_path(h, static_cast<cudaStream_t>(cuda_stream), a);
+    h->ws = keep_ws; h->ws_bytes = keep_bytes; h->ws_owned = keep_owned;
+    return s;
+}

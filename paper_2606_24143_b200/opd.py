@@ -20,11 +20,12 @@ FKL_TOPK, RKL_MC, MIXED, RKL_TOPK = 0, 1, 2, 3
 BF16, FP32 = 0, 1
 F_NO_RENORM_TEACHER, F_RENORM_STUDENT, F_GRADW_ACCUM, F_GRADW_BF16, F_VALIDATE_IDX, F_FWD_ONLY = 1, 2, 4, 8, 16, 32
 F_SUR_CLIP, F_SUR_A_OLD, F_DENSE_REVERSE = 64, 128, 256
+STATIC_SCRATCH_BYTES = 32 << 20          # OPD_STATIC_SCRATCH_BYTES of include/opd.h
 N_PHASES = 4
 PHASE_NAMES = ("prep", "fwd", "est", "bwd")
 
 EXPORTS = ("opd_create", "opd_destroy", "opd_last_error", "opd_version", "opd_workspace_bytes", "opd_set_workspace",
-           "opd_loss_fwd_bwd", "opd_loss_fwd_bwd_host", "opd_loss_fwd_bwd_host_submit", "opd_loss_fwd_bwd_host_wait", "opd_debug_logits", "opd_debug_gemm", "opd_last_launch_stats",
+           "opd_loss_fwd_bwd", "opd_loss_fwd_bwd_static", "opd_loss_fwd_bwd_host", "opd_loss_fwd_bwd_host_submit", "opd_loss_fwd_bwd_host_wait", "opd_debug_logits", "opd_debug_gemm", "opd_last_launch_stats",
            "opd_set_phase_events", "opd_set_diagnostics", "opd_set_seq_diagnostics", "opd_debug_occupy", "opd_cache_workspace_bytes", "opd_cache_topk", "opd_cache_sample",
            "opd_dense_kl_workspace_bytes", "opd_dense_kl_fwd_bwd")
 
@@ -61,6 +62,8 @@ def load_library():
                                      c_int, c_int, c_uint, c_float, c_void_p, c_void_p, c_void_p, c_void_p,
                                      c_void_p, c_long, c_void_p, c_long, c_long]
     lib.opd_loss_fwd_bwd.restype = c_int
+    lib.opd_loss_fwd_bwd_static.argtypes = list(lib.opd_loss_fwd_bwd.argtypes)
+    lib.opd_loss_fwd_bwd_static.restype = c_int
     lib.opd_loss_fwd_bwd_host.argtypes = [c_void_p, c_int, c_int, c_int, c_int, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
                                           c_void_p, c_int, c_int, c_uint, c_float, c_void_p, c_void_p, c_void_p, c_void_p,
                                           POINTER(c_size_t), POINTER(c_size_t)]
@@ -319,6 +322,63 @@ class Handle:
         if slp is not None:
             slp = slp[:, :cache_idx.shape[1]]
         return dict(loss=loss, per_token_kl=ptk, grad_hidden=grad_hidden, grad_W=grad_W, lse=lse, student_logp=slp)
+
+    def loss_fwd_bwd_static(self, hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K, out, flags=0,
+                            norm_override=0.0, stream=None):
+        """opd_loss_fwd_bwd_static: the same computation as loss_fwd_bwd for a caller that may not allocate GPU memory -- a
+        learner whose GPU's free memory already belongs to another tenant (an inference engine's pool, a caching allocator
+        sized to the device), or a loop that cannot take the device-wide stall of cudaMalloc / cudaFree.  The library keeps
+        the call's scratch in a fixed 32 MiB array inside its own device image (STATIC_SCRATCH_BYTES) and this wrapper
+        allocates nothing either, so the caller supplies every buffer:
+          out = dict(loss [1] f32, per_token_kl [T] f32, grad_hidden [T,d] like hidden, grad_W logical [d,V] f32 (bf16 with
+                     F_GRADW_BF16) with W's unit stride; optional lse [T] f32, student_logp [T, row stride of cache_idx] f32);
+                grad_hidden / grad_W may be left out with F_FWD_ONLY.  The results are written into these tensors; `out` is returned.
+        Inputs must already be in the form the C ABI takes (int32 indices, uint8 / bool mask, unit inner strides, one common
+        row stride for the three cache arrays): where loss_fwd_bwd would make a converted copy, this raises instead.
+        Raises OpdError(ERR_WORKSPACE) when the shape needs more scratch than the array holds (see workspace_bytes).
+        The first call on a device resolves the array's address; make it once before any stream capture.  One array per GPU
+        is shared by all handles and streams: calls that could overlap on the GPU must be serialised by the caller."""
+        given = (hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask)
+        ready = _marshal(*given)
+        for name, a, b in zip(("hidden", "W", "cache_idx", "cache_teacher_logp", "cache_old_logp", "mask"), given, ready):
+            if (a is None) != (b is None) or (a is not None and (a.data_ptr() != b.data_ptr() or a.stride() != b.stride())):
+                raise OpdError(ERR_BAD_ARG, f"{name} would need a converted copy (dtype / strides); the static entry point allocates nothing")
+        hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask = ready
+        T, d = hidden.shape
+        dt = _dtype_code(hidden)
+        if W.dtype != hidden.dtype:
+            raise OpdError(ERR_BAD_ARG, "hidden and W must have the same dtype")
+        ldk, ldv = _w_strides(W, d)
+        V = W.shape[1]
+        dev = hidden.device
+        fwd_only = bool(flags & F_FWD_ONLY)
+        gw_dtype = torch.bfloat16 if flags & F_GRADW_BF16 else torch.float32
+        want = [("loss", (1,), torch.float32), ("per_token_kl", (T,), torch.float32)]
+        if not fwd_only:
+            want += [("grad_hidden", (T, d), hidden.dtype), ("grad_W", (d, V), gw_dtype)]
+        for name, shape, dtype in want:
+            t = out.get(name)
+            if t is None or t.dtype != dtype or tuple(t.shape) != shape or t.device != dev:
+                raise OpdError(ERR_BAD_ARG, f"out['{name}'] must be a {shape} {dtype} tensor on {dev}")
+        lse, slp = out.get("lse"), out.get("student_logp")
+        if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (T,) or lse.device != dev or lse.stride(0) != 1):
+            raise OpdError(ERR_BAD_ARG, "out['lse'] must be a dense [T] float32 tensor on hidden's device")
+        if slp is not None and (slp.dtype != torch.float32 or slp.dim() != 2 or slp.shape[0] != T or slp.device != dev or
+                                slp.stride(1) != 1 or slp.stride(0) != cache_idx.stride(0)):
+            raise OpdError(ERR_BAD_ARG, "out['student_logp'] must be float32 [T, .] with the row stride of cache_idx")
+        gh, gw = (None, None) if fwd_only else (out["grad_hidden"], out["grad_W"])
+        if gh is not None and gh.stride(1) != 1:
+            raise OpdError(ERR_BAD_ARG, "out['grad_hidden'] needs a unit inner stride")
+        if not (out["loss"].is_contiguous() and out["per_token_kl"].is_contiguous()):
+            raise OpdError(ERR_BAD_ARG, "out['loss'] / out['per_token_kl'] must be dense")
+        s = torch.cuda.current_stream(dev).cuda_stream if stream is None else stream
+        gk, gv = (gw.stride(0), gw.stride(1)) if gw is not None else (0, 0)
+        self._check(self.lib.opd_loss_fwd_bwd_static(
+            self._h, c_void_p(s), T, d, V, dt, _ptr(hidden), hidden.stride(0), _ptr(W), ldk, ldv,
+            _ptr(cache_idx), cache_idx.stride(0), _ptr(cache_teacher_logp), _ptr(cache_old_logp), _ptr(mask),
+            mode, k_or_K, flags, float(norm_override), _ptr(out["loss"]), _ptr(out["per_token_kl"]), _ptr(lse), _ptr(slp),
+            _ptr(gh), gh.stride(0) if gh is not None else 0, _ptr(gw), gk, gv))
+        return out
 
     def loss_fwd_bwd_host(self, hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K, flags=0,
                           norm_override=0.0, out=None):
