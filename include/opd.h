@@ -71,6 +71,13 @@ opd_status_t opd_create(opd_handle_t* out, int device);
 opd_status_t opd_destroy(opd_handle_t h);
 const char* opd_last_error(opd_handle_t h); /* host string, valid until the next call on h */
 const char* opd_version(void);
+/* ABI revision of this header. It goes up whenever an existing entry point changes its argument list (a caller built against
+ * an older header would otherwise link and pass shifted arguments silently): 1 = round-1 header; 2 = opd_set_diagnostics took
+ * (rows, cols), opd_cache_topk / opd_cache_sample took a mask; 3 = opd_abi_version and opd_loss_fwd_bwd_static added (no
+ * signature changed). opd_abi_version() returns the value the LIBRARY was built with: compare it with OPD_ABI_VERSION once
+ * after loading and refuse to run on a mismatch (paper_2606_24143_b200/opd.py does). */
+#define OPD_ABI_VERSION 3
+int opd_abi_version(void);
 
 /* workspace ------------------------------------------------------------------------------------
  * Bytes of device scratch one opd_loss_fwd_bwd call with these arguments needs. No buffer of size
@@ -263,7 +270,11 @@ opd_status_t opd_set_diagnostics(opd_handle_t h, int rows, int cols, float* rho_
  *   seq_var_m[n]  = (1/T_n^2) sum_t Var^(L^MC_1 | s_t) / m   the variance of seq_mean_m over the local draws with the prefix
  *                   path fixed, from the within-prefix sample variances of Eq.(16) (draws are iid)
  * R_m^seq is a ratio of variances of these sequence means (m-sample over one-sample) which the caller forms over its
- * sequences or batches. Pass n_seq = 0 to switch off. */
+ * sequences or batches. Pass n_seq = 0 to switch off.
+ * The three outputs describe ONE estimator, Eq.(15) with A_theta and the unclipped ratio: while the hook is on, an
+ * OPD_RKL_MC / OPD_MIXED call that carries OPD_F_SUR_CLIP or OPD_F_SUR_A_OLD is refused (OPD_ERR_BAD_ARG) — its per-token
+ * values would follow the surrogate while the one-sample terms and variances would not, and their ratio would compare two
+ * different objectives. */
 opd_status_t opd_set_seq_diagnostics(opd_handle_t h, int n_seq, const int* cu_seqlens,
                                      float* seq_mean_m, float* seq_mean_1, float* seq_var_m);
 

@@ -5,7 +5,11 @@
 
 Marshalling only: forward calls opd_loss_fwd_bwd once (loss AND both gradients are produced by that call, the
 logits are never materialised); backward hands the stored gradients to autograd, scaled (out of place: a second
-backward with retain_graph=True sees the same saved tensors) by the incoming scalar gradient.  There is no PyTorch fallback: without libopd.so / off sm_100 the call raises.
+backward with retain_graph=True sees the same saved tensors) by the incoming scalar gradient.  Peak memory: for a bf16 head
+the library is asked for a bf16 grad_W (OPD_F_GRADW_BF16: fp32 sums stay in the handle's workspace and are rounded once), so
+what is saved for backward is already in the parameter's dtype (2*d*V bytes instead of 4*d*V), and the scale by the incoming
+gradient writes straight into one tensor of that dtype (no fp32 temporary, no separate cast copy).
+There is no PyTorch fallback: without libopd.so / off sm_100 the call raises.
 """
 from __future__ import annotations
 
@@ -19,6 +23,8 @@ class _OpdLoss(torch.autograd.Function):
     def forward(ctx, hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K, flags, norm_override):
         need_grad = hidden.requires_grad or W.requires_grad
         h = opd.default_handle(hidden.device.index)
+        if need_grad and W.dtype == torch.bfloat16 and not (flags & opd.F_GRADW_ACCUM):
+            flags |= opd.F_GRADW_BF16                   # the gradient autograd wants has W's dtype anyway: save it as such
         r = h.loss_fwd_bwd(hidden.detach(), W.detach(), cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K,
                            flags=flags | (0 if need_grad else opd.F_FWD_ONLY), norm_override=norm_override)
         ctx.need_grad = need_grad
@@ -35,8 +41,10 @@ class _OpdLoss(torch.autograd.Function):
         gh, gw = ctx.saved_tensors
         if g_loss is not None:                  # chain rule with the incoming scalar: out of place, without a host sync
             gh = gh * g_loss.to(gh.dtype)
-            gw = gw * g_loss.to(gw.dtype)
-        gw = gw if gw.dtype == ctx.w_dtype else gw.to(ctx.w_dtype)
+            # one output in W's dtype; the product is formed in fp32 and rounded on the way out (no full-size temporary)
+            gw = torch.mul(gw, g_loss.float(), out=torch.empty_like(gw, dtype=ctx.w_dtype))
+        elif gw.dtype != ctx.w_dtype:
+            gw = gw.to(ctx.w_dtype)
         return gh, gw, None, None, None, None, None, None, None, None
 
 

@@ -108,6 +108,8 @@ struct Plan {
     int gs_bufs;          // ring depth of the G super-tile buffer
     size_t xc_plane, w_plane, gs_plane;   // elements per plane
     size_t sort_n; int sort_blocks;       // sparse backward: entries to sort, blocks of the radix sort
+    size_t dv_bytes;      // bytes of the items of size O(d*V) (bf16 planes of an fp32 W, transposed W, fp32 sums behind a bf16 grad_W):
+                          // weight-sized, not logits-sized, so they do not count against the T x V budget of make_plan
 };
 
 inline int env_int(const char* name, int dflt) {
@@ -178,6 +180,7 @@ inline Plan make_plan_cfg(int T, int d, int V, int C, int fp32, unsigned flags, 
     p.off_shist = take(bwd && p.sparse_bwd ? sizeof(uint32_t) * 256 * (size_t)p.sort_blocks : 0);
     p.off_gw32 = take(bwd && (flags & OPD_F_GRADW_BF16) ? (size_t)d * V * 4 : 0);      // fp32 sums behind a bf16 grad_W
     p.off_seq_l1 = take(sizeof(float) * (size_t)p.t_pad);                               // per-token terms of opd_set_seq_diagnostics
+    p.dv_bytes = (p.off_sorted - p.off_wsplit) + (p.off_skeys - p.off_wt) + (p.off_seq_l1 - p.off_gw32);   // each followed by the next take()
     p.off_seq_var1 = take(sizeof(float) * (size_t)p.t_pad);
     p.gs_plane = (size_t)p.Tb * p.Vb;
     p.gs_bufs = std::min(3, std::max(2, gbufs));
@@ -198,7 +201,10 @@ inline Plan make_plan_cfg(int T, int d, int V, int C, int fp32, unsigned flags, 
 }
 
 // Chooses the super-tile width Vb (= K depth of a grad_hidden tile) and the depth of the G ring under a workspace budget of
-// 4.8% of the bf16 logits (no buffer of the order of T x V), from the sweeps of profiles/r02_experiments.md:
+// 4.8% of the bf16 logits (no buffer of the order of T x V), from the sweeps of profiles/r02_experiments.md.
+// The budget is applied to what grows with T (and with the super-tile): the weight-sized items (Plan::dv_bytes: the bf16
+// planes of an fp32 W, the transposed W of the sparse backward, the fp32 sums behind a bf16 grad_W) are the same for every
+// candidate and are left out, so OPD_F_GRADW_BF16 gets the same super-tiles as the fp32-grad_W call:
 //   T >= 32768: the widest of 16384 / 12288 / 8192 / 4096 columns that fits, two G buffers (wider = fewer fp32 partial-sum passes:
 //               C4 8192 columns, 2.5% faster than 4096; C5 16384 columns, 2.6% faster than 8192);
 //   smaller T:  4096 columns and THREE G buffers (no wait at the block boundaries: C3 +2%, C2 +4%) if that fits, else
@@ -213,12 +219,12 @@ inline Plan make_plan(int T, int d, int V, int C, int fp32, unsigned flags, int 
     if (t_pad >= 32768) {
         for (int vb : {16384, 12288, 8192}) {
             const Plan p = plan(vb, 2);
-            if ((double)p.total <= budget) return p;
+            if ((double)(p.total - p.dv_bytes) <= budget) return p;
         }
         return plan(4096, 2);
     }
     const Plan p3 = plan(4096, 3);
-    if ((double)p3.total <= budget) return p3;
+    if ((double)(p3.total - p3.dv_bytes) <= budget) return p3;
     if (logits < 1e9) return plan(2048, 3);
     return plan(4096, 2);
 }

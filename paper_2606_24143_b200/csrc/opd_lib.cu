@@ -34,7 +34,8 @@ struct DeviceGuard {
     DeviceGuard _device_guard((h)->device);                                                                    \
     if (!_device_guard.ok) OPD_FAIL(h, OPD_ERR_CUDA, "cannot make device %d current", (h)->device)
 
-extern "C" const char* opd_version(void) { return "opd-b200 0.1 (sm_100a, tcgen05/TMEM/TMA)"; }
+extern "C" const char* opd_version(void) { return "opd-b200 0.3 (sm_100a, tcgen05/TMEM/TMA)"; }
+extern "C" int opd_abi_version(void) { return OPD_ABI_VERSION; }
 
 extern "C" opd_status_t opd_create(opd_handle_t* out, int device) {
     if (!out) return OPD_ERR_BAD_ARG;

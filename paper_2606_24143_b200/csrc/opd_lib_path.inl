@@ -55,6 +55,9 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
     const unsigned known = OPD_F_NO_RENORM_TEACHER | OPD_F_RENORM_STUDENT | OPD_F_GRADW_ACCUM | OPD_F_GRADW_BF16 | OPD_F_VALIDATE_IDX |
                            OPD_F_FWD_ONLY | OPD_F_SUR_CLIP | OPD_F_SUR_A_OLD;
     if (a.flags & ~known) OPD_FAIL(h, OPD_ERR_BAD_ARG, "unknown flag bits 0x%x", a.flags & ~known);
+    if (h->seq_n > 0 && !a.stop_after_fwd && (a.mode == OPD_RKL_MC || a.mode == OPD_MIXED) && (a.flags & (OPD_F_SUR_CLIP | OPD_F_SUR_A_OLD)))
+        OPD_FAIL(h, OPD_ERR_BAD_ARG, "opd_set_seq_diagnostics is on: its outputs describe Eq.(15) (A_theta, unclipped ratio) and cannot be "
+                 "combined with OPD_F_SUR_CLIP / OPD_F_SUR_A_OLD (flags 0x%x); switch the hook off for surrogate calls", a.flags);
     const bool fwd_only = (a.flags & OPD_F_FWD_ONLY) || a.stop_after_fwd;
     const bool fp32 = a.dtype == OPD_FP32;
     const int esz = fp32 ? 4 : 2;

@@ -24,7 +24,9 @@ STATIC_SCRATCH_BYTES = 32 << 20          # OPD_STATIC_SCRATCH_BYTES of include/o
 N_PHASES = 4
 PHASE_NAMES = ("prep", "fwd", "est", "bwd")
 
-EXPORTS = ("opd_create", "opd_destroy", "opd_last_error", "opd_version", "opd_workspace_bytes", "opd_set_workspace",
+ABI_VERSION = 3                          # OPD_ABI_VERSION of include/opd.h this binding was written against
+
+EXPORTS = ("opd_create", "opd_destroy", "opd_last_error", "opd_version", "opd_abi_version", "opd_workspace_bytes", "opd_set_workspace",
            "opd_loss_fwd_bwd", "opd_loss_fwd_bwd_static", "opd_loss_fwd_bwd_host", "opd_loss_fwd_bwd_host_submit", "opd_loss_fwd_bwd_host_wait", "opd_debug_logits", "opd_debug_gemm", "opd_last_launch_stats",
            "opd_set_phase_events", "opd_set_diagnostics", "opd_set_seq_diagnostics", "opd_debug_occupy", "opd_cache_workspace_bytes", "opd_cache_topk", "opd_cache_sample",
            "opd_dense_kl_workspace_bytes", "opd_dense_kl_fwd_bwd")
@@ -46,6 +48,12 @@ def load_library():
     if not os.path.exists(LIB_PATH):
         raise OpdError(ERR_CUDA, f"{LIB_PATH} not built: run `python -m paper_2606_24143_b200.build` (no CPU fallback exists)")
     lib = ctypes.CDLL(LIB_PATH)
+    if not hasattr(lib, "opd_abi_version"):
+        raise OpdError(ERR_BAD_ARG, f"{LIB_PATH} predates opd_abi_version (argument lists have changed since): rebuild it")
+    lib.opd_abi_version.restype = c_int
+    if lib.opd_abi_version() != ABI_VERSION:
+        raise OpdError(ERR_BAD_ARG, f"{LIB_PATH} was built with OPD_ABI_VERSION {lib.opd_abi_version()}, this binding expects "
+                                    f"{ABI_VERSION}: rebuild with `python -m paper_2606_24143_b200.build --force`")
     lib.opd_create.argtypes = [POINTER(c_void_p), c_int]
     lib.opd_create.restype = c_int
     lib.opd_destroy.argtypes = [c_void_p]

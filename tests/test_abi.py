@@ -60,6 +60,32 @@ def test_workspace_plan_has_no_logits_sized_buffer(lib):
     assert lib.opd_workspace_bytes(0, 256, 4096, 4, 0, 0, 0) == 0
 
 
+def test_abi_version_is_exported_and_checked(lib):
+    """The header's OPD_ABI_VERSION, the library's opd_abi_version() and the binding's ABI_VERSION agree; the version string moved on
+    from the round-1 "0.1" (argument lists changed since)."""
+    from paper_2606_24143_b200 import opd
+    src = open(os.path.join(ROOT, "include", "opd.h")).read()
+    m = re.search(r"#define\s+OPD_ABI_VERSION\s+(\d+)", src)
+    assert m and int(m.group(1)) == lib.opd_abi_version() == opd.ABI_VERSION >= 3
+    assert b"0.1" not in lib.opd_version()
+    m = re.search(r"#define\s+OPD_STATIC_SCRATCH_BYTES\s+\((\d+)u\s*<<\s*(\d+)\)", src)
+    assert m and int(m.group(1)) << int(m.group(2)) == opd.STATIC_SCRATCH_BYTES
+
+
+def test_bf16_grad_W_keeps_the_tuned_super_tiles(lib):
+    """OPD_F_GRADW_BF16 adds exactly its fp32 sum array (4*d*V bytes, weight-sized) to the workspace and nothing else changes: the
+    4.8% budget of the planner applies to what grows with T, so the flag gets the same super-tile width and G-ring depth."""
+    from gen import synth
+    from paper_2606_24143_b200 import opd
+    for c in (2, 3, 4, 5):
+        cfg = synth.CONFIGS[c]
+        T, d, V, C = cfg["T"], cfg["d"], cfg["V"], max(cfg["k"], cfg["K"])
+        base = lib.opd_workspace_bytes(T, d, V, C, 0, 1, 0)
+        with_bf16 = lib.opd_workspace_bytes(T, d, V, C, 0, 1, opd.F_GRADW_BF16)
+        extra = (4 * d * V + 1023) // 1024 * 1024
+        assert with_bf16 - base == extra, (c, with_bf16 - base, extra)
+
+
 def test_no_cpu_fallback():
     """Without a GPU the product path raises; it never routes anywhere else."""
     import torch

@@ -297,6 +297,18 @@ def test_seq_diagnostics_outputs(handle, opd):
     assert np.abs(f64(out["seq_mean_m"]) - mm).max() <= 2e-3 * np.abs(mm).max()
     assert np.abs(f64(out["seq_mean_1"]) - m1).max() <= 2e-3 * np.abs(m1).max()
     assert np.abs(f64(out["seq_var_m"]) - vm).max() <= 2e-3 * np.abs(vm).max()
+    # surrogate flags would mix objectives in the three outputs (per-token values follow the surrogate, the one-sample terms do
+    # not): refused on the host while the hook is on, accepted again once it is off
+    handle.set_seq_diagnostics(cu)
+    try:
+        for fl in (opd.F_SUR_CLIP, opd.F_SUR_A_OLD, opd.F_SUR_CLIP | opd.F_SUR_A_OLD):
+            with pytest.raises(opd.OpdError) as e:
+                handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, m, O.RKL_MC, kk, flags=fl)
+            assert e.value.status == opd.ERR_BAD_ARG and "opd_set_seq_diagnostics" in str(e.value)
+    finally:
+        handle.set_seq_diagnostics(None)
+    handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, m, O.RKL_MC, kk, flags=opd.F_SUR_CLIP)
+    torch.cuda.synchronize()
 
 
 @pytest.mark.parametrize("case", ["C1", "C2", "ragged_vd", "ragged_sparse"])
