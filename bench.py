@@ -85,6 +85,8 @@ def workload(cfg_id: int, args):
         cfg["T"] = args.tokens
     if args.cache_width:
         cfg["k"] = cfg["K"] = args.cache_width
+    if args.hot_columns:
+        cfg["hot_columns"] = args.hot_columns
     return cfg
 
 
@@ -290,6 +292,8 @@ def main():
     ap.add_argument("--tokens", type=int, default=0, help="override T (debugging)")
     ap.add_argument("--sigma", type=float, default=None, help="staleness of the rollout policy: W_old = W + sigma*N(0,1/d)")
     ap.add_argument("--cache-width", type=int, default=0, help="override the config's k and K (C4's cost-vs-cache-size sweep)")
+    ap.add_argument("--hot-columns", type=int, default=0, help="skewed top-k supports: this many fixed columns sit in (almost) every row's top-k cache "
+                    "(gen/synth.py; the tail case of the sparse backward of --mode rtopk)")
     ap.add_argument("--layout", default="dv", choices=["dv", "vd"], help="storage order of W: [d,V] row-major (BASELINE.json) or [V,d] (lm_head.weight)")
     ap.add_argument("--diag", action="store_true", help="also report rho statistics of the MC cache (opd_set_diagnostics)")
     ap.add_argument("--fwd-only", action="store_true", help="diagnostic: time OPD_F_FWD_ONLY calls (S0-S5: pre-pass, forward contraction, estimators) back to back")

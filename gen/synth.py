@@ -21,6 +21,10 @@ Stress variants (reported / tested, not bench configs): cfg["hidden
 standard deviation 4: a few columns hold most of the mass, most exponentials are tiny); cfg["order"] = "monotone" scales
 column v of the student heads by 0.5 + 1.5 v/V, so column norms grow with the index and the running maximum of a row keeps
 moving to later vocabulary tiles (online-max rescaling); a large sigma gives heavy importance-ratio tails.
+cfg["hot_columns"] = h gives SKEWED SUPPORTS: h fixed columns (spread over the vocabulary: v_i = (i * 9973 + 7) mod V) are
+put into the last h slots of every row's top-k caches (teacher's and stale student's) unless the row already holds them, with
+the teacher's log-prob of that column; real LM supports look like this (a few very common tokens sit in most rows' top-k), and
+one column then owns about T of the T*k cache entries.  Indices stay distinct within a row.
 All cache values are fp32, indices int32.  Rollout settings follow PAPER.md:332 (temperature 1,
 no truncation).  These are stand-ins for the paper's Qwen3 workloads: V=151936 and
 d in {2048,2560,4096} are the 1.7B/4B/8B-class student heads.
@@ -131,9 +135,15 @@ def make_inputs(cfg: dict, c: int = 0, device="cpu", keep_teacher_rows: bool = F
         logq = torch.log_softmax(h @ WTf, dim=-1)
         logpo = torch.log_softmax(h @ Woldf, dim=-1)
         tv, ti = torch.topk(logq, k, dim=-1)               # descending
+        si = torch.topk(logpo, k, dim=-1).indices            # stale student's support S_old = TopK(p_old, k)
+        for j in range(int(cfg.get("hot_columns", 0))):      # skewed supports: see the module docstring
+            col = (j * 9973 + 7) % V
+            for sup in (ti, si):
+                sup[~(sup == col).any(dim=1), k - 1 - j] = col
+        if cfg.get("hot_columns"):
+            tv = torch.gather(logq, 1, ti)
         topk_idx[r0:r1] = ti.to(torch.int32)
         topk_logq[r0:r1] = tv
-        si = torch.topk(logpo, k, dim=-1).indices            # stale student's support S_old = TopK(p_old, k)
         stopk_idx[r0:r1] = si.to(torch.int32)
         stopk_logq[r0:r1] = torch.gather(logq, 1, si)
         a = torch.multinomial(torch.exp(logpo), K, replacement=True, generator=g5)

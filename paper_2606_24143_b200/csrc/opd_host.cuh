@@ -101,7 +101,7 @@ struct Plan {
     int Tb, Vb;           // backward super-tile (rows of tokens x vocabulary columns), multiples of 128 / 256
     int est_blocks;
     size_t off_nlive, off_badidx, off_live_rows, off_xc, off_wsplit, off_sorted, off_perm, off_zc, off_beta,
-           off_partials, off_lse2, off_coef, off_gs, off_dxacc, off_block_sums, off_counters, off_wt, off_skeys, off_shist, off_gw32,
+           off_partials, off_lse2, off_coef, off_gs, off_dxacc, off_block_sums, off_counters, off_wt, off_skeys, off_shist, off_gwseg, off_gw32,
            off_seq_l1, off_seq_var1, total;
     bool sparse_bwd;      // alpha == 0 on every row: gradients live on the cached columns only (no dense backward)
     int n_super;          // number of backward super-tiles (upper bound)
@@ -178,6 +178,7 @@ inline Plan make_plan_cfg(int T, int d, int V, int C, int fp32, unsigned flags, 
     p.sort_blocks = (int)((p.sort_n + RS_TILE - 1) / RS_TILE);
     p.off_skeys = take(bwd && p.sparse_bwd ? 4 * sizeof(uint32_t) * p.sort_n : 0);          // keys / values, ping-pong
     p.off_shist = take(bwd && p.sparse_bwd ? sizeof(uint32_t) * 256 * (size_t)p.sort_blocks : 0);
+    p.off_gwseg = take(bwd && p.sparse_bwd ? sizeof(float) * (p.sort_n / GW_SEG) * (size_t)d : 0);   // per-segment partial sums (hot columns)
     p.off_gw32 = take(bwd && (flags & OPD_F_GRADW_BF16) ? (size_t)d * V * 4 : 0);      // fp32 sums behind a bf16 grad_W
     p.off_seq_l1 = take(sizeof(float) * (size_t)p.t_pad);                               // per-token terms of opd_set_seq_diagnostics
     p.dv_bytes = (p.off_sorted - p.off_wsplit) + (p.off_skeys - p.off_wt) + (p.off_seq_l1 - p.off_gw32);   // each followed by the next take()

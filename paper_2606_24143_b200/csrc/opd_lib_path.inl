@@ -271,10 +271,18 @@ static opd_status_t run_path(opd_handle_s* h, cudaStream_t st, const PathIO& a) 
             k_radix_scatter<<<p.sort_blocks, 256, 0, st>>>(kbuf[cur], vbuf[cur], N, shift, hist, p.sort_blocks, kbuf[cur ^ 1], vbuf[cur ^ 1]);
             h->n_kernels += 3;
         }
+        // hot columns: segments of GW_SEG sorted entries that lie inside one column's run are summed first, all in parallel
+        float* part = reinterpret_cast<float*>(ws + p.off_gwseg);
+        const dim3 seg_grid((unsigned)(N / GW_SEG), (unsigned)ceil_div(d, GW_KCHUNK));
+        if (seg_grid.x) {
+            if (fp32) k_sparse_gw_seg<float><<<seg_grid, 256, 0, st>>>(kbuf[cur], vbuf[cur], V, C, beta, live_rows, a.hidden, a.ld_hidden, d, part);
+            else k_sparse_gw_seg<__nv_bfloat16><<<seg_grid, 256, 0, st>>>(kbuf[cur], vbuf[cur], V, C, beta, live_rows, a.hidden, a.ld_hidden, d, part);
+            h->n_kernels++;
+        }
         if (fp32) k_sparse_gw<float><<<V / 8, 256, 0, st>>>(kbuf[cur], vbuf[cur], N, V, C, beta, live_rows, a.hidden, a.ld_hidden, d,
-                                                             gw32, ldgw32, wl, gw_accum ? 1 : 0);
+                                                             part, gw32, ldgw32, wl, gw_accum ? 1 : 0);
         else k_sparse_gw<__nv_bfloat16><<<V / 8, 256, 0, st>>>(kbuf[cur], vbuf[cur], N, V, C, beta, live_rows, a.hidden, a.ld_hidden, d,
-                                                                gw32, ldgw32, wl, gw_accum ? 1 : 0);
+                                                                part, gw32, ldgw32, wl, gw_accum ? 1 : 0);
         h->n_kernels += 3;
         OPD_CUDA(h, cudaGetLastError());
     }

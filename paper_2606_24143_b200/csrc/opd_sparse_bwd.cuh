@@ -6,6 +6,12 @@
 // added in (token, slot) order by ONE block: no atomics, bit-reproducible, and grad_W is written exactly once (zeros
 // where no token cached the column).  W is read as contiguous d-vectors per column: the caller's array when it is stored
 // [V,d], else a transposed scratch copy (k_transpose); grad_W is written in the caller's layout directly.
+// Hot columns (real top-k supports: a few tokens such as punctuation sit in the support of most rows, so one column's
+// run holds 1e4-1e5 entries): the sorted entry array is cut into fixed segments of GW_SEG entries; every segment that
+// lies inside ONE column's run is summed by its own block beforehand (k_sparse_gw_seg, the whole grid in parallel), and
+// the column's block adds these partial sums in segment order instead of walking the entries.  Which segments qualify
+// depends on the sorted keys only, so the summation order stays fixed and the result bit-reproducible; a support
+// without such runs takes exactly the arithmetic path it took before.
 #pragma once
 #include "opd_small_kernels.cuh"
 
@@ -15,6 +21,19 @@ template <typename T>
 __device__ __forceinline__ float ld_as_float(const void* base, size_t i) {
     if constexpr (sizeof(T) == 2) return __bfloat162float(static_cast<const __nv_bfloat16*>(base)[i]);
     else return static_cast<const float*>(base)[i];
+}
+
+// four consecutive elements starting at element i (i % 4 == 0, base 16-byte aligned) as floats, one vector load
+template <typename T>
+__device__ __forceinline__ void ld4_as_float(const void* base, size_t i, float (&x)[4]) {
+    if constexpr (sizeof(T) == 2) {
+        const uint2 v = *reinterpret_cast<const uint2*>(static_cast<const __nv_bfloat16*>(base) + i);
+        x[0] = __uint_as_float(v.x << 16); x[1] = __uint_as_float(v.x & 0xffff0000u);
+        x[2] = __uint_as_float(v.y << 16); x[3] = __uint_as_float(v.y & 0xffff0000u);
+    } else {
+        const float4 v = *reinterpret_cast<const float4*>(static_cast<const float*>(base) + i);
+        x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
+    }
 }
 
 // grad_hidden row of one live token (one block per compact row); columns in ascending order: a fixed summation order
@@ -136,12 +155,44 @@ __global__ void __launch_bounds__(256) k_radix_scatter(const uint32_t* __restric
 // are added in run order (token, slot).  [d,V] storage: the 8 columns of a k-chunk are staged in shared memory and
 // written as 32-byte rows; [V,d] storage: each column's d-vector is written directly.
 constexpr int GW_KCHUNK = 1024;    // k values per pass of a block (4 per thread)
+constexpr int GW_SEG = 256;        // entries per segment of the sorted entry array (hot columns: summed per segment first)
+
+// Partial sums of the segments that lie inside one column's run: part[s][0..d) = sum over the GW_SEG entries of segment s, in
+// entry order, of beta * x.  Grid (N / GW_SEG, ceil(d / GW_KCHUNK)); blocks of other segments return at once.
+template <typename T>
+__global__ void __launch_bounds__(256) k_sparse_gw_seg(const uint32_t* __restrict__ scol, const uint32_t* __restrict__ sent, int V, int C,
+                                                       const float* __restrict__ beta, const int* __restrict__ live_rows,
+                                                       const void* __restrict__ hidden, long ld_hidden, int d, float* __restrict__ part) {
+    __shared__ float sb[GW_SEG];
+    __shared__ size_t srow[GW_SEG];
+    const size_t e0 = static_cast<size_t>(blockIdx.x) * GW_SEG;
+    const uint32_t col = scol[e0];
+    if (col >= static_cast<uint32_t>(V) || scol[e0 + GW_SEG - 1] != col) return;      // sorted: first == last means one column
+    for (int i = threadIdx.x; i < GW_SEG; i += 256) {
+        const uint32_t ent = sent[e0 + i];
+        sb[i] = beta[ent];
+        srow[i] = static_cast<size_t>(live_rows[ent / C]) * ld_hidden;
+    }
+    __syncthreads();
+    const int k = blockIdx.y * GW_KCHUNK + threadIdx.x * 4;
+    if (k >= d) return;
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll 4
+    for (int i = 0; i < GW_SEG; ++i) {
+        float x[4];
+        ld4_as_float<T>(hidden, srow[i] + k, x);
+        const float b = sb[i];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[j] = fmaf(b, x[j], acc[j]);
+    }
+    *reinterpret_cast<float4*>(part + static_cast<size_t>(blockIdx.x) * d + k) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+}
 
 template <typename T>
 __global__ void __launch_bounds__(256) k_sparse_gw(const uint32_t* __restrict__ scol, const uint32_t* __restrict__ sent, size_t N, int V, int C,
                                                    const float* __restrict__ beta, const int* __restrict__ live_rows,
                                                    const void* __restrict__ hidden, long ld_hidden, int d,
-                                                   float* __restrict__ gw, long ldgw, int wl, int accumulate) {
+                                                   const float* __restrict__ part, float* __restrict__ gw, long ldgw, int wl, int accumulate) {
     __shared__ size_t range[2];
     __shared__ float tile[GW_KCHUNK][8 + 1];
     const uint32_t c0 = blockIdx.x * 8u;
@@ -170,16 +221,27 @@ __global__ void __launch_bounds__(256) k_sparse_gw(const uint32_t* __restrict__ 
             }
             acc[0] = acc[1] = acc[2] = acc[3] = 0.f;
         };
-        for (size_t e = lo; e < hi; ++e) {
+        for (size_t e = lo; e < hi;) {
             const uint32_t col = scol[e];
             while (cur < col) { flush(cur); ++cur; }
+            if (e % GW_SEG == 0 && e + GW_SEG <= hi && scol[e + GW_SEG - 1] == col) {
+                // a whole segment of this column: k_sparse_gw_seg has summed it (same test there, on the sorted keys only)
+                if (kin) {
+                    const float4 p = *reinterpret_cast<const float4*>(part + (e / GW_SEG) * d + k);
+                    acc[0] += p.x; acc[1] += p.y; acc[2] += p.z; acc[3] += p.w;
+                }
+                e += GW_SEG;
+                continue;
+            }
             if (kin) {
                 const uint32_t ent = sent[e];
                 const float b = beta[ent];
-                const size_t row = static_cast<size_t>(live_rows[ent / C]) * ld_hidden + k;
+                float x[4];
+                ld4_as_float<T>(hidden, static_cast<size_t>(live_rows[ent / C]) * ld_hidden + k, x);
 #pragma unroll
-                for (int j = 0; j < 4; ++j) acc[j] = fmaf(b, ld_as_float<T>(hidden, row + j), acc[j]);
+                for (int j = 0; j < 4; ++j) acc[j] = fmaf(b, x[j], acc[j]);
             }
+            ++e;
         }
         while (cur < c0 + 8u) { flush(cur); ++cur; }
         if (wl == 0) {                                      // rows of 8 floats: grad_W[k][c0 .. c0 + 8)

@@ -119,6 +119,29 @@ def test_ragged_shapes_and_super_tiles(handle, dtype, mode, tiles, monkeypatch):
         assert handle.launch_stats()["super_rows"] == tiles[0]
 
 
+@pytest.mark.parametrize("dtype", ["bf16", "fp32"])
+@pytest.mark.parametrize("mode,flags", [(O.RKL_TOPK, 0), (O.FKL_TOPK, O.F_RENORM_STUDENT)])
+@pytest.mark.parametrize("layout", ["dv", "vd"])
+def test_sparse_backward_hot_columns(handle, dtype, mode, flags, layout):
+    """Skewed supports (gen/synth hot_columns): three columns sit in the support of (almost) every row, so their runs of sorted
+    cache entries are ~1350 long and span several of the sparse backward's 256-entry segments (summed by k_sparse_gw_seg and added
+    in segment order); d = 1280 needs two k-chunks.  Element-wise against the oracle, and bitwise equal on a second call."""
+    cfg = dict(dtype=dtype, T=1500, d=1280, V=2056, k=8, K=4, sigma=0.05, mask="random10", hot_columns=3)
+    inp = synth.make_inputs(cfg, c=23, device=DEV)
+    idx, lam, old, kk = pick(inp, cfg, mode)
+    live = inp["mask"] != 0
+    assert int((idx[live] == 7).sum()) > 4 * 256                    # the hot column's run really spans several segments
+    r = run(handle, inp, idx, lam, old, mode, kk, flags, layout)
+    compare_all(r, oracle_for(inp, idx, lam, old, mode, kk, flags), f64(inp["mask"]), dtype)
+    r2 = run(handle, inp, idx, lam, old, mode, kk, flags, layout)
+    assert torch.equal(r["grad_W"], r2["grad_W"]) and torch.equal(r["grad_hidden"], r2["grad_hidden"])
+    W = inp["W"] if layout == "dv" else inp["W"].t().contiguous().t()
+    gw = torch.empty_strided(tuple(W.shape), W.stride(), dtype=torch.float32, device=DEV).fill_(1.0)
+    r3 = handle.loss_fwd_bwd(inp["hidden"], W, idx, lam, old, inp["mask"], mode, kk, flags=flags | 4, grad_W=gw)   # OPD_F_GRADW_ACCUM: added onto 1.0
+    torch.cuda.synchronize()
+    assert (r3["grad_W"] - 1.0 - r["grad_W"]).abs().max() <= 1e-6 * max(1.0, float(r["grad_W"].abs().max()))
+
+
 STRESS = {
     "peaked": dict(hidden_scale=4.0, sigma=0.05),                   # a few columns hold the mass, most exponentials are tiny
     "monotone": dict(order="monotone", sigma=0.05),                 # the row maximum keeps moving to later vocabulary tiles
