@@ -5,8 +5,10 @@
 
 A "step" is one pass of the whole hot path (pre-pass, forward contraction + LSE + gather, estimators,
 backward super-tiles) over one batch of seeded synthetic input.  Prints ONE JSON line (rank 0).
-Under torchrun (N>1) every rank runs its own token shard (replicas of W, no data-path collective:
-DESIGN.md "Multi-GPU"), timing = max over ranks, value = tokens of all ranks / that time ("weak").
+Under torchrun (N>1) every rank runs its own token shard against a replica of W (no collective inside the loss itself:
+DESIGN.md "Multi-GPU"); the exchange a data-parallel learner needs after it (all-reduce of loss and grad_W over NCCL, on a side
+stream, overlapping the next step) is inside the timed region and reported under "collective".  Timing = max over ranks,
+value = tokens of all ranks / that time ("weak").
 """
 from __future__ import annotations
 
@@ -27,11 +29,28 @@ METRIC = "OPD loss fwd+bwd tokens/s on 1 B200; % of dense BF16 tensor peak"
 UNIT = "live tokens/s"
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from one committed `ncu --set full` capture of this
-# workload (a citation: bench.py never runs under a profiler, so the line carries "traffic_measured": false)
-NCU_TRAFFIC = {
-    "C4": dict(bwd_kernel=139_389_495_000, fwd_kernel=10_921_094_000, source="profiles/r02_final_c4.md"),
-}
+def csrc_sha16() -> str:
+    """sha256 (first 16 hex digits) over include/opd.h and the kernel sources, in name order: identifies the build a capture under
+    profiles/ belongs to (the GPU box has no .git, so a commit id is not available at run time)."""
+    import hashlib
+    from paper_2606_24143_b200 import build
+    hsh = hashlib.sha256()
+    for f in build.sources():
+        hsh.update(os.path.basename(f).encode() + b"\0" + open(f, "rb").read())
+    return hsh.hexdigest()[:16]
+
+
+def ncu_traffic(workload_key: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of this workload
+    (profiles/ncu_traffic.json names the capture and the command). bench.py never runs under a profiler, so this is a citation
+    ("traffic_measured": false), and it is only given while the kernel sources are the ones the capture was taken from."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(p):
+        return None
+    ent = json.load(open(p)).get(workload_key)
+    if not ent or ent.get("csrc_sha16") != csrc_sha16():
+        return None
+    return ent
 
 
 def config_dict(cfg, mode_name, C, sigma):
@@ -228,9 +247,13 @@ def run_producer_bench(args, h, inp, cfg, dev, world, rank, dist):
         th = torch.randn(T, d, device=dev, generator=g).to(inp["hidden"].dtype)
         wt = (torch.randn(d, V, device=dev, generator=g) * d ** -0.5).to(inp["W"].dtype)
         gh = torch.empty_like(inp["hidden"]); gw = torch.empty(d, V, dtype=torch.float32, device=dev)
-        call = lambda: h.dense_kl_fwd_bwd(inp["hidden"], inp["W"], th, wt, inp["mask"], grad_hidden=gh, grad_W=gw)
+        from paper_2606_24143_b200 import opd as _opd
+        dflags = _opd.F_DENSE_REVERSE if args.reverse else 0
+        call = lambda: h.dense_kl_fwd_bwd(inp["hidden"], inp["W"], th, wt, inp["mask"], flags=dflags, grad_hidden=gh, grad_W=gw)
         n_tok = int((inp["mask"] != 0).sum().item())
-        flops = 12.0 * d * V * n_tok    # two forward heads, Q and G re-formation, grad_hidden, grad_W: 2 d V each
+        # two forward heads, Q and G re-formation, grad_hidden, grad_W: 2 d V each; the reverse direction re-forms both heads
+        # once more in the streamed pass that produces the per-token value before the gradient tiles
+        flops = (16.0 if args.reverse else 12.0) * d * V * n_tok
         n = 0
     elif args.op == "topk":
         call = lambda: h.cache_topk(inp["hidden"], Wt, n)
@@ -264,10 +287,10 @@ def run_producer_bench(args, h, inp, cfg, dev, world, rank, dist):
     ach = flops / (ms * 1e-3) / 1e12
     st = h.launch_stats()
     line = dict(metric=(f"cache producer ({args.op}) tokens scored/s on 1 B200" if args.op != "dense" else
-                        "dense two-head forward KL fwd+bwd tokens/s on 1 B200"), value=n_tok * world / (ms * 1e-3), unit="live tokens/s" if args.op == "dense" else "tokens/s", n_gpus=world,
+                        ("dense two-head reverse KL fwd+bwd tokens/s on 1 B200" if args.reverse else "dense two-head forward KL fwd+bwd tokens/s on 1 B200")), value=n_tok * world / (ms * 1e-3), unit="live tokens/s" if args.op == "dense" else "tokens/s", n_gpus=world,
                 steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="bf16" if cfg["dtype"] == "bf16" else "f32(3xbf16)", data="synthetic",
-                config=dict(workload=(f"{cfg['name']} opd_cache_{args.op} n={n}" if args.op != "dense" else f"{cfg['name']} opd_dense_kl_fwd_bwd dT=d"),
+                config=dict(workload=(f"{cfg['name']} opd_cache_{args.op} n={n}" if args.op != "dense" else f"{cfg['name']} opd_dense_kl_fwd_bwd dT=d" + (" reverse" if args.reverse else "")),
                             T=T, d=d, V=V,
                             l2_policy="inputs larger than L2 (W alone is %.0f MB)" % (d * V * 2 / 1e6)),
                 clocks=clocks, e2e=None, gpu_launches=st["kernels"] * args.steps,
@@ -297,6 +320,10 @@ def main():
     ap.add_argument("--layout", default="dv", choices=["dv", "vd"], help="storage order of W: [d,V] row-major (BASELINE.json) or [V,d] (lm_head.weight)")
     ap.add_argument("--diag", action="store_true", help="also report rho statistics of the MC cache (opd_set_diagnostics)")
     ap.add_argument("--fwd-only", action="store_true", help="diagnostic: time OPD_F_FWD_ONLY calls (S0-S5: pre-pass, forward contraction, estimators) back to back")
+    ap.add_argument("--force-dist", action="store_true", help="run the N > 1 code path (global normaliser, all-reduce of loss and grad_W on a side "
+                    "stream) with a one-rank NCCL group: a test aid for boxes with one GPU")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the >= 4 s back-to-back loop that follows a timed region shorter than 4 s")
+    ap.add_argument("--reverse", action="store_true", help="--op dense: the reverse direction KL(p || q) (OPD_F_DENSE_REVERSE)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-probe", action="store_true", help="skip the same-box cuBLAS measurement (3 s, after the timed steps)")
@@ -317,8 +344,10 @@ def main():
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     dist = None
-    if world > 1:
+    if world > 1 or args.force_dist:
         import torch.distributed as dist
+        if "RANK" not in os.environ:                  # --force-dist without torchrun: a one-rank group on this process
+            os.environ.update(RANK="0", WORLD_SIZE="1", MASTER_ADDR="127.0.0.1", MASTER_PORT=os.environ.get("MASTER_PORT", "29533"))
         dist.init_process_group("nccl", device_id=dev)
 
     from gen import synth
@@ -356,8 +385,43 @@ def main():
     else:
         gw = torch.empty(d, V, dtype=torch.float32, device=dev)
 
+    # N > 1: every rank runs its own token shard against a replica of W with the GLOBAL live count as the
+    # normaliser, and what a data-parallel learner must exchange afterwards is inside the timed region: loss and grad_W (fp32
+    # d x V: 2.49 GB at C4) are all-reduced over NCCL on a side stream, so the reduction of step i overlaps the kernels of step
+    # i + 1 (two grad_W buffers alternate; a buffer is not written again before its all-reduce has finished).
+    norm = 0.0
+    comm = None
+    if dist is not None:
+        ng = torch.tensor([n_live], device=dev, dtype=torch.int64)
+        dist.all_reduce(ng)
+        norm = float(ng.item())
+        comm = dict(stream=torch.cuda.Stream(dev), bufs=[gw, torch.empty_like(gw)], done=[None, None], i=0, spans=[])
+
     def step():
-        return h.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, grad_hidden=gh, grad_W=gw)
+        if comm is None:
+            return h.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, grad_hidden=gh, grad_W=gw)
+        b = comm["i"] % 2
+        comm["i"] += 1
+        if comm["done"][b] is not None:
+            torch.cuda.current_stream(dev).wait_event(comm["done"][b])       # the buffer's previous all-reduce
+        r = h.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, norm_override=norm, grad_hidden=gh,
+                           grad_W=comm["bufs"][b])
+        ready = torch.cuda.Event()
+        ready.record()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(comm["stream"]):
+            comm["stream"].wait_event(ready)
+            a0.record()
+            dist.all_reduce(r["loss"])
+            dist.all_reduce(comm["bufs"][b])
+            a1.record()
+        comm["done"][b] = a1
+        comm["spans"].append((a0, a1))
+        return r
+
+    def drain():                                        # the last all-reduces belong to the timed region
+        if comm is not None:
+            torch.cuda.current_stream(dev).wait_stream(comm["stream"])
 
     def barrier():
         if dist is not None:
@@ -366,7 +430,10 @@ def main():
 
     for _ in range(max(args.warmup, 3)):
         r = step()
+    drain()
     barrier()
+    if comm is not None:
+        comm["spans"].clear()
     stats = h.launch_stats()
     phase_sets = [h.new_phase_events() for _ in range(args.steps)]      # one set of phase events per timed step
     sampler = ClockSampler(local) if rank == 0 else None
@@ -376,10 +443,22 @@ def main():
     for i in range(args.steps):
         h.use_phase_events(phase_sets[i])
         r = step()
+        if i == args.steps - 1:
+            drain()
         ev[i + 1].record()
     barrier()
     h.use_phase_events(None)
     total_ms = ev[0].elapsed_time(ev[-1])
+    collective = None
+    if comm is not None:
+        ar = [a.elapsed_time(b) for a, b in comm["spans"]]
+        comm["spans"].clear()
+        compute_ms = float(np.sum([sum(q.values()) for q in [h.phase_times_ms(ps) for ps in phase_sets]]))
+        collective = dict(what="all_reduce(loss) + all_reduce(grad_W fp32 d x V) per step over NCCL, side stream, two grad_W buffers",
+                          bytes_per_step=int(gw.numel() * 4 + 4), allreduce_ms=float(np.mean(ar)),
+                          exposed_ms_per_step=max(0.0, (total_ms - compute_ms) / args.steps),
+                          overlap_hidden_ms=max(0.0, float(np.mean(ar)) - max(0.0, (total_ms - compute_ms) / args.steps)),
+                          norm_override=norm)
     step_ms = [round(ev[i].elapsed_time(ev[i + 1]), 3) for i in range(args.steps)]
     per_step = [h.phase_times_ms(ps) for ps in phase_sets]               # every timed step, CUDA events on the launching stream
     pm = {k: float(np.mean([q[k] for q in per_step])) for k in opd.PHASE_NAMES}          # average over the timed steps
@@ -397,6 +476,31 @@ def main():
         n_live_all = n_live
     ms_per_step = total_ms / args.steps
     value = n_live_all / (ms_per_step * 1e-3)
+    # SURVEY 8(d) protocol: a timed region shorter than 4 s does not reach the power-capped steady state the sustained peak was
+    # measured in, so a second loop of back-to-back steps runs for at least 4 s (the way MEASURED_PEAKS.json's sustained figure
+    # was taken) and is reported beside the contract's K-step number
+    sustained = None
+    if total_ms < 4000.0 and not args.no_sustained:
+        n_sus = int(4200.0 / max(ms_per_step, 1e-3)) + 1
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        s0.record()
+        for _ in range(n_sus):
+            step()
+        drain()
+        s1.record()
+        barrier()
+        sus_ms = s0.elapsed_time(s1)
+        if dist is not None:
+            t = torch.tensor([sus_ms], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            sus_ms = float(t.item())
+        sustained = dict(steps=n_sus, seconds=sus_ms * 1e-3, ms_per_step=sus_ms / n_sus, value=n_live_all / (sus_ms / n_sus * 1e-3))
+    ws_bytes = h.workspace_bytes(T, d, V, idx.shape[1], opd.BF16 if cfg["dtype"] == "bf16" else opd.FP32, mode)
+    free_b, total_b = torch.cuda.mem_get_info(dev)
+    memory = dict(torch_peak_allocated_bytes=int(torch.cuda.max_memory_allocated(dev)), opd_workspace_bytes=int(ws_bytes),
+                  device_used_bytes=int(total_b - free_b), device_total_bytes=int(total_b),
+                  note="device_used = everything on the GPU after the timed steps (inputs, generator leftovers in torch's cache, outputs, libopd workspace, CUDA context)")
 
     # ---- e2e: same call through the C ABI with HOST buffers (H2D + D2H inside the timed region)
     e2e = None
@@ -410,6 +514,8 @@ def main():
                         grad_W=torch.empty(d, V, dtype=torch.float32).pin_memory())
         outs = [host_out(), host_out()]
         del gw, gh
+        if comm is not None:
+            comm["bufs"] = None
         torch.cuda.empty_cache()
         n_e2e = max(2, min(args.steps, 20))      # the fill (first copy-in) and drain (last copy-out) of the pipeline are inside the timed region
 
@@ -483,7 +589,7 @@ def main():
     bwd_flops, fwd_flops = 6.0 * d * V * n_live, 2.0 * d * V * n_live
     ach = bwd_flops / (pm["bwd"] * 1e-3) / 1e12
     ach_fwd = fwd_flops / (pm["fwd"] * 1e-3) / 1e12
-    tr = NCU_TRAFFIC.get(f"C{args.config}") if args.mode == "mc" and not args.tokens else None
+    tr = ncu_traffic(f"C{args.config} {args.mode}") if not (args.tokens or args.cache_width or args.hot_columns or args.sigma is not None) else None
     roofline = dict(bound="tensor", achieved=ach, peak=pk["sustained"], unit="TFLOP/s", frac=ach / pk["sustained"],
                     traffic=tr["bwd_kernel"] if tr else None, traffic_measured=False,
                     kernel="opd::bwd_kernel<2,false> (persistent: G re-formation, grad_hidden, grad_W tiles on tcgen05 cta_group::2)",
@@ -512,6 +618,8 @@ def main():
                 dtype="bf16" if cfg["dtype"] == "bf16" else "f32(3xbf16)", data="synthetic",
                 config=config_dict(cfg, args.mode, idx.shape[1], inp["sigma"]),
                 launch=dict(live_tokens_per_gpu=n_live, super_tile=[stats["super_rows"], stats["super_cols"]], layout=args.layout),
+                all_T_tokens_per_s=(T * world / (ms_per_step * 1e-3) if n_live < T else None),   # padding rows counted too (C3)
+                sustained=sustained, memory=memory, collective=collective,
                 pct_of_bf16_peak=dict(executed_8dV_vs_burst=100 * whole / pk["burst"], executed_8dV_vs_sustained=100 * whole / pk["sustained"],
                                       model_6dV_vs_burst=100 * whole * 0.75 / pk["burst"], tflops_executed=whole, peaks=pk, same_box_cublas=box),
                 phase_ms=pm, phase_ms_per_step=phase_steps, step_ms=step_ms, loss=loss_val, clocks=clocks, e2e=e2e, gpu_launches=stats["kernels"] * args.steps,

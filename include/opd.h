@@ -82,12 +82,14 @@ int opd_abi_version(void);
 /* workspace ------------------------------------------------------------------------------------
  * Bytes of device scratch one opd_loss_fwd_bwd call with these arguments needs. No buffer of size
  * O(T*V) exists: the largest items are the compacted copy of hidden (T*d), the per-tile (max,sumexp)
- * partials (T*ceil(V/256)*8 B) and, aliased with them, a two-deep ring of bounded super-tiles of re-formed softmax
- * gradients G (at most 4608 x 4096 bf16 each) plus fp32 grad_hidden partial sums of one token super-tile, consumed out of L2 by
- * the backward contractions (C4: 431 MB in total, 4.3% of the bf16 logits). The modes whose gradient is purely sparse
+ * partials (T*ceil(V/256)*8 B) and, aliased with them, a two- or three-deep ring of bounded super-tiles of re-formed softmax
+ * gradients G (up to 4096 token rows x 16384 vocabulary columns of bf16 each; the planner takes the widest that keeps the
+ * T-dependent scratch under 4.8% of the bf16 logits) plus fp32 grad_hidden partial sums of one token super-tile, consumed out
+ * of L2 by the backward contractions (C4: 4096 x 8192 tiles, 477 MB in total, 4.8% of the bf16 logits). The modes whose gradient is purely sparse
  * (OPD_RKL_TOPK; OPD_FKL_TOPK with OPD_F_RENORM_STUDENT) instead need 16 bytes per cache entry for a column sort (their
  * grad_W is a segmented sum per column, bit-reproducible, no atomics) and, only when W is stored [d,V], a transposed copy of
- * W (2*d*V bytes for bf16; a [V,d] lm_head.weight needs none). OPD_F_GRADW_BF16 adds 4*d*V bytes (fp32 sums behind the bf16 grad_W).
+ * W (2*d*V bytes for bf16; a [V,d] lm_head.weight needs none), plus 4*d bytes per 256 cache entries for the partial sums of
+ * hot columns. OPD_F_GRADW_BF16 adds 4*d*V bytes (fp32 sums behind the bf16 grad_W).
  * The handle-owned workspace only grows: a call that needs more than any earlier call on the handle frees and reallocates
  * it, which synchronises the device (that one call is not asynchronous) and is refused inside a stream capture
  * (OPD_ERR_WORKSPACE: run the shapes once eagerly first, or provide the memory with opd_set_workspace). */

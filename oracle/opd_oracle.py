@@ -241,10 +241,13 @@ def opd_oracle(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, m
 
 
 def grad_W_columns(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mask, mode, k_or_K,
-                   cols, flags: int = 0, norm_override: float = 0.0, chunk: int = 512):
+                   cols, flags: int = 0, norm_override: float = 0.0, chunk: int = 512,
+                   surrogate: int = SUR_THETA_NOCLIP, clip_eps: float = 0.2):
     """O9 restricted to the vocabulary columns ``cols``: grad_W[:, cols]  ([d, len(cols)]).
 
     Every live token contributes to every column, so this still runs O1-O2 for all live tokens.
+    ``surrogate`` / ``clip_eps``: the reverse-KL surrogate of Eq.(4),(6),(7), handed to
+    ``token_terms`` exactly as ``opd_oracle`` does (pinned against it for all four surrogates).
     """
     X = np.asarray(hidden, dtype=np.float64)
     Wd = np.asarray(W, dtype=np.float64)
@@ -270,7 +273,7 @@ def grad_W_columns(hidden, W, cache_idx, cache_teacher_logp, cache_old_logp, mas
             C = k_f if tmode == FKL_TOPK else K_m
             a = idx[t, :C]
             old = None if old_all is None else old_all[t, :C]
-            _, alpha, beta = token_terms(tmode, lam_all[t, :C], old, logp[i, a], flags)
+            _, alpha, beta = token_terms(tmode, lam_all[t, :C], old, logp[i, a], flags, surrogate, clip_eps)
             g = alpha * np.exp(logp[i, cols])
             for j in range(C):
                 g += beta[j] * (cols == a[j])
@@ -481,3 +484,32 @@ def dense_kl_oracle(hidden, W, teacher_hidden, W_T, mask, norm_override: float =
         gh[tt] = G @ Wd.T
         gW += X[tt].T @ G
     return dict(loss=float(np.sum(per_token)) * scale, N=N, per_token_kl=per_token, grad_hidden=gh, grad_W=gW)
+
+
+def dense_grad_W_columns(hidden, W, teacher_hidden, W_T, mask, cols, norm_override: float = 0.0, chunk: int = 512,
+                         reverse: bool = False):
+    """grad_W[:, cols] of ``dense_kl_oracle`` ([d, len(cols)]) without holding the [d,V] gradient: the same per-token logit
+    gradients (Eq.(1): p - q;  reverse, Eq.(2),(3) PAPER.md:63-68: p (log p - log q - L_t)), restricted to the
+    columns ``cols`` before the contraction with hidden (O9).  Both softmaxes still run over the whole vocabulary."""
+    X = np.asarray(hidden, dtype=np.float64)
+    Wd = np.asarray(W, dtype=np.float64)
+    XT = np.asarray(teacher_hidden, dtype=np.float64)
+    WT = np.asarray(W_T, dtype=np.float64)
+    msk = np.asarray(mask).astype(np.int64)
+    cols = np.asarray(cols, dtype=np.int64)
+    N = float(np.count_nonzero(msk))
+    norm = float(norm_override) if norm_override > 0 else N
+    scale = 0.0 if norm == 0 else 1.0 / norm
+    out = np.zeros((X.shape[1], cols.size))
+    live = np.flatnonzero(msk)
+    for s in range(0, live.size, chunk):
+        tt = live[s:s + chunk]
+        logp, _ = log_softmax_rows(X[tt] @ Wd)
+        logq, _ = log_softmax_rows(XT[tt] @ WT)
+        if reverse:
+            Lt = np.sum(np.exp(logp) * (logp - logq), axis=1)
+            Gc = np.exp(logp[:, cols]) * (logp[:, cols] - logq[:, cols] - Lt[:, None])
+        else:
+            Gc = np.sum(np.exp(logq), axis=1, keepdims=True) * np.exp(logp[:, cols]) - np.exp(logq[:, cols])
+        out += X[tt].T @ (Gc * scale)
+    return out

@@ -36,7 +36,7 @@ constexpr int PUB_Q = 4;                              // tiles the epilogue warp
 constexpr int EPI_SMEM_BYTES = 32768;                 // 4 epilogue warps x 2 staging buffers x (32 rows x 128 B)
 constexpr int TMEM_COLS = 512;                        // 2 accumulator stages x 256 columns
 constexpr int MAX_STAGES = 6;
-// TMA ring depth of the CTA-pair configuration (32 KiB per stage), per kernel (profiles/r02_ring_depth.md):
+// TMA ring depth of the CTA-pair configuration (32 KiB per stage), per kernel (profiles/r02_experiments.md section 3):
 //   one-GEMM kernels (forward logits, producers): 4 stages keep the tensor pipe 98% busy and read W from HBM about once per
 //     token panel (10.6 GB per C4 launch; 6 stages let the pairs sharing a panel drift apart and re-fetch 46 GB);
 //   persistent backward: its operands miss L2 more often (G ring, partial sums, two W panels), 6 stages hide that latency

@@ -4,7 +4,8 @@ Tolerances (BASELINE.json north_star; derivations in DESIGN.md "Tolerances"):
   loss            |dloss| <= 2e-3 * max(|loss_ref|, mean_t |L_t,ref|)
   gradients       max|g - g_ref| <= tol * max|g_ref|, tol = 1e-2 (bf16 inputs) / 1e-4 (fp32 inputs)
   gathers         bit-exact against the logits the same kernel held (debug entry); against the fp64 oracle
-                  the student log-probs agree to 1e-4 absolute (fp32 accumulation over d terms)
+                  the student log-probs and lse agree to 1e-4 absolute with bf16 inputs (fp32 accumulation over d terms)
+                  and to 1e-5 with fp32 inputs
 """
 import numpy as np
 import torch
@@ -14,7 +15,21 @@ from gen import synth
 
 GRAD_TOL = {"bf16": 1e-2, "fp32": 1e-4}
 LOSS_RTOL = 2e-3
-LOGP_ATOL = 1e-4
+LOGP_ATOL = 1e-4                                   # bf16 inputs, and the producers' scores
+LOGP_ATOL_BY_DTYPE = {"bf16": 1e-4, "fp32": 1e-5}  # the fp32 path (3 x bf16 split, fp32 accumulation) is held to 1e-5
+
+
+def logp_bar(dtype, ref, live):
+    """Absolute bar on lse / student log-probs.  bf16 inputs: 1e-4.  fp32 inputs: 1e-5 while the logits stay within +-5 (the
+    workloads: N(0,1) logits, |z| < 5 at the cached positions); the error of an fp32 sum over d products is a few ulps of the
+    sum's magnitude, so beyond that the bar grows in proportion to the largest cached logit of the call (stress inputs with
+    |z| ~ 20-30: 4e-5 - 6e-5, still half the bf16 bar)."""
+    bar = LOGP_ATOL_BY_DTYPE[dtype]
+    if dtype == "fp32" and ref.get("student_logp") is not None and live.any():
+        z = np.abs(ref["student_logp"][live] + ref["lse"][live][:, None])
+        if np.isfinite(z).any():
+            bar *= max(1.0, float(np.nanmax(z)) / 5.0)
+    return bar
 
 
 def f64(t):
@@ -54,13 +69,16 @@ def compare_all(r, ref, mask, dtype):
     bar = LOSS_RTOL * max(1e-30, float(np.abs(ref["per_token_kl"]).max()))
     assert np.abs(ptk - ref["per_token_kl"]).max() <= bar
     assert np.all(ptk[~live] == 0)
+    lbar = logp_bar(dtype, ref, live)
     if r.get("lse") is not None:
-        assert np.abs(f64(r["lse"])[live] - ref["lse"][live]).max() <= LOGP_ATOL
+        err = np.abs(f64(r["lse"])[live] - ref["lse"][live]).max()
+        assert err <= lbar, f"lse: max err {err:.3e} vs {lbar:.1e}"
     if r.get("student_logp") is not None:
         a, b = f64(r["student_logp"])[live], ref["student_logp"][live]
         used = ~np.isnan(b)
         assert np.array_equal(np.isnan(a), ~used)            # unused slots are not written
-        assert np.abs(a[used] - b[used]).max() <= LOGP_ATOL
+        err = np.abs(a[used] - b[used]).max()
+        assert err <= lbar, f"student_logp: max err {err:.3e} vs {lbar:.1e}"
     if r.get("grad_hidden") is not None:
         gh = f64(r["grad_hidden"])
         assert np.all(gh[~live] == 0)                          # masked rows are exact zeros

@@ -10,3 +10,5 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a B200 (run with -m gpu on the GPU box)")
+    config.addinivalue_line("markers", "slow: full-size oracle comparisons that take minutes of host time (part of -m gpu; "
+                                       "deselect with -m 'gpu and not slow')")

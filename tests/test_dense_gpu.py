@@ -110,24 +110,54 @@ def test_dense_kl_super_tiles_fwd_only_and_zero_case(handle, monkeypatch):
     assert none["loss"].item() == 0 and not none["grad_W"].any() and not none["grad_hidden"].any()
 
 
-def test_dense_kl_at_C3_shape_sampled_rows(handle):
-    """T=16384 (varlen mask), d=2048, dT=4096, V=151936: per-token values and grad_hidden rows of sampled tokens against the
-    oracle, grad_W through its identities (column sums 0; <W, grad_W>_k = <x, grad_hidden>_k)."""
+def _dense_C3_check(handle, reverse, n_live_target=None):
+    """T=16384 (varlen mask), d=2048, dT=4096, V=151936: per-token values and whole grad_hidden rows of sampled tokens against
+    the oracle, grad_W element by element on >= 256 vocabulary columns (random ones, tile edges, the last partial vocabulary
+    tile) against oracle.dense_grad_W_columns, and the per-k identity <W, grad_W>_k = <x, grad_hidden>_k."""
+    from paper_2606_24143_b200 import opd
     cfg = synth.CONFIGS[3]
     T, d, V, dT = cfg["T"], cfg["d"], cfg["V"], 4096
     X, W, XT, WT, _ = make("bf16", T, d, dT, V, 3, masked=False)
     mask = synth.make_mask(cfg, 3, DEV)
-    r = handle.dense_kl_fwd_bwd(X, W, XT, WT, mask)
+    if n_live_target is not None:                                 # scattered subset of the live rows (bounds the oracle's time)
+        live0 = torch.nonzero(mask).flatten()
+        keep = live0[torch.randperm(live0.numel(), generator=torch.Generator().manual_seed(3))[:n_live_target].to(DEV)]
+        mask = torch.zeros_like(mask)
+        mask[keep] = 1
+    r = handle.dense_kl_fwd_bwd(X, W, XT, WT, mask, flags=opd.F_DENSE_REVERSE if reverse else 0)
     torch.cuda.synchronize()
     live = np.flatnonzero(f64(mask))
-    rows = np.sort(np.random.default_rng(5).choice(live, 10, replace=False))
+    rng = np.random.default_rng(5)
+    rows = np.sort(rng.choice(live, 10, replace=False))
     sel = torch.as_tensor(rows, device=DEV)
-    ref = O.dense_kl_oracle(f64(X[sel]), f64(W), f64(XT[sel]), f64(WT), np.ones(len(rows)), norm_override=float(live.size))
+    ref = O.dense_kl_oracle(f64(X[sel]), f64(W), f64(XT[sel]), f64(WT), np.ones(len(rows)), norm_override=float(live.size),
+                            reverse=reverse)
     assert np.abs(f64(r["per_token_kl"][sel]) - ref["per_token_kl"]).max() <= LOSS_RTOL * np.abs(ref["per_token_kl"]).max()
     check_grad(f64(r["grad_hidden"][sel]), ref["grad_hidden"], "bf16", "grad_hidden rows")
     assert abs(r["loss"].item() - r["per_token_kl"].double().sum().item() / live.size) <= 1e-5 * abs(r["loss"].item())
     gw, gh = r["grad_W"], r["grad_hidden"]
-    assert gw.double().sum(dim=1).abs().max().item() <= 1e-2 * gw.abs().max().item() * np.sqrt(V)
+    dead = mask == 0
+    assert not gh[dead].any() and not r["per_token_kl"][dead].any()
     lhs = (W.double() * gw.double()).sum(dim=1)
     rhs = (X.double() * gh.double()).sum(dim=0)
     assert (lhs - rhs).abs().max().item() <= 2e-2 * lhs.abs().max().item()
+    cols = np.unique(np.concatenate([rng.choice(V, 160, replace=False), np.arange(V - V % 256, V), [0, 255, 256, 4095, 4096, 8191]]))
+    assert cols.size >= 256
+    want = O.dense_grad_W_columns(f64(X), f64(W), f64(XT), f64(WT), f64(mask), cols, reverse=reverse)
+    got = f64(gw[:, torch.as_tensor(cols, device=DEV)])
+    check_grad(got, want, "bf16", f"dense grad_W[:, {cols.size} columns], reverse={reverse}")
+    col_scale = np.maximum(np.abs(want).max(axis=0), 1e-3 * np.abs(want).max())
+    assert (np.abs(got - want).max(axis=0) <= 4 * GRAD_TOL["bf16"] * col_scale).all()
+
+
+@pytest.mark.slow
+def test_dense_kl_at_C3_shape_forward(handle):
+    """Eq.(1) at the C3 shape with its own variable-length mask (about 10.9k live rows)."""
+    _dense_C3_check(handle, reverse=False)
+
+
+@pytest.mark.slow
+def test_dense_kl_at_C3_shape_reverse(handle):
+    """OPD_F_DENSE_REVERSE (Eq.(2),(3)) at the C3 shape: three launches, fp32 log-q ring; 6144 scattered live
+    rows (two token super-tiles)."""
+    _dense_C3_check(handle, reverse=True, n_live_target=6144)

@@ -683,3 +683,42 @@ def test_dense_two_head_reverse_kl_pins():
         assert abs((f(t["X"], Wp) - f(t["X"], Wm)) / (2 * h) - r["grad_W"][ki, vi]) < 2e-8
     # the two directions differ (a swapped-roles mistake would show)
     assert abs(O.dense_kl_oracle(t["X"], t["W"], XT, WT, t["mask"])["loss"] - r["loss"]) > 1e-3
+
+
+# ---------------------------------------------------------------- column-restricted gradients used by the full-size GPU checks
+@pytest.mark.parametrize("mode", [O.RKL_MC, O.MIXED])
+def test_grad_W_columns_with_surrogates_equals_the_full_oracle(mode):
+    """grad_W_columns(surrogate=s) is opd_oracle(surrogate=s)["grad_W"][:, cols] for the four surrogates of Eq.(6),(7)
+    (PAPER.md:132-141), on a stale cache (rho far from 1) where the four gradients really differ from one another."""
+    mask = [2, 1, 0, 2, 2, 1, 2, 2] if mode == O.MIXED else [1, 1, 0, 1, 1, 1, 1, 1]
+    t = tiny(41, T=8, d=5, V=11, C=4, dup=True, mask=mask)
+    old = t["old"] + np.random.default_rng(5).normal(size=t["old"].shape) * 0.6        # heavy importance-ratio tails
+    kk = (3 | (4 << 16)) if mode == O.MIXED else 4
+    cols = [0, 3, int(t["idx"][0, 0]), int(t["idx"][3, 1]), 10]
+    seen = []
+    for sur in (O.SUR_THETA_NOCLIP, O.SUR_THETA_CLIP, O.SUR_OLD_NOCLIP, O.SUR_OLD_CLIP):
+        full = O.opd_oracle(t["X"], t["W"], t["idx"], t["lam"], old, t["mask"], mode, kk, surrogate=sur, norm_override=3.0)
+        gc = O.grad_W_columns(t["X"], t["W"], t["idx"], t["lam"], old, t["mask"], mode, kk, cols, surrogate=sur, norm_override=3.0,
+                              chunk=3)
+        np.testing.assert_allclose(gc, full["grad_W"][:, cols], atol=1e-13)
+        seen.append(gc)
+    for i in range(4):
+        for j in range(i + 1, 4):
+            assert np.abs(seen[i] - seen[j]).max() > 1e-3          # a dropped `surrogate` argument would not pass
+
+
+@pytest.mark.parametrize("reverse", [False, True])
+def test_dense_grad_W_columns_equals_the_full_dense_oracle(reverse):
+    """dense_grad_W_columns is dense_kl_oracle(...)["grad_W"][:, cols] in both directions (Eq.(1) / Eq.(2),(3)),
+    with masked rows, a normaliser override and a chunk size that does not divide the live count."""
+    rng = np.random.default_rng(43)
+    T, d, dT, V = 9, 5, 7, 13
+    X, XT = rng.normal(size=(T, d)), rng.normal(size=(T, dT))
+    W, WT = rng.normal(size=(d, V)) / math.sqrt(d), rng.normal(size=(dT, V)) / math.sqrt(dT)
+    mask = np.array([1, 1, 0, 1, 1, 1, 0, 1, 1])
+    cols = [0, 5, 12, 7]
+    full = O.dense_kl_oracle(X, W, XT, WT, mask, norm_override=4.0, reverse=reverse)
+    gc = O.dense_grad_W_columns(X, W, XT, WT, mask, cols, norm_override=4.0, chunk=4, reverse=reverse)
+    np.testing.assert_allclose(gc, full["grad_W"][:, cols], atol=1e-13)
+    other = O.dense_grad_W_columns(X, W, XT, WT, mask, cols, norm_override=4.0, reverse=not reverse)
+    assert np.abs(gc - other).max() > 1e-3                          # the two directions are not interchangeable

@@ -7,8 +7,10 @@ directly, and (ii) grad_W is checked through properties that hold at any size:
    sum_v W[k,v] grad_W[k,v] = sum_t x[t,k] grad_hidden[t,k]   for every k   (both equal <z, G> split by k)
 plus (iii) a few-live-token variant of the 1.7B-class shape where the oracle computes grad_W in full, and (iv) grad_W element by
 element on >= 256 vocabulary columns at the full T / d / V of C3, C4 and C5 (oracle.grad_W_columns: every live token contributes to
-every column, so the oracle runs one fp64 forward over all live tokens; C3 keeps its own variable-length mask, C4 and C5 use a
-scattered subset of live tokens that still spans several token super-tiles so that the check finishes in about a minute)."""
+every column, so the oracle runs one fp64 forward over all live tokens; C3 keeps its own variable-length mask, C4 runs with all
+32 768 tokens live and C5 with 32 768 of its 65 536, so that at least 8 token super-tiles reduce into every grad_W panel as in the
+timed configuration; these two are marked `slow`: the oracle needs minutes of host time).  C4's staleness sweep (sigma = 0 / 0.1)
+and the surrogate flags are covered on sampled rows and on grad_W columns of a thinned mask."""
 import numpy as np
 import pytest
 import torch
@@ -27,13 +29,32 @@ def handle():
     return opd.Handle(0)
 
 
-def sampled_check(handle, cfg, c, mode, n_rows=12, layout="dv"):
-    inp = synth.make_inputs(cfg, c=c, device=DEV)
+def _surrogate(flags):
+    """OPD_F_SUR_CLIP (64) / OPD_F_SUR_A_OLD (128) -> the oracle's surrogate code (Eq.(6),(7) PAPER.md:132-141)."""
+    return {0: O.SUR_THETA_NOCLIP, 64: O.SUR_THETA_CLIP, 128: O.SUR_OLD_NOCLIP, 192: O.SUR_OLD_CLIP}[flags & 192]
+
+
+def sampled_check(handle, cfg, c, mode, n_rows=12, layout="dv", sigma=None, flags=0, rho_is_one=False):
+    """sigma: staleness of the rollout policy (None = the config's); flags: surrogate flags; rho_is_one: the cache was scored by
+    the current weights (sigma = 0), so every importance ratio the kernel forms must be 1 to 1e-4 (checked on ALL live slots
+    through opd_set_diagnostics, not on a sample)."""
+    inp = synth.make_inputs(cfg, c=c, device=DEV, sigma=sigma)
     if layout == "vd":                                       # the same logical [d,V] matrix stored [V,d] like lm_head.weight
         inp["W"] = inp["W"].t().contiguous().t()
     idx, lam, old, kk = pick(inp, cfg, mode)
-    r = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, want_lse=True, want_student_logp=True)
-    torch.cuda.synchronize()
+    rho = torch.full(tuple(idx.shape), float("nan"), device=DEV) if rho_is_one else None
+    if rho is not None:
+        handle.set_diagnostics(rho_out=rho)
+    try:
+        r = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, flags=flags, want_lse=True,
+                                want_student_logp=True)
+        torch.cuda.synchronize()
+    finally:
+        if rho is not None:
+            handle.set_diagnostics(None, None)
+    if rho is not None:
+        lv = rho[inp["mask"] != 0]
+        assert not torch.isnan(lv).any() and float((lv - 1.0).abs().max()) <= 1e-4
     mask = f64(inp["mask"])
     live = np.flatnonzero(mask)
     rng = np.random.default_rng(c)
@@ -43,7 +64,7 @@ def sampled_check(handle, cfg, c, mode, n_rows=12, layout="dv"):
     sub = dict(hidden=inp["hidden"][sel], W=inp["W"], mask=inp["mask"][sel])
     # the oracle on the sampled rows only, with the normaliser of the whole call
     ref = O.opd_oracle(f64(sub["hidden"]), W, f64(idx[sel]), f64(lam[sel]), f64(old[sel]) if old is not None else None,
-                       f64(sub["mask"]), mode, kk, norm_override=float(live.size), want_grad_W=False)
+                       f64(sub["mask"]), mode, kk, norm_override=float(live.size), want_grad_W=False, surrogate=_surrogate(flags))
     assert np.abs(f64(r["lse"][sel]) - ref["lse"]).max() <= LOGP_ATOL
     a, b = f64(r["student_logp"][sel]), ref["student_logp"]
     used = ~np.isnan(b)
@@ -72,7 +93,7 @@ def sampled_check(handle, cfg, c, mode, n_rows=12, layout="dv"):
     # pair claims a tile (a race between a tile's stores and its publication would show up here first)
     keep = (r["loss"].clone(), gh.clone(), gw.clone())
     del r, gh, gw
-    r2 = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk)
+    r2 = handle.loss_fwd_bwd(inp["hidden"], inp["W"], idx, lam, old, inp["mask"], mode, kk, flags=flags)
     torch.cuda.synchronize()
     assert torch.equal(keep[0], r2["loss"]) and torch.equal(keep[1], r2["grad_hidden"]) and torch.equal(keep[2], r2["grad_W"])
 
@@ -89,6 +110,14 @@ def test_C3_shape_sampled_vd_storage(handle):
 
 def test_C4_shape_sampled(handle):
     sampled_check(handle, synth.CONFIGS[4], 4, O.RKL_MC)
+
+
+def test_C4_staleness_sweep_is_parity_tested(handle):
+    """BASELINE.json configs[3]: "staleness sweep with W_old perturbation 0.0/0.02/0.1" (0.02 is test_C4_shape_sampled).
+    sigma = 0: the cache holds the current student's own log-probs, so rho = 1 on every live slot (to 1e-4) and the sampled rows
+    match the oracle; sigma = 0.1 (p99 of rho about 1.26: the clip bites) with the clipped A_old surrogate, sampled rows."""
+    sampled_check(handle, synth.CONFIGS[4], 4, O.RKL_MC, sigma=0.0, rho_is_one=True)
+    sampled_check(handle, synth.CONFIGS[4], 4, O.RKL_MC, sigma=0.1, flags=192)
 
 
 def test_C5_shape_sampled_mixed(handle):
@@ -158,8 +187,8 @@ def _columns_for(idx, live, V, rng, n_tok=16, n_rand=96):
     return np.unique(np.concatenate([cached, rng.choice(V, n_rand, replace=False), tail, [0, 255, 256, 4095, 4096]]))
 
 
-def grad_W_column_check(handle, cfg, c, mode, n_live_target=None, layout="dv", flags=0):
-    inp = synth.make_inputs(cfg, c=c, device=DEV)
+def grad_W_column_check(handle, cfg, c, mode, n_live_target=None, layout="dv", flags=0, sigma=None):
+    inp = synth.make_inputs(cfg, c=c, device=DEV, sigma=sigma)
     T, V = cfg["T"], cfg["V"]
     if n_live_target is not None:        # scattered subset of the live tokens (the mode codes of OPD_MIXED are kept)
         live0 = torch.nonzero(inp["mask"] != 0).flatten()
@@ -178,7 +207,7 @@ def grad_W_column_check(handle, cfg, c, mode, n_live_target=None, layout="dv", f
     cols = _columns_for(idx, live, V, np.random.default_rng(100 + c))
     assert cols.size >= 256
     ref = O.grad_W_columns(f64(inp["hidden"]), f64(inp["W"]), f64(idx), f64(lam), f64(old) if old is not None else None, mask,
-                           mode, kk, cols)
+                           mode, kk, cols, surrogate=_surrogate(flags))
     got = f64(r["grad_W"][:, torch.as_tensor(cols, device=DEV)])
     # the bar is relative to the largest entry of the compared columns (they hold the cached columns, where grad_W peaks)
     check_grad(got, ref, "bf16", f"grad_W[:, {cols.size} columns] at {cfg['name']}")
@@ -194,11 +223,24 @@ def test_C3_grad_W_columns_full_mask(handle):
     grad_W_column_check(handle, synth.CONFIGS[3], 3, O.FKL_TOPK, layout="vd")
 
 
-def test_C4_grad_W_columns(handle):
-    """C4 (T=32768, d=4096, V=151936): 6144 scattered live tokens (two token super-tiles, all 38 vocabulary super-tiles)."""
-    grad_W_column_check(handle, synth.CONFIGS[4], 4, O.RKL_MC, n_live_target=6144)
+def test_C4_grad_W_columns_surrogate_thinned(handle):
+    """C4 (T=32768, d=4096, V=151936) with sigma = 0.1 and the clipped A_old surrogate (flags 192): 6144 scattered live tokens
+    (two token super-tiles, all vocabulary super-tiles), grad_W columns element by element."""
+    grad_W_column_check(handle, synth.CONFIGS[4], 4, O.RKL_MC, n_live_target=6144, flags=192, sigma=0.1)
 
 
+@pytest.mark.slow
+def test_C4_grad_W_columns_all_tokens_live(handle):
+    """The configuration bench.py times, unthinned: all 32 768 tokens live, so each grad_W panel is the sum of the 8 token
+    super-tiles' reduce-add passes.  >= 256 columns (cached columns, random ones, the last partial vocabulary tile) element by
+    element.  The oracle's fp64 forward over 32 768 x 151 936 logits takes about two minutes of host time."""
+    r, inp = grad_W_column_check(handle, synth.CONFIGS[4], 4, O.RKL_MC)
+    assert int((inp["mask"] != 0).sum()) == 32768 and 32768 // handle.launch_stats()["super_rows"] >= 8
+
+
+@pytest.mark.slow
 def test_C5_grad_W_columns_mixed(handle):
-    """C5 (T=65536, d=2560, V=151936, mixed FKL k=64 / MC K=8 rows): 8192 scattered live tokens."""
-    grad_W_column_check(handle, synth.CONFIGS[5], 5, O.MIXED, n_live_target=8192)
+    """C5 (T=65536, d=2560, V=151936, mixed FKL k=64 / MC K=8 rows): 32 768 scattered live tokens over all 16 token super-tiles
+    (>= 8 of them reduce into each panel)."""
+    r, inp = grad_W_column_check(handle, synth.CONFIGS[5], 5, O.MIXED, n_live_target=32768)
+    assert 65536 // handle.launch_stats()["super_rows"] >= 8

@@ -166,6 +166,60 @@ def test_stress_variants(handle, variant, dtype, mode):
     compare_all(r, ref, f64(inp["mask"]), dtype)
 
 
+def stale_clip_inputs(dtype, mode):
+    """A stale cache on which the PPO clip is active on both sides with advantages of both signs, without the extreme ratios
+    that would let a few slots dominate the max-abs bar: the rollout-time log-probs are placed at fixed distances from the
+    current student's (rho = exp(shift), shift in {+-0.9, +-0.45, +0.05, -0.07}: 2.46, 0.41, 1.57, 0.64, 1.05, 0.93 -- none
+    near a clip edge, so fp64 and the kernel's fp32 take the same branch), and the teacher scores around both
+    (lam = (ell + old)/2 + 0.8 N(0,1), seeded).  `ell` comes from the oracle's forward.  Returns the inputs, the caches, a
+    boolean [T,K] array of the live Monte-Carlo slots and ell on them."""
+    cfg = dict(RAGGED, dtype=dtype, T=520, V=4360, K=8)
+    inp = synth.make_inputs(cfg, c=11, device=DEV)
+    if mode == O.MIXED:
+        m = inp["mask"].clone()
+        m[(torch.arange(cfg["T"], device=DEV) % 3 != 0) & (m != 0)] = 2
+        inp["mask"] = m
+    idx, lam, old, kk = pick(inp, cfg, mode)
+    Km = kk >> 16 if mode == O.MIXED else kk
+    mk = f64(inp["mask"])
+    slots = np.zeros(tuple(idx.shape), dtype=bool)
+    slots[(mk == 2) if mode == O.MIXED else (mk != 0), :Km] = True
+    ell = oracle_for(inp, idx, lam, old, mode, kk, want_grads=False)["student_logp"]
+    rng = np.random.default_rng(77)
+    shift = rng.choice(np.array([0.9, -0.9, 0.45, -0.45, 0.05, -0.07]), size=slots.shape)
+    old64 = np.where(slots, ell - shift, f64(old))
+    lam64 = np.where(slots, 0.5 * (ell + old64) + 0.8 * rng.normal(size=slots.shape), f64(lam))   # FKL rows keep their teacher cache
+    old = torch.as_tensor(old64, dtype=torch.float32, device=DEV)
+    lam = torch.as_tensor(lam64, dtype=torch.float32, device=DEV)
+    return inp, idx, lam, old, kk, slots, np.where(slots, ell, np.nan)
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "fp32"])
+@pytest.mark.parametrize("mode", [O.RKL_MC, O.MIXED])
+@pytest.mark.parametrize("flags", [64, 128, 192])
+def test_surrogates_reach_every_clip_corner(handle, dtype, mode, flags):
+    """OPD_F_SUR_CLIP / OPD_F_SUR_A_OLD (Eq.(4); Eq.(6),(7) PAPER.md:132-141; eps = 0.2 PAPER.md:330) on inputs where
+    the clip is active on both sides with advantages of both signs: before comparing, the oracle's rho and A must put at least
+    8 live slots into each of the four corners (rho > 1.2 | rho < 0.8) x (A > 0 | A < 0), for the advantage the flag selects."""
+    inp, idx, lam, old, kk, slots, ell = stale_clip_inputs(dtype, mode)
+    rho = np.exp(ell - f64(old))
+    A = (f64(lam) - f64(old)) if flags & 128 else (f64(lam) - ell)
+    for hi in (True, False):
+        for pos in (True, False):
+            n = int((slots & ((rho > 1.2) if hi else (rho < 0.8)) & ((A > 0) if pos else (A < 0))).sum())
+            assert n >= 8, (hi, pos, n)
+    assert np.nanmin(np.abs(np.abs(rho - 1.0) - 0.2)) > 0.1                   # no slot near a clip edge
+    r = run(handle, inp, idx, lam, old, mode, kk, flags)
+    ref = oracle_for(inp, idx, lam, old, mode, kk, flags)
+    compare_all(r, ref, f64(inp["mask"]), dtype)
+    # discriminating power: the other three surrogates give gradients that differ from this one by many times the bar, so a
+    # kernel that dropped the clip, clipped the wrong side or took the other advantage could not pass
+    for other_flags in ({0, 64, 128, 192} - {flags}):
+        other = oracle_for(inp, idx, lam, old, mode, kk, other_flags, want_grad_W=False)
+        gap = np.abs(other["grad_hidden"] - ref["grad_hidden"]).max() / np.abs(ref["grad_hidden"]).max()
+        assert gap > 10 * GRAD_TOL[dtype], (other_flags, gap)
+
+
 def test_degenerate_cases(handle, opd):
     cfg = dict(RAGGED, T=130, k=64, K=64)
     inp = synth.make_inputs(cfg, c=8, device=DEV)
